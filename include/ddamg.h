@@ -1,0 +1,180 @@
+/*
+ * ddamg.h -- C ABI of libddamg.so: the finest-level hot path of DD-alphaAMG as
+ * extended by arXiv:2407.08092, hand-written for NVIDIA B200 (sm_100a).
+ *
+ * The path (PAPER.md = /root/reference/PAPER.md, the paper's text):
+ *   * odd-even reordering of D x = b                        eq. 1
+ *   * Schur factorisation of D^-1                           eq. 2
+ *   * Schur complement  D_S = D_ee - D_eo D_oo^-1 D_oe      eq. 3
+ *   * modified Richardson on D_S x_e = bhat_e               Alg. 4
+ *   * restarted GMRES(n, m) on D_S x_e = bhat_e             Alg. 2
+ *   * "odd-even + {GMRES, Richardson}": whole lattice reordered, iteration runs on the
+ *     Schur system
+ * D is the Wilson-clover operator with 12 d.o.f. per site;
+ * D_ee, D_oo are block diagonal with 6x6 blocks and D_oo^-1 is stored.
+ * The paper never writes D down; DESIGN.md lists the readings (gamma basis, hopping
+ * normalisation, clover leaves, boundary condition) this library and the oracle use:
+ *   D = A + H,  A(x) = (m0+4) - (csw/32) sum_{mu!=nu} gamma_mu gamma_nu (x) F'_munu(x),
+ *   (H psi)(x) = -1/2 sum_mu [(1-gamma_mu) U_mu(x) psi(x+mu) + (1+gamma_mu) U_mu(x-mu)^H psi(x-mu)].
+ *
+ * Conventions
+ *   * One context = one lattice, one precision, one CUDA stream, one GPU (the current
+ *     device at ddamg_create).  No multi-GPU sharding, no collectives.
+ *   * "natural" layout (external): site n = x + L*(y + L*(z + L*t)); complex numbers are
+ *     (re, im) pairs of the context precision unless an argument says otherwise.
+ *       gauge   U[n][mu][row][col]      mu = 0..3 = x,y,z,t       (72 reals / site)
+ *       spinor  psi[n][spin][colour]                              (24 reals / site)
+ *   * "native" layout (internal, checkerboarded SoA): a half-lattice spinor of parity p
+ *     holds the V/2 sites with (x+y+z+t) mod 2 == p (even = 0) at
+ *     checkerboard index cb = n >> 1, as 24/NV planes of V/2 16-byte vectors
+ *     (NV = 4 floats or 2 doubles); plane j holds reals NV*j .. NV*j+NV-1 of the site's
+ *     24 reals (spin-major, then colour, then re/im).  Size: 12*V complex = 24*(V/2) reals.
+ *     Callers obtain native buffers only through ddamg_pack_spinor / ddamg_unpack_spinor;
+ *     every x_e / x_o / b_e / b_o argument below is a DEVICE pointer to such a buffer,
+ *     16-byte aligned, of ddamg_half_spinor_bytes() bytes, owned by the caller.
+ *   * All work is enqueued on the context's stream.  Functions that return a residual
+ *     history synchronise that stream once before returning; the others are asynchronous.
+ *   * Every function returns DDAMG_OK (0) or a negative status and never aborts, exits
+ *     or throws.  A CUDA error is sticky: all later calls return DDAMG_ECUDA until
+ *     ddamg_destroy.  ddamg_last_error() gives a human-readable message.
+ *   * There is no CPU fallback: without a CUDA device ddamg_create returns DDAMG_ECUDA.
+ */
+#ifndef DDAMG_H
+#define DDAMG_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ddamg_ctx ddamg_ctx;   /* opaque; owns all internal device memory */
+
+enum {
+    DDAMG_OK = 0,
+    DDAMG_EINVAL = -1,     /* bad argument (null pointer, odd L/T, nu < 0, k < 1, ...) */
+    DDAMG_ENOMEM = -2,     /* device or host allocation failed                        */
+    DDAMG_ESTATE = -3,     /* call out of order (no gauge loaded / clover not built)  */
+    DDAMG_ECUDA = -4,      /* CUDA runtime error (sticky)                             */
+    DDAMG_ESINGULAR = -5   /* a 6x6 clover block is numerically singular              */
+};
+enum { DDAMG_F32 = 0, DDAMG_F64 = 1 };
+enum { DDAMG_BC_PERIODIC = 0, DDAMG_BC_ANTIPERIODIC_T = 1 };
+
+/* Library version string, e.g. "ddamg-b200 0.1 (sm_100a)". Never NULL. */
+const char* ddamg_version(void);
+
+/*
+ * Create a context for an L^3 x T lattice (L, T even, >= 2; L^3*T/2 < 2^31).
+ *   csw, m0   clover coefficient and bare mass of D (Table 5 names them)
+ *   bc        DDAMG_BC_PERIODIC or DDAMG_BC_ANTIPERIODIC_T (time links of slice T-1 negated)
+ *   prec      DDAMG_F32 or DDAMG_F64: precision of every stored field and of every
+ *             spinor argument (reductions always accumulate in fp64)
+ *   cuda_stream  a cudaStream_t (host value) or NULL for the legacy default stream
+ * On success *out is a new context (caller destroys it).  EINVAL / ENOMEM / ECUDA.
+ */
+int ddamg_create(ddamg_ctx** out, int L, int T, double csw, double m0, int bc, int prec,
+                 void* cuda_stream);
+
+/* Free everything the context owns (synchronises its stream first). NULL is a no-op. */
+int ddamg_destroy(ddamg_ctx* ctx);
+
+/* Message of the last failure on this context ("" if none).  ctx may be NULL. */
+const char* ddamg_last_error(ddamg_ctx* ctx);
+
+/* Bytes of one native half-lattice spinor = 24 * (V/2) * sizeof(real).  0 if ctx is NULL. */
+size_t ddamg_half_spinor_bytes(ddamg_ctx* ctx);
+
+/*
+ * Load the gauge field (step a0).  U: natural layout, u_prec = DDAMG_F32/F64 complex,
+ * HOST pointer if on_device == 0 (copied with cudaMemcpyAsync, then the stream is
+ * synchronised), DEVICE pointer otherwise.  The field is rounded to the context
+ * precision, repacked per parity and direction, and the antiperiodic sign is folded into
+ * the time links of slice T-1.  The caller keeps U.  Invalidates a previously built clover.
+ */
+int ddamg_load_gauge(ddamg_ctx* ctx, const void* U, int u_prec, int on_device);
+
+/*
+ * Build the clover term (step a1) from the loaded links: per site the two Hermitian 6x6
+ * blocks of A(x), computed in fp64, stored in the context precision;
+ * A itself is kept on even sites, its INVERSE on odd sites ("explicitly storing the data
+ * for D_oo^-1 is cheap").  Synchronises.  ESTATE without a gauge field; ESINGULAR if an
+ * odd-site block has a pivot below 1e-12 * (largest entry of the block).
+ */
+int ddamg_build_clover(ddamg_ctx* ctx);
+
+/* eq. 3:  y_e = D_S x_e = A_ee x_e - H_eo A_oo^-1 H_oe x_e.   y_e must not alias x_e. */
+int ddamg_apply_schur(ddamg_ctx* ctx, const void* x_e, void* y_e);
+
+/*
+ * Alg. 4 with omega supplied (lines 2-4):  nu times  r = b_e - D_S x_e;  x_e += omega r.
+ *   x_e        in: x^(0) (ignored if zero_init != 0, then x^(0) = 0 and the first sweep is
+ *              x = omega b_e without an operator application); out: x^(nu).  In place.
+ *   res_hist   HOST array of nu doubles or NULL; res_hist[i] = || b_e - D_S x^(i) ||_2,
+ *              i = 0..nu-1 (by-product of sweep i+1).  NULL skips the reductions and the
+ *              stream synchronisation.
+ * EINVAL if nu < 0 or b_e aliases x_e.
+ */
+int ddamg_richardson(ddamg_ctx* ctx, const void* b_e, void* x_e, int nu, double omega,
+                     int zero_init, double* res_hist);
+
+/*
+ * Alg. 2: restarted GMRES(n = cycles, m = k) on D_S x_e = b_e.
+ *   x_e        in: x^(0) (ignored if zero_init); out: the final iterate.
+ *   tol        0: run all cycles*k steps (smoother use); > 0: stop as soon as the Givens
+ *              residual estimate <= tol * ||b_e|| (checked on the host every step)
+ *   res_hist   HOST array of cycles*(k+1)+1 doubles or NULL: for each cycle the true
+ *              ||b_e - D_S x|| at its start followed by the k residual estimates, then the
+ *              true residual norm at the end.  *n_hist (may be NULL) = entries written.
+ * Orthogonalisation: classical Gram-Schmidt in two fused passes (one multi-dot, one
+ * multi-axpy + norm), partial sums in fp64 (reading R15).
+ * EINVAL if k < 1, cycles < 1 or b_e aliases x_e.  ENOMEM if the Krylov basis
+ * ((k+1) half spinors) cannot be allocated.
+ */
+int ddamg_gmres_oe(ddamg_ctx* ctx, const void* b_e, void* x_e, int k, int cycles, double tol,
+                   int zero_init, double* res_hist, int* n_hist);
+
+/* eq. 2, left factor:  x_o = A_oo^-1 (b_o - H_oe x_e). */
+int ddamg_reconstruct_odd(ddamg_ctx* ctx, const void* b_o, const void* x_e, void* x_o);
+
+/* eq. 2, right factor: bhat_e = b_e - H_eo A_oo^-1 b_o.   bhat_e may alias b_e. */
+int ddamg_prepare_rhs(ddamg_ctx* ctx, const void* b_e, const void* b_o, void* bhat_e);
+
+/*
+ * Alg. 4 line 1: a few power iterations for |lambda_max(D_S)| starting from v_e
+ * (overwritten).  *lambda_max (HOST) = ||D_S v|| / ||v|| of the last iteration.  Synchronises.
+ */
+int ddamg_power_iteration(ddamg_ctx* ctx, void* v_e, int iters, double* lambda_max);
+
+/* natural (DEVICE, context precision, full lattice) -> native halves.  x_e or x_o may be NULL. */
+int ddamg_pack_spinor(ddamg_ctx* ctx, const void* nat, void* x_e, void* x_o);
+/* native halves -> natural (DEVICE).  A NULL half writes zeros on that parity. */
+int ddamg_unpack_spinor(ddamg_ctx* ctx, const void* x_e, const void* x_o, void* nat);
+
+/*
+ * Debug / parity: the stored clover blocks as dense matrices, natural site order, DEVICE
+ * buffers of V*2*6*6 complex numbers of the context precision ([n][block][row][col],
+ * block 0 = spins 0,1, block 1 = spins 2,3, row = 3*(spin mod 2) + colour).
+ *   A_nat     A(x) blocks on even sites, zeros on odd sites  (may be NULL)
+ *   Ainv_nat  A(x)^-1 blocks on odd sites, zeros on even     (may be NULL)
+ */
+int ddamg_get_clover(ddamg_ctx* ctx, void* A_nat, void* Ainv_nat);
+
+/* Number of kernel launches this context has enqueued since creation (bench accounting). */
+long long ddamg_launch_count(ddamg_ctx* ctx);
+
+/*
+ * Time the kernels of the last ddamg_apply_schur / ddamg_richardson call pattern:
+ * when enabled (on != 0) every hot-path kernel launch is bracketed by CUDA events on the
+ * context's stream; ddamg_kernel_time_ms returns the accumulated device time (ms) and the
+ * number of launches of kernel class `which` (0 = kernel A: A_oo^-1 H_oe, 1 = kernel B /
+ * B': A_ee x - H_eo t with optional Richardson update) since the last reset, after
+ * synchronising the stream.  Used by bench.py for the per-kernel roofline.
+ */
+int ddamg_kernel_timing(ddamg_ctx* ctx, int on);
+int ddamg_kernel_time_ms(ddamg_ctx* ctx, int which, double* ms, long long* launches, int reset);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DDAMG_H */

@@ -1,0 +1,569 @@
+// ddamg_api.cu -- the C ABI of include/ddamg.h: context, state machine, launch order.
+//
+// Host orchestration only: every arithmetic step of the path runs in the kernels of
+// ddamg_dslash.cu / ddamg_setup.cu / ddamg_blas.cu.  Nothing here touches spinor data on the
+// host, and there is no CPU fallback.
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/ddamg.h"
+#include "ddamg_internal.h"
+
+using namespace ddamg;
+
+struct ddamg_ctx {
+    Geom g;
+    double csw, m0;
+    int bc, prec;
+    cudaStream_t stream;
+    size_t real_bytes;
+    size_t half_bytes;          // one native half spinor
+    size_t nreal;               // reals per half spinor = 24 * Vh
+    void* gauge;                // [parity][mu] link blocks
+    void* clov[2];              // [0] = A_ee blocks, [1] = A_oo^-1 blocks
+    void* tmp_o;                // t_o of eq. 3
+    void* tmp_e;                // scratch half spinor (power iteration, final residual)
+    void* krylov;               // (kcap + 1) half spinors
+    int kcap;
+    double* partials;           // reduction scratch
+    size_t partials_len;
+    Scalars* sc;                // device scalars
+    double* host_hist;          // pinned
+    int* singular;              // device flag
+    bool have_gauge, have_clover;
+    int sticky;                 // DDAMG_OK or DDAMG_ECUDA
+    long long launches;
+    std::string err;
+    // optional per-kernel timing
+    bool timing;
+    struct Ev { cudaEvent_t a, b; int which; };
+    std::vector<Ev> events;
+};
+
+static thread_local std::string g_err_noctx;
+
+static int fail(ddamg_ctx* c, int code, const std::string& msg)
+{
+    if (c) {
+        c->err = msg;
+        if (code == DDAMG_ECUDA) c->sticky = DDAMG_ECUDA;
+    } else {
+        g_err_noctx = msg;
+    }
+    return code;
+}
+
+static int check_cuda(ddamg_ctx* c, cudaError_t e, const char* what)
+{
+    if (e == cudaSuccess) return DDAMG_OK;
+    return fail(c, DDAMG_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
+}
+
+#define CK(expr)                                                     \
+    do {                                                             \
+        int _s = check_cuda(ctx, (expr), #expr);                     \
+        if (_s != DDAMG_OK) return _s;                               \
+    } while (0)
+
+#define ENTER(ctx)                                                           \
+    do {                                                                     \
+        if (!(ctx)) return DDAMG_EINVAL;                                     \
+        if ((ctx)->sticky != DDAMG_OK) return (ctx)->sticky;                 \
+    } while (0)
+
+static int after_launch(ddamg_ctx* ctx, int n = 1)
+{
+    ctx->launches += n;
+    return check_cuda(ctx, cudaGetLastError(), "kernel launch");
+}
+
+static void* gauge_block(ddamg_ctx* c, int parity)
+{
+    return (char*)c->gauge + (size_t)parity * 4 * 18 * c->g.Vh * c->real_bytes;
+}
+
+extern "C" const char* ddamg_version(void) { return "ddamg-b200 0.1 (sm_100a)"; }
+
+extern "C" const char* ddamg_last_error(ddamg_ctx* ctx) { return ctx ? ctx->err.c_str() : g_err_noctx.c_str(); }
+
+extern "C" size_t ddamg_half_spinor_bytes(ddamg_ctx* ctx) { return ctx ? ctx->half_bytes : 0; }
+
+extern "C" long long ddamg_launch_count(ddamg_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+extern "C" int ddamg_create(ddamg_ctx** out, int L, int T, double csw, double m0, int bc, int prec, void* cuda_stream)
+{
+    if (!out) return fail(nullptr, DDAMG_EINVAL, "ddamg_create: out is NULL");
+    *out = nullptr;
+    if (L < 2 || T < 2 || (L & 1) || (T & 1)) return fail(nullptr, DDAMG_EINVAL, "ddamg_create: L and T must be even and >= 2");
+    if (bc != DDAMG_BC_PERIODIC && bc != DDAMG_BC_ANTIPERIODIC_T) return fail(nullptr, DDAMG_EINVAL, "ddamg_create: bad bc");
+    if (prec != DDAMG_F32 && prec != DDAMG_F64) return fail(nullptr, DDAMG_EINVAL, "ddamg_create: bad prec");
+    const double vh = 0.5 * (double)L * L * L * T;
+    if (vh >= 1073741824.0) return fail(nullptr, DDAMG_EINVAL, "ddamg_create: lattice too large");
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+        cudaGetLastError();
+        return fail(nullptr, DDAMG_ECUDA, "ddamg_create: no CUDA device (there is no CPU fallback)");
+    }
+    ddamg_ctx* ctx = new (std::nothrow) ddamg_ctx();
+    if (!ctx) return fail(nullptr, DDAMG_ENOMEM, "ddamg_create: host allocation failed");
+    ctx->g.L = L; ctx->g.T = T; ctx->g.Lh = L / 2;
+    ctx->g.Vh = (int)vh;
+    ctx->g.sy = ctx->g.Lh; ctx->g.sz = ctx->g.Lh * L; ctx->g.st = ctx->g.Lh * L * L;
+    ctx->csw = csw; ctx->m0 = m0; ctx->bc = bc; ctx->prec = prec;
+    ctx->stream = (cudaStream_t)cuda_stream;
+    ctx->real_bytes = prec == DDAMG_F32 ? 4 : 8;
+    ctx->nreal = (size_t)24 * ctx->g.Vh;
+    ctx->half_bytes = ctx->nreal * ctx->real_bytes;
+    ctx->gauge = ctx->clov[0] = ctx->clov[1] = ctx->tmp_o = ctx->tmp_e = ctx->krylov = nullptr;
+    ctx->kcap = 0;
+    ctx->partials = nullptr; ctx->sc = nullptr; ctx->host_hist = nullptr; ctx->singular = nullptr;
+    ctx->have_gauge = ctx->have_clover = false;
+    ctx->sticky = DDAMG_OK; ctx->launches = 0; ctx->timing = false;
+
+    const size_t gauge_bytes = (size_t)2 * 4 * 18 * ctx->g.Vh * ctx->real_bytes;
+    const size_t clov_bytes = (size_t)72 * ctx->g.Vh * ctx->real_bytes;
+    const int dgrid = dslash_grid(ctx->g);
+    const int bgrid = blas_grid(ctx->nreal / 2);
+    ctx->partials_len = (size_t)(dgrid > bgrid * 2 * MDOT_NB ? dgrid : bgrid * 2 * MDOT_NB);
+    cudaError_t e = cudaSuccess;
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->gauge, gauge_bytes);
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->clov[0], clov_bytes);
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->clov[1], clov_bytes);
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->tmp_o, ctx->half_bytes);
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->tmp_e, ctx->half_bytes);
+    if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->partials, ctx->partials_len * sizeof(double));
+    if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->sc, sizeof(Scalars));
+    if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->singular, sizeof(int));
+    if (e == cudaSuccess) e = cudaMallocHost((void**)&ctx->host_hist, sizeof(double) * (HIST_MAX + 8));
+    if (e == cudaSuccess) e = cudaMemsetAsync(ctx->sc, 0, sizeof(Scalars), ctx->stream);
+    if (e != cudaSuccess) {
+        const int code = (e == cudaErrorMemoryAllocation) ? DDAMG_ENOMEM : DDAMG_ECUDA;
+        fail(nullptr, code, std::string("ddamg_create: ") + cudaGetErrorString(e));
+        cudaGetLastError();
+        ddamg_destroy(ctx);
+        return code;
+    }
+    *out = ctx;
+    return DDAMG_OK;
+}
+
+extern "C" int ddamg_destroy(ddamg_ctx* ctx)
+{
+    if (!ctx) return DDAMG_OK;
+    cudaStreamSynchronize(ctx->stream);
+    for (auto& ev : ctx->events) { cudaEventDestroy(ev.a); cudaEventDestroy(ev.b); }
+    cudaFree(ctx->gauge); cudaFree(ctx->clov[0]); cudaFree(ctx->clov[1]);
+    cudaFree(ctx->tmp_o); cudaFree(ctx->tmp_e); cudaFree(ctx->krylov);
+    cudaFree(ctx->partials); cudaFree(ctx->sc); cudaFree(ctx->singular);
+    if (ctx->host_hist) cudaFreeHost(ctx->host_hist);
+    cudaGetLastError();
+    delete ctx;
+    return DDAMG_OK;
+}
+
+// --------------------------------------------------------------------------- setup
+extern "C" int ddamg_load_gauge(ddamg_ctx* ctx, const void* U, int u_prec, int on_device)
+{
+    ENTER(ctx);
+    if (!U) return fail(ctx, DDAMG_EINVAL, "ddamg_load_gauge: U is NULL");
+    if (u_prec != DDAMG_F32 && u_prec != DDAMG_F64) return fail(ctx, DDAMG_EINVAL, "ddamg_load_gauge: bad u_prec");
+    const size_t in_bytes = (size_t)2 * ctx->g.Vh * 72 * (u_prec == DDAMG_F32 ? 4 : 8);
+    const void* src = U;
+    void* staging = nullptr;
+    if (!on_device) {
+        cudaError_t e = cudaMalloc(&staging, in_bytes);
+        if (e != cudaSuccess) { cudaGetLastError(); return fail(ctx, DDAMG_ENOMEM, "ddamg_load_gauge: staging allocation failed"); }
+        int s = check_cuda(ctx, cudaMemcpyAsync(staging, U, in_bytes, cudaMemcpyHostToDevice, ctx->stream), "gauge H2D");
+        if (s != DDAMG_OK) { cudaFree(staging); return s; }
+        src = staging;
+    }
+    if (ctx->prec == DDAMG_F32) {
+        if (u_prec == DDAMG_F32) launch_pack_gauge<float, float>(ctx->g, ctx->bc, src, ctx->gauge, ctx->stream);
+        else launch_pack_gauge<double, float>(ctx->g, ctx->bc, src, ctx->gauge, ctx->stream);
+    } else {
+        if (u_prec == DDAMG_F32) launch_pack_gauge<float, double>(ctx->g, ctx->bc, src, ctx->gauge, ctx->stream);
+        else launch_pack_gauge<double, double>(ctx->g, ctx->bc, src, ctx->gauge, ctx->stream);
+    }
+    int s = after_launch(ctx);
+    if (staging) {
+        int s2 = check_cuda(ctx, cudaStreamSynchronize(ctx->stream), "gauge sync");
+        cudaFree(staging);
+        if (s == DDAMG_OK) s = s2;
+    }
+    if (s != DDAMG_OK) return s;
+    ctx->have_gauge = true;
+    ctx->have_clover = false;
+    return DDAMG_OK;
+}
+
+extern "C" int ddamg_build_clover(ddamg_ctx* ctx)
+{
+    ENTER(ctx);
+    if (!ctx->have_gauge) return fail(ctx, DDAMG_ESTATE, "ddamg_build_clover: no gauge field loaded");
+    CK(cudaMemsetAsync(ctx->singular, 0, sizeof(int), ctx->stream));
+    if (ctx->prec == DDAMG_F32)
+        launch_build_clover<float>(ctx->g, ctx->csw, ctx->m0, ctx->gauge, ctx->clov[0], ctx->clov[1], ctx->singular, ctx->stream);
+    else
+        launch_build_clover<double>(ctx->g, ctx->csw, ctx->m0, ctx->gauge, ctx->clov[0], ctx->clov[1], ctx->singular, ctx->stream);
+    int s = after_launch(ctx);
+    if (s != DDAMG_OK) return s;
+    int flag = 0;
+    CK(cudaMemcpyAsync(&flag, ctx->singular, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    if (flag) return fail(ctx, DDAMG_ESINGULAR, "ddamg_build_clover: a 6x6 odd-site block is numerically singular");
+    ctx->have_clover = true;
+    return DDAMG_OK;
+}
+
+extern "C" int ddamg_pack_spinor(ddamg_ctx* ctx, const void* nat, void* x_e, void* x_o)
+{
+    ENTER(ctx);
+    if (!nat || (!x_e && !x_o)) return fail(ctx, DDAMG_EINVAL, "ddamg_pack_spinor: NULL argument");
+    if (ctx->prec == DDAMG_F32) launch_pack_spinor<float>(ctx->g, nat, x_e, x_o, ctx->stream);
+    else launch_pack_spinor<double>(ctx->g, nat, x_e, x_o, ctx->stream);
+    return after_launch(ctx);
+}
+
+extern "C" int ddamg_unpack_spinor(ddamg_ctx* ctx, const void* x_e, const void* x_o, void* nat)
+{
+    ENTER(ctx);
+    if (!nat) return fail(ctx, DDAMG_EINVAL, "ddamg_unpack_spinor: nat is NULL");
+    if (ctx->prec == DDAMG_F32) launch_unpack_spinor<float>(ctx->g, x_e, x_o, nat, ctx->stream);
+    else launch_unpack_spinor<double>(ctx->g, x_e, x_o, nat, ctx->stream);
+    return after_launch(ctx);
+}
+
+extern "C" int ddamg_get_clover(ddamg_ctx* ctx, void* A_nat, void* Ainv_nat)
+{
+    ENTER(ctx);
+    if (!ctx->have_clover) return fail(ctx, DDAMG_ESTATE, "ddamg_get_clover: clover not built");
+    if (!A_nat && !Ainv_nat) return fail(ctx, DDAMG_EINVAL, "ddamg_get_clover: both outputs NULL");
+    if (ctx->prec == DDAMG_F32) launch_get_clover<float>(ctx->g, ctx->clov[0], ctx->clov[1], A_nat, Ainv_nat, ctx->stream);
+    else launch_get_clover<double>(ctx->g, ctx->clov[0], ctx->clov[1], A_nat, Ainv_nat, ctx->stream);
+    return after_launch(ctx);
+}
+
+// --------------------------------------------------------------------------- hot path
+// One fused hopping launch.  parity = parity of the output sites.
+static int dslash(ddamg_ctx* ctx, int epi, bool norm, int parity, const void* in, const void* own, const void* rhs,
+                  void* out, double omega, int which)
+{
+    ddamg_ctx::Ev ev;
+    if (ctx->timing) {
+        if (cudaEventCreate(&ev.a) != cudaSuccess || cudaEventCreate(&ev.b) != cudaSuccess)
+            return check_cuda(ctx, cudaGetLastError(), "cudaEventCreate");
+        ev.which = which;
+        cudaEventRecord(ev.a, ctx->stream);
+    }
+    if (ctx->prec == DDAMG_F32)
+        launch_dslash<float>(ctx->g, epi, norm, parity, in, gauge_block(ctx, parity), gauge_block(ctx, 1 - parity),
+                             ctx->clov[parity], own, rhs, out, omega, ctx->partials, ctx->stream);
+    else
+        launch_dslash<double>(ctx->g, epi, norm, parity, in, gauge_block(ctx, parity), gauge_block(ctx, 1 - parity),
+                              ctx->clov[parity], own, rhs, out, omega, ctx->partials, ctx->stream);
+    if (ctx->timing) {
+        cudaEventRecord(ev.b, ctx->stream);
+        ctx->events.push_back(ev);
+    }
+    return after_launch(ctx);
+}
+
+static int need_ready(ddamg_ctx* ctx, const char* who)
+{
+    if (!ctx->have_gauge || !ctx->have_clover)
+        return fail(ctx, DDAMG_ESTATE, std::string(who) + ": load the gauge field and build the clover term first");
+    return DDAMG_OK;
+}
+
+// y_e = D_S x_e  (kernel A then kernel B)
+static int schur(ddamg_ctx* ctx, const void* x_e, void* y_e)
+{
+    int s = dslash(ctx, EPI_CLOV_HOP, false, 1, x_e, nullptr, nullptr, ctx->tmp_o, 0.0, 0);
+    if (s != DDAMG_OK) return s;
+    return dslash(ctx, EPI_SCHUR, false, 0, ctx->tmp_o, x_e, nullptr, y_e, 0.0, 1);
+}
+
+extern "C" int ddamg_apply_schur(ddamg_ctx* ctx, const void* x_e, void* y_e)
+{
+    ENTER(ctx);
+    if (!x_e || !y_e || x_e == y_e) return fail(ctx, DDAMG_EINVAL, "ddamg_apply_schur: NULL or aliased arguments");
+    int s = need_ready(ctx, "ddamg_apply_schur");
+    if (s != DDAMG_OK) return s;
+    return schur(ctx, x_e, y_e);
+}
+
+static int copy_hist(ddamg_ctx* ctx, double* dst, int n, int* n_out)
+{
+    // nhist, then the entries
+    CK(cudaMemcpyAsync(ctx->host_hist, (char*)ctx->sc + offsetof(Scalars, hist), sizeof(double) * n, cudaMemcpyDeviceToHost, ctx->stream));
+    int nh = 0;
+    CK(cudaMemcpyAsync(&nh, (char*)ctx->sc + offsetof(Scalars, nhist), sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    if (nh > n) nh = n;
+    if (dst) memcpy(dst, ctx->host_hist, sizeof(double) * nh);
+    if (n_out) *n_out = nh;
+    return DDAMG_OK;
+}
+
+static int reset_hist(ddamg_ctx* ctx)
+{
+    return check_cuda(ctx, cudaMemsetAsync((char*)ctx->sc + offsetof(Scalars, nhist), 0, sizeof(int), ctx->stream), "reset hist");
+}
+
+template <typename T>
+static void t_axpy_norm(ddamg_ctx* ctx, double alpha, const void* x, void* y, double* partials)
+{
+    launch_axpy_norm<T>(ctx->nreal, alpha, x, y, partials, ctx->stream);
+}
+
+extern "C" int ddamg_richardson(ddamg_ctx* ctx, const void* b_e, void* x_e, int nu, double omega, int zero_init,
+                                double* res_hist)
+{
+    ENTER(ctx);
+    if (!b_e || !x_e || b_e == x_e || nu < 0) return fail(ctx, DDAMG_EINVAL, "ddamg_richardson: bad arguments");
+    if (res_hist && nu > HIST_MAX) return fail(ctx, DDAMG_EINVAL, "ddamg_richardson: nu exceeds the history capacity");
+    int s = need_ready(ctx, "ddamg_richardson");
+    if (s != DDAMG_OK) return s;
+    const bool hist = res_hist != nullptr;
+    if (hist) { s = reset_hist(ctx); if (s != DDAMG_OK) return s; }
+    int done = 0;
+    if (zero_init && nu > 0) {
+        // x^(0) = 0:  r = b,  x^(1) = omega b  (no operator application; Alg. 4 line 3-4)
+        if (ctx->prec == DDAMG_F32) t_axpy_norm<float>(ctx, omega, b_e, x_e, hist ? ctx->partials : nullptr);
+        else t_axpy_norm<double>(ctx, omega, b_e, x_e, hist ? ctx->partials : nullptr);
+        s = after_launch(ctx);
+        if (s != DDAMG_OK) return s;
+        if (hist) { launch_finalize_norm(ctx->partials, blas_grid(ctx->nreal / (16 / ctx->real_bytes)), ctx->sc, 1, ctx->stream); s = after_launch(ctx); if (s != DDAMG_OK) return s; }
+        done = 1;
+    } else if (zero_init) {
+        CK(cudaMemsetAsync(x_e, 0, ctx->half_bytes, ctx->stream));
+    }
+    for (int i = done; i < nu; ++i) {
+        s = dslash(ctx, EPI_CLOV_HOP, false, 1, x_e, nullptr, nullptr, ctx->tmp_o, 0.0, 0);        // kernel A
+        if (s != DDAMG_OK) return s;
+        s = dslash(ctx, EPI_RICHARDSON, hist, 0, ctx->tmp_o, x_e, b_e, x_e, omega, 1);              // kernel B'
+        if (s != DDAMG_OK) return s;
+        if (hist) {
+            launch_finalize_norm(ctx->partials, dslash_grid(ctx->g), ctx->sc, 1, ctx->stream);
+            s = after_launch(ctx);
+            if (s != DDAMG_OK) return s;
+        }
+    }
+    if (hist && nu > 0) return copy_hist(ctx, res_hist, nu, nullptr);
+    return DDAMG_OK;
+}
+
+extern "C" int ddamg_reconstruct_odd(ddamg_ctx* ctx, const void* b_o, const void* x_e, void* x_o)
+{
+    ENTER(ctx);
+    if (!b_o || !x_e || !x_o) return fail(ctx, DDAMG_EINVAL, "ddamg_reconstruct_odd: NULL argument");
+    int s = need_ready(ctx, "ddamg_reconstruct_odd");
+    if (s != DDAMG_OK) return s;
+    return dslash(ctx, EPI_CLOV_RHS_MINUS_HOP, false, 1, x_e, nullptr, b_o, x_o, 0.0, 2);
+}
+
+extern "C" int ddamg_prepare_rhs(ddamg_ctx* ctx, const void* b_e, const void* b_o, void* bhat_e)
+{
+    ENTER(ctx);
+    if (!b_e || !b_o || !bhat_e) return fail(ctx, DDAMG_EINVAL, "ddamg_prepare_rhs: NULL argument");
+    int s = need_ready(ctx, "ddamg_prepare_rhs");
+    if (s != DDAMG_OK) return s;
+    if (ctx->prec == DDAMG_F32) launch_clover_apply<float>(ctx->g, ctx->clov[1], b_o, ctx->tmp_o, ctx->stream);     // t_o = A_oo^-1 b_o
+    else launch_clover_apply<double>(ctx->g, ctx->clov[1], b_o, ctx->tmp_o, ctx->stream);
+    s = after_launch(ctx);
+    if (s != DDAMG_OK) return s;
+    return dslash(ctx, EPI_RHS_MINUS_HOP, false, 0, ctx->tmp_o, nullptr, b_e, bhat_e, 0.0, 2);         // b_e - H_eo t_o
+}
+
+// --------------------------------------------------------------------------- GMRES
+template <typename T>
+static int gmres_impl(ddamg_ctx* ctx, const void* b_e, void* x_e, int k, int cycles, double tol, int zero_init,
+                      double* res_hist, int* n_hist)
+{
+    cudaStream_t st = ctx->stream;
+    const size_t nreal = ctx->nreal;
+    const int vecN = (int)(16 / ctx->real_bytes);
+    const int bgrid = blas_grid(nreal / vecN);
+    const int dgrid = dslash_grid(ctx->g);
+    char* V = (char*)ctx->krylov;
+    auto Vj = [&](int j) { return (void*)(V + (size_t)j * ctx->half_bytes); };
+    double* coef_y = (double*)((char*)ctx->sc + offsetof(Scalars, y));
+    double* coef_negh = (double*)((char*)ctx->sc + offsetof(Scalars, negh));
+    double* scale = (double*)((char*)ctx->sc + offsetof(Scalars, scale));
+    int s = reset_hist(ctx);
+    if (s != DDAMG_OK) return s;
+    double bnorm = 0.0;
+    if (tol > 0.0) {
+        launch_copy_norm<T>(nreal, b_e, Vj(0), ctx->partials, st);
+        launch_finalize_norm(ctx->partials, bgrid, ctx->sc, 0, st);
+        s = after_launch(ctx, 2); if (s != DDAMG_OK) return s;
+        CK(cudaMemcpyAsync(&bnorm, (char*)ctx->sc + offsetof(Scalars, value), sizeof(double), cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+    }
+    if (zero_init) CK(cudaMemsetAsync(x_e, 0, ctx->half_bytes, st));
+    bool converged = false;
+    for (int c = 0; c < cycles && !converged; ++c) {
+        // line 2: r = b - D_S x, beta = ||r||
+        if (zero_init && c == 0) {
+            launch_copy_norm<T>(nreal, b_e, Vj(0), ctx->partials, st);
+            s = after_launch(ctx); if (s != DDAMG_OK) return s;
+            launch_finalize_norm(ctx->partials, bgrid, ctx->sc, 1, st);
+        } else {
+            s = dslash(ctx, EPI_CLOV_HOP, false, 1, x_e, nullptr, nullptr, ctx->tmp_o, 0.0, 0);
+            if (s != DDAMG_OK) return s;
+            s = dslash(ctx, EPI_RESIDUAL, true, 0, ctx->tmp_o, x_e, b_e, Vj(0), 0.0, 1);
+            if (s != DDAMG_OK) return s;
+            launch_finalize_norm(ctx->partials, dgrid, ctx->sc, 1, st);
+        }
+        launch_gmres_begin_cycle(ctx->sc, st);
+        launch_scale_by_dev<T>(nreal, Vj(0), scale, st);                 // v_1 = r / beta
+        s = after_launch(ctx, 3); if (s != DDAMG_OK) return s;
+        if (tol > 0.0) {
+            double beta = 0.0;
+            CK(cudaMemcpyAsync(&beta, (char*)ctx->sc + offsetof(Scalars, value), sizeof(double), cudaMemcpyDeviceToHost, st));
+            CK(cudaStreamSynchronize(st));
+            if (beta <= tol * bnorm) { converged = true; break; }
+        }
+        int m = 0;
+        for (int j = 0; j < k; ++j) {
+            // line 5: w = D_S v_j  -> V[j+1]
+            s = schur(ctx, Vj(j), Vj(j + 1));
+            if (s != DDAMG_OK) return s;
+            // lines 6-7 (fused classical Gram-Schmidt): h_ij = <v_i, w>, i = 0..j
+            for (int i0 = 0; i0 <= j; i0 += MDOT_NB) {
+                const int nb = (j + 1 - i0) < MDOT_NB ? (j + 1 - i0) : MDOT_NB;
+                launch_multi_dot<T>(nreal, nb, Vj(i0), nreal, Vj(j + 1), ctx->partials, st);
+                launch_finalize_dots(ctx->partials, bgrid, nb, ctx->sc, i0, st);
+                s = after_launch(ctx, 2); if (s != DDAMG_OK) return s;
+            }
+            // w -= sum_i h_ij v_i ; line 8: h_{j+1,j} = ||w||
+            for (int i0 = 0; i0 <= j; i0 += MDOT_NB) {
+                const int nb = (j + 1 - i0) < MDOT_NB ? (j + 1 - i0) : MDOT_NB;
+                const bool last = i0 + MDOT_NB > j;
+                launch_multi_axpy<T>(nreal, nb, Vj(i0), nreal, coef_negh + 2 * i0, Vj(j + 1), last ? ctx->partials : nullptr, st);
+                s = after_launch(ctx); if (s != DDAMG_OK) return s;
+            }
+            launch_finalize_norm(ctx->partials, bgrid, ctx->sc, 0, st);
+            launch_gmres_givens(ctx->sc, j, st);
+            launch_scale_by_dev<T>(nreal, Vj(j + 1), scale, st);         // v_{j+1} = w / h_{j+1,j}
+            s = after_launch(ctx, 3); if (s != DDAMG_OK) return s;
+            m = j + 1;
+            if (tol > 0.0) {
+                int nh = 0;
+                CK(cudaMemcpyAsync(&nh, (char*)ctx->sc + offsetof(Scalars, nhist), sizeof(int), cudaMemcpyDeviceToHost, st));
+                CK(cudaStreamSynchronize(st));
+                double est = 0.0;
+                CK(cudaMemcpyAsync(&est, (char*)ctx->sc + offsetof(Scalars, hist) + sizeof(double) * (nh - 1), sizeof(double), cudaMemcpyDeviceToHost, st));
+                CK(cudaStreamSynchronize(st));
+                if (est <= tol * bnorm) break;
+            }
+        }
+        // line 10: y = argmin, x += V_m y
+        launch_gmres_solve(ctx->sc, m, st);
+        s = after_launch(ctx); if (s != DDAMG_OK) return s;
+        for (int i0 = 0; i0 < m; i0 += MDOT_NB) {
+            const int nb = (m - i0) < MDOT_NB ? (m - i0) : MDOT_NB;
+            launch_multi_axpy<T>(nreal, nb, Vj(i0), nreal, coef_y + 2 * i0, x_e, nullptr, st);
+            s = after_launch(ctx); if (s != DDAMG_OK) return s;
+        }
+    }
+    if (!converged) {
+        // true residual at the end
+        s = dslash(ctx, EPI_CLOV_HOP, false, 1, x_e, nullptr, nullptr, ctx->tmp_o, 0.0, 0);
+        if (s != DDAMG_OK) return s;
+        s = dslash(ctx, EPI_RESIDUAL, true, 0, ctx->tmp_o, x_e, b_e, Vj(0), 0.0, 1);
+        if (s != DDAMG_OK) return s;
+        launch_finalize_norm(ctx->partials, dgrid, ctx->sc, 1, st);
+        s = after_launch(ctx); if (s != DDAMG_OK) return s;
+    }
+    return copy_hist(ctx, res_hist, cycles * (k + 1) + 1, n_hist);
+}
+
+extern "C" int ddamg_gmres_oe(ddamg_ctx* ctx, const void* b_e, void* x_e, int k, int cycles, double tol, int zero_init,
+                              double* res_hist, int* n_hist)
+{
+    ENTER(ctx);
+    if (!b_e || !x_e || b_e == x_e || k < 1 || cycles < 1 || tol < 0.0)
+        return fail(ctx, DDAMG_EINVAL, "ddamg_gmres_oe: bad arguments");
+    if (k > GMRES_KMAX) return fail(ctx, DDAMG_EINVAL, "ddamg_gmres_oe: k exceeds GMRES_KMAX (64)");
+    if ((long long)cycles * (k + 1) + 1 > HIST_MAX) return fail(ctx, DDAMG_EINVAL, "ddamg_gmres_oe: history too long");
+    int s = need_ready(ctx, "ddamg_gmres_oe");
+    if (s != DDAMG_OK) return s;
+    if (k > ctx->kcap) {
+        CK(cudaStreamSynchronize(ctx->stream));
+        cudaFree(ctx->krylov);
+        ctx->krylov = nullptr; ctx->kcap = 0;
+        cudaError_t e = cudaMalloc(&ctx->krylov, (size_t)(k + 1) * ctx->half_bytes);
+        if (e != cudaSuccess) { cudaGetLastError(); return fail(ctx, DDAMG_ENOMEM, "ddamg_gmres_oe: cannot allocate the Krylov basis"); }
+        ctx->kcap = k;
+    }
+    if (ctx->prec == DDAMG_F32) return gmres_impl<float>(ctx, b_e, x_e, k, cycles, tol, zero_init, res_hist, n_hist);
+    return gmres_impl<double>(ctx, b_e, x_e, k, cycles, tol, zero_init, res_hist, n_hist);
+}
+
+// --------------------------------------------------------------------------- power iteration
+extern "C" int ddamg_power_iteration(ddamg_ctx* ctx, void* v_e, int iters, double* lambda_max)
+{
+    ENTER(ctx);
+    if (!v_e || !lambda_max || iters < 1) return fail(ctx, DDAMG_EINVAL, "ddamg_power_iteration: bad arguments");
+    int s = need_ready(ctx, "ddamg_power_iteration");
+    if (s != DDAMG_OK) return s;
+    cudaStream_t st = ctx->stream;
+    const int vecN = (int)(16 / ctx->real_bytes);
+    const int bgrid = blas_grid(ctx->nreal / vecN);
+    double* scale = (double*)((char*)ctx->sc + offsetof(Scalars, scale));
+    const bool f32 = ctx->prec == DDAMG_F32;
+    // v <- v / ||v||
+    if (f32) launch_copy_norm<float>(ctx->nreal, v_e, v_e, ctx->partials, st);
+    else launch_copy_norm<double>(ctx->nreal, v_e, v_e, ctx->partials, st);
+    launch_finalize_norm(ctx->partials, bgrid, ctx->sc, 0, st);
+    if (f32) launch_scale_by_dev<float>(ctx->nreal, v_e, scale, st);
+    else launch_scale_by_dev<double>(ctx->nreal, v_e, scale, st);
+    s = after_launch(ctx, 3); if (s != DDAMG_OK) return s;
+    for (int i = 0; i < iters; ++i) {
+        s = schur(ctx, v_e, ctx->tmp_e);                                     // w = D_S v
+        if (s != DDAMG_OK) return s;
+        if (f32) launch_copy_norm<float>(ctx->nreal, ctx->tmp_e, v_e, ctx->partials, st);   // v = w, |w|^2
+        else launch_copy_norm<double>(ctx->nreal, ctx->tmp_e, v_e, ctx->partials, st);
+        launch_finalize_norm(ctx->partials, bgrid, ctx->sc, 0, st);          // lambda = ||w||
+        if (f32) launch_scale_by_dev<float>(ctx->nreal, v_e, scale, st);
+        else launch_scale_by_dev<double>(ctx->nreal, v_e, scale, st);
+        s = after_launch(ctx, 3); if (s != DDAMG_OK) return s;
+    }
+    CK(cudaMemcpyAsync(lambda_max, (char*)ctx->sc + offsetof(Scalars, value), sizeof(double), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    return DDAMG_OK;
+}
+
+// --------------------------------------------------------------------------- kernel timing
+extern "C" int ddamg_kernel_timing(ddamg_ctx* ctx, int on)
+{
+    ENTER(ctx);
+    ctx->timing = on != 0;
+    return DDAMG_OK;
+}
+
+extern "C" int ddamg_kernel_time_ms(ddamg_ctx* ctx, int which, double* ms, long long* launches, int reset)
+{
+    ENTER(ctx);
+    CK(cudaStreamSynchronize(ctx->stream));
+    double tot = 0.0;
+    long long n = 0;
+    for (auto& ev : ctx->events) {
+        if (ev.which != which) continue;
+        float t = 0.f;
+        CK(cudaEventElapsedTime(&t, ev.a, ev.b));
+        tot += t;
+        ++n;
+    }
+    if (ms) *ms = tot;
+    if (launches) *launches = n;
+    if (reset) {
+        for (auto& ev : ctx->events) { cudaEventDestroy(ev.a); cudaEventDestroy(ev.b); }
+        ctx->events.clear();
+    }
+    return DDAMG_OK;
+}

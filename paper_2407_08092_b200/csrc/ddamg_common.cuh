@@ -1,0 +1,161 @@
+// ddamg_common.cuh -- geometry, native (checkerboard SoA) layout and vector access.
+//
+// Native layout:
+//   * site of parity p with coordinates (x,y,z,t):  cb = (x>>1) + Lh*(y + L*(z + L*t)),
+//     Lh = L/2  (== natural index >> 1 because L is even and x is fastest)
+//   * half-lattice spinor: 24/NV planes of Vh 16-byte vectors, plane j = reals NV*j..
+//   * gauge: per (parity, mu) one block of 18*Vh reals holding U_mu(x) for the Vh sites of
+//     that parity: fp32 = 4 planes of float4 (reals 0..15) + 1 plane of float2 (reals 16,17);
+//     fp64 = 9 planes of double2; reals are row-major (row, col, re/im)
+//   * clover: per parity 2 blocks/site, each block 36 reals = 6 real diagonal entries then
+//     the 15 complex strictly-lower entries (1,0),(2,0),(2,1),(3,0),...,(5,4); stored as
+//     72/NV planes of Vh vectors (block 0 first)
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace ddamg {
+
+struct Geom {
+    int L, T, Lh;        // Lh = L/2
+    int Vh;              // sites per parity
+    int sy, sz, st;      // cb strides of +1 in y, z, t:  Lh, Lh*L, Lh*L*L
+};
+
+template <typename T> struct VecOf;
+template <> struct VecOf<float>  { using type = float4;  static constexpr int N = 4; };
+template <> struct VecOf<double> { using type = double2; static constexpr int N = 2; };
+
+// ----------------------------------------------------------------- cache-hinted access
+// Spinor neighbours are re-read up to 8 times by different CTAs: keep them cacheable
+// (read-only path).  Gauge links and clover blocks are read exactly once per kernel:
+// stream them with an evict-first policy so that they do not push spinors out of L2.
+
+__device__ __forceinline__ float4 ld_reuse(const float4* p) { return __ldg(p); }
+__device__ __forceinline__ double2 ld_reuse(const double2* p) { return __ldg(p); }
+__device__ __forceinline__ float4 ld_stream(const float4* p) { return __ldcs(p); }
+__device__ __forceinline__ float2 ld_stream(const float2* p) { return __ldcs(p); }
+__device__ __forceinline__ double2 ld_stream(const double2* p) { return __ldcs(p); }
+
+__device__ __forceinline__ void unpack(const float4& v, float* r) { r[0] = v.x; r[1] = v.y; r[2] = v.z; r[3] = v.w; }
+__device__ __forceinline__ void unpack(const double2& v, double* r) { r[0] = v.x; r[1] = v.y; }
+__device__ __forceinline__ float4 pack(const float* r) { return make_float4(r[0], r[1], r[2], r[3]); }
+__device__ __forceinline__ double2 pack(const double* r) { return make_double2(r[0], r[1]); }
+
+// 24 reals of one site of a native half-lattice spinor
+template <typename T, bool STREAM = false>
+__device__ __forceinline__ void load_spinor(const T* __restrict__ base, int Vh, int cb, T (&s)[24])
+{
+    using V = typename VecOf<T>::type;
+    constexpr int N = VecOf<T>::N;
+    const V* p = reinterpret_cast<const V*>(base) + cb;
+#pragma unroll
+    for (int k = 0; k < 24 / N; ++k) {
+        V v = STREAM ? ld_stream(p + (size_t)k * Vh) : ld_reuse(p + (size_t)k * Vh);
+        unpack(v, &s[k * N]);
+    }
+}
+
+template <typename T>
+__device__ __forceinline__ void store_spinor(T* __restrict__ base, int Vh, int cb, const T (&s)[24])
+{
+    using V = typename VecOf<T>::type;
+    constexpr int N = VecOf<T>::N;
+    V* p = reinterpret_cast<V*>(base) + cb;
+#pragma unroll
+    for (int k = 0; k < 24 / N; ++k) p[(size_t)k * Vh] = pack(&s[k * N]);
+}
+
+// 18 reals of one link; blk = start of the (parity, mu) block
+__device__ __forceinline__ void load_link(const float* __restrict__ blk, int Vh, int cb, float (&u)[18])
+{
+    const float4* p4 = reinterpret_cast<const float4*>(blk) + cb;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) unpack(ld_stream(p4 + (size_t)k * Vh), &u[4 * k]);
+    const float2 v = ld_stream(reinterpret_cast<const float2*>(blk + (size_t)16 * Vh) + cb);
+    u[16] = v.x; u[17] = v.y;
+}
+__device__ __forceinline__ void load_link(const double* __restrict__ blk, int Vh, int cb, double (&u)[18])
+{
+    const double2* p = reinterpret_cast<const double2*>(blk) + cb;
+#pragma unroll
+    for (int k = 0; k < 9; ++k) unpack(ld_stream(p + (size_t)k * Vh), &u[2 * k]);
+}
+__device__ __forceinline__ void store_link(float* __restrict__ blk, int Vh, int cb, const float (&u)[18])
+{
+    float4* p4 = reinterpret_cast<float4*>(blk) + cb;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) p4[(size_t)k * Vh] = pack(&u[4 * k]);
+    reinterpret_cast<float2*>(blk + (size_t)16 * Vh)[cb] = make_float2(u[16], u[17]);
+}
+__device__ __forceinline__ void store_link(double* __restrict__ blk, int Vh, int cb, const double (&u)[18])
+{
+    double2* p = reinterpret_cast<double2*>(blk) + cb;
+#pragma unroll
+    for (int k = 0; k < 9; ++k) p[(size_t)k * Vh] = pack(&u[2 * k]);
+}
+
+// 36 reals of clover block b (0/1) of one site
+template <typename T>
+__device__ __forceinline__ void load_clover_block(const T* __restrict__ base, int Vh, int cb, int b, T (&c)[36])
+{
+    using V = typename VecOf<T>::type;
+    constexpr int N = VecOf<T>::N;
+    const V* p = reinterpret_cast<const V*>(base) + (size_t)b * (36 / N) * Vh + cb;
+#pragma unroll
+    for (int k = 0; k < 36 / N; ++k) unpack(ld_stream(p + (size_t)k * Vh), &c[k * N]);
+}
+template <typename T>
+__device__ __forceinline__ void store_clover_block(T* __restrict__ base, int Vh, int cb, int b, const T (&c)[36])
+{
+    using V = typename VecOf<T>::type;
+    constexpr int N = VecOf<T>::N;
+    V* p = reinterpret_cast<V*>(base) + (size_t)b * (36 / N) * Vh + cb;
+#pragma unroll
+    for (int k = 0; k < 36 / N; ++k) p[(size_t)k * Vh] = pack(&c[k * N]);
+}
+
+// ------------------------------------------------------------------------- geometry
+struct Site {
+    int xh, y, z, t;
+    int q;               // x & 1  == (y + z + t + parity) & 1
+};
+
+__device__ __forceinline__ Site site_of_cb(const Geom& g, int cb, int parity)
+{
+    Site s;
+    s.xh = cb % g.Lh;
+    int r = cb / g.Lh;
+    s.y = r % g.L;
+    r /= g.L;
+    s.z = r % g.L;
+    s.t = r / g.L;
+    s.q = (s.y + s.z + s.t + parity) & 1;
+    return s;
+}
+
+// checkerboard index (in the opposite-parity arrays) of the neighbour x + dir*mu_hat
+template <int MU, int DIR>
+__device__ __forceinline__ int neighbour_cb(const Geom& g, int cb, const Site& s)
+{
+    if (MU == 0) {
+        if (DIR > 0) {
+            if (s.q == 0) return cb;                               // x even: x+1 shares xh
+            return (s.xh == g.Lh - 1) ? cb - (g.Lh - 1) : cb + 1;
+        } else {
+            if (s.q == 1) return cb;                               // x odd: x-1 shares xh
+            return (s.xh == 0) ? cb + (g.Lh - 1) : cb - 1;
+        }
+    } else if (MU == 1) {
+        if (DIR > 0) return (s.y == g.L - 1) ? cb - (g.L - 1) * g.sy : cb + g.sy;
+        return (s.y == 0) ? cb + (g.L - 1) * g.sy : cb - g.sy;
+    } else if (MU == 2) {
+        if (DIR > 0) return (s.z == g.L - 1) ? cb - (g.L - 1) * g.sz : cb + g.sz;
+        return (s.z == 0) ? cb + (g.L - 1) * g.sz : cb - g.sz;
+    } else {
+        if (DIR > 0) return (s.t == g.T - 1) ? cb - (g.T - 1) * g.st : cb + g.st;
+        return (s.t == 0) ? cb + (g.T - 1) * g.st : cb - g.st;
+    }
+}
+
+}  // namespace ddamg

@@ -1,0 +1,170 @@
+// ddamg_dslash.cu -- the fused hopping + clover kernels of the Schur complement (eq. 3).
+//
+//   kernel A   t_o = A_oo^-1 (H_oe x_e)                         EPI_CLOV_HOP      (steps a2-a5)
+//   kernel B   y_e = A_ee x_e - H_eo t_o                         EPI_SCHUR         (step a6)
+//   kernel B'  r = b_e - (A_ee x_e - H_eo t_o); x_e += w r       EPI_RICHARDSON    (step a7)
+//              out = b_e - (A_ee x_e - H_eo t_o)  (+ ||out||^2)  EPI_RESIDUAL      (GMRES line 2)
+//              x_o = A_oo^-1 (b_o - H_oe x_e)                    EPI_CLOV_RHS_MINUS_HOP (eq. 2 left)
+//              bhat_e = b_e - H_eo t_o                           EPI_RHS_MINUS_HOP (eq. 2 right)
+//
+// One thread per output site; consecutive threads = consecutive checkerboard indices, so
+// every plane access of a warp is one contiguous 512-byte (16-byte vectors) run.
+#include "ddamg_internal.h"
+#include "ddamg_hop.cuh"
+
+namespace ddamg {
+
+template <typename T>
+struct DslashArgs {
+    Geom g;
+    int parity;              // parity of the output sites
+    const T* in;             // opposite-parity spinor (the 8 neighbours)
+    const T* gauge_own;      // 4 link blocks of the output parity
+    const T* gauge_opp;      // 4 link blocks of the opposite parity
+    const T* clov;           // clover blocks stored for the output parity
+    const T* own;            // own-site spinor (EPI_SCHUR / RICHARDSON / RESIDUAL)
+    const T* rhs;            // b (EPI_RICHARDSON / RESIDUAL / *_RHS_*)
+    T* out;
+    T omega;
+    double* partials;        // per-block sum of |r|^2 (NORM) or nullptr
+};
+
+__device__ __forceinline__ double block_sum(double v)
+{
+    __shared__ double warp_part[32];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    if (lane == 0) warp_part[w] = v;
+    __syncthreads();
+    const int nw = (blockDim.x + 31) >> 5;
+    v = (threadIdx.x < nw) ? warp_part[threadIdx.x] : 0.0;
+    if (w == 0) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    }
+    return v;     // valid in thread 0
+}
+
+template <typename T, int EPI, bool NORM>
+__global__ void __launch_bounds__(DSLASH_THREADS)
+dslash_kernel(const DslashArgs<T> a)
+{
+    const int cb = blockIdx.x * DSLASH_THREADS + threadIdx.x;
+    double nrm = 0.0;
+    if (cb < a.g.Vh) {
+        const Site s = site_of_cb(a.g, cb, a.parity);
+        T acc[24];
+        hop_site<T>(a.g, cb, s, a.in, a.gauge_own, a.gauge_opp, acc);
+        T res[24];
+        if (EPI == EPI_CLOV_HOP) {
+#pragma unroll
+            for (int i = 0; i < 24; ++i) acc[i] *= (T)(-0.5);
+            clover_site_mul<T>(a.clov, a.g.Vh, cb, acc, res);
+        } else if (EPI == EPI_CLOV_RHS_MINUS_HOP) {
+            T b[24];
+            load_spinor<T, true>(a.rhs, a.g.Vh, cb, b);
+#pragma unroll
+            for (int i = 0; i < 24; ++i) acc[i] = b[i] + (T)0.5 * acc[i];
+            clover_site_mul<T>(a.clov, a.g.Vh, cb, acc, res);
+        } else if (EPI == EPI_RHS_MINUS_HOP) {
+            T b[24];
+            load_spinor<T, true>(a.rhs, a.g.Vh, cb, b);
+#pragma unroll
+            for (int i = 0; i < 24; ++i) res[i] = b[i] + (T)0.5 * acc[i];
+        } else {
+            T x[24], ax[24];
+            load_spinor<T, true>(a.own, a.g.Vh, cb, x);
+            clover_site_mul<T>(a.clov, a.g.Vh, cb, x, ax);
+            if (EPI == EPI_SCHUR) {
+#pragma unroll
+                for (int i = 0; i < 24; ++i) res[i] = ax[i] + (T)0.5 * acc[i];     // A x - H t
+            } else {
+                T b[24];
+                load_spinor<T, true>(a.rhs, a.g.Vh, cb, b);
+#pragma unroll
+                for (int i = 0; i < 24; ++i) {
+                    const T r = b[i] - (ax[i] + (T)0.5 * acc[i]);
+                    if (NORM) nrm += (double)r * (double)r;
+                    res[i] = (EPI == EPI_RICHARDSON) ? x[i] + a.omega * r : r;
+                }
+            }
+        }
+        store_spinor<T>(a.out, a.g.Vh, cb, res);
+    }
+    if (NORM) {
+        const double tot = block_sum(nrm);
+        if (threadIdx.x == 0) a.partials[blockIdx.x] = tot;
+    }
+}
+
+template <typename T, int EPI, bool NORM>
+static void launch(const DslashArgs<T>& a, cudaStream_t st)
+{
+    const int grid = (a.g.Vh + DSLASH_THREADS - 1) / DSLASH_THREADS;
+    dslash_kernel<T, EPI, NORM><<<grid, DSLASH_THREADS, 0, st>>>(a);
+}
+
+template <typename T>
+void launch_dslash(const Geom& g, int epi, bool norm, int parity, const void* in, const void* gauge_own,
+                   const void* gauge_opp, const void* clov, const void* own, const void* rhs, void* out,
+                   double omega, double* partials, cudaStream_t st)
+{
+    DslashArgs<T> a;
+    a.g = g;
+    a.parity = parity;
+    a.in = (const T*)in;
+    a.gauge_own = (const T*)gauge_own;
+    a.gauge_opp = (const T*)gauge_opp;
+    a.clov = (const T*)clov;
+    a.own = (const T*)own;
+    a.rhs = (const T*)rhs;
+    a.out = (T*)out;
+    a.omega = (T)omega;
+    a.partials = partials;
+    switch (epi) {
+    case EPI_CLOV_HOP: launch<T, EPI_CLOV_HOP, false>(a, st); break;
+    case EPI_CLOV_RHS_MINUS_HOP: launch<T, EPI_CLOV_RHS_MINUS_HOP, false>(a, st); break;
+    case EPI_RHS_MINUS_HOP: launch<T, EPI_RHS_MINUS_HOP, false>(a, st); break;
+    case EPI_SCHUR: launch<T, EPI_SCHUR, false>(a, st); break;
+    case EPI_RICHARDSON:
+        if (norm) launch<T, EPI_RICHARDSON, true>(a, st);
+        else launch<T, EPI_RICHARDSON, false>(a, st);
+        break;
+    case EPI_RESIDUAL:
+        if (norm) launch<T, EPI_RESIDUAL, true>(a, st);
+        else launch<T, EPI_RESIDUAL, false>(a, st);
+        break;
+    }
+}
+
+template void launch_dslash<float>(const Geom&, int, bool, int, const void*, const void*, const void*, const void*,
+                                   const void*, const void*, void*, double, double*, cudaStream_t);
+template void launch_dslash<double>(const Geom&, int, bool, int, const void*, const void*, const void*, const void*,
+                                    const void*, const void*, void*, double, double*, cudaStream_t);
+
+// out = Cl in on one parity (right factor of eq. 2: t_o = A_oo^-1 b_o)
+template <typename T>
+__global__ void __launch_bounds__(DSLASH_THREADS)
+clover_apply_kernel(Geom g, const T* __restrict__ clov, const T* __restrict__ in, T* __restrict__ out)
+{
+    const int cb = blockIdx.x * DSLASH_THREADS + threadIdx.x;
+    if (cb >= g.Vh) return;
+    T v[24], res[24];
+    load_spinor<T, true>(in, g.Vh, cb, v);
+    clover_site_mul<T>(clov, g.Vh, cb, v, res);
+    store_spinor<T>(out, g.Vh, cb, res);
+}
+
+template <typename T>
+void launch_clover_apply(const Geom& g, const void* clov, const void* in, void* out, cudaStream_t st)
+{
+    const int grid = (g.Vh + DSLASH_THREADS - 1) / DSLASH_THREADS;
+    clover_apply_kernel<T><<<grid, DSLASH_THREADS, 0, st>>>(g, (const T*)clov, (const T*)in, (T*)out);
+}
+template void launch_clover_apply<float>(const Geom&, const void*, const void*, void*, cudaStream_t);
+template void launch_clover_apply<double>(const Geom&, const void*, const void*, void*, cudaStream_t);
+
+int dslash_grid(const Geom& g) { return (g.Vh + DSLASH_THREADS - 1) / DSLASH_THREADS; }
+
+}  // namespace ddamg

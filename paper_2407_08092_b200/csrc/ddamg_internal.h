@@ -1,0 +1,84 @@
+// ddamg_internal.h -- declarations shared by the translation units of libddamg.so.
+#pragma once
+#include <cuda_runtime.h>
+#include <stddef.h>
+#include "ddamg_common.cuh"
+
+namespace ddamg {
+
+constexpr int DSLASH_THREADS = 128;
+constexpr int BLAS_THREADS = 256;
+constexpr int GMRES_KMAX = 64;          // largest cycle length m of GMRES(n, m)
+constexpr int HIST_MAX = 8192;         // residual-history entries kept on the device
+constexpr int MDOT_NB = 8;              // basis vectors handled per fused multi-dot / multi-axpy pass
+
+// epilogues of the fused hopping kernel (ddamg_dslash.cu)
+enum {
+    EPI_CLOV_HOP = 0,            // out = Cl (H in)                         kernel A
+    EPI_CLOV_RHS_MINUS_HOP = 1,  // out = Cl (rhs - H in)                   reconstruct_odd
+    EPI_RHS_MINUS_HOP = 2,       // out = rhs - H in                        prepare_rhs
+    EPI_SCHUR = 3,               // out = Cl own - H in                     kernel B
+    EPI_RICHARDSON = 4,          // r = rhs - (Cl own - H in); out = own + w r   kernel B'
+    EPI_RESIDUAL = 5             // out = rhs - (Cl own - H in)
+};
+
+template <typename T>
+void launch_dslash(const Geom& g, int epi, bool norm, int parity, const void* in, const void* gauge_own,
+                   const void* gauge_opp, const void* clov, const void* own, const void* rhs, void* out,
+                   double omega, double* partials, cudaStream_t st);
+template <typename T>
+void launch_clover_apply(const Geom& g, const void* clov, const void* in, void* out, cudaStream_t st);
+int dslash_grid(const Geom& g);
+
+// ---- setup (ddamg_setup.cu)
+template <typename Tin, typename T>
+void launch_pack_gauge(const Geom& g, int bc, const void* U_nat, void* gauge, cudaStream_t st);
+template <typename T>
+void launch_pack_spinor(const Geom& g, const void* nat, void* x_e, void* x_o, cudaStream_t st);
+template <typename T>
+void launch_unpack_spinor(const Geom& g, const void* x_e, const void* x_o, void* nat, cudaStream_t st);
+template <typename T>
+void launch_build_clover(const Geom& g, double csw, double m0, const void* gauge, void* clov_e, void* clov_o,
+                         int* singular_flag, cudaStream_t st);
+template <typename T>
+void launch_get_clover(const Geom& g, const void* clov_e, const void* clov_o, void* A_nat, void* Ainv_nat,
+                       cudaStream_t st);
+
+// ---- BLAS-1 and the small dense part of GMRES (ddamg_blas.cu)
+// device scalar block used by Richardson / GMRES / power iteration (all fp64)
+struct Scalars {
+    double hist[HIST_MAX];                              // residual history
+    double H[(GMRES_KMAX + 1) * GMRES_KMAX * 2];        // Hessenberg / R factor, column major, complex
+    double cs[GMRES_KMAX * 2], sn[GMRES_KMAX * 2];      // Givens rotations
+    double gvec[(GMRES_KMAX + 1) * 2];                  // rotated beta e_1
+    double y[GMRES_KMAX * 2];                           // least-squares solution
+    double hcol[(GMRES_KMAX + 1) * 2];                  // current column h_{1..j,j}
+    double negh[(GMRES_KMAX + 1) * 2];                  // -hcol (axpy coefficients)
+    double scale;                                       // 1/beta or 1/h_{j+1,j}
+    double value;                                       // last reduced norm
+    int nhist;
+};
+
+int blas_grid(size_t nvec);
+// dst = sqrt(sum partials); stores into sc->value, optionally appends to sc->hist, sets sc->scale = 1/value
+void launch_finalize_norm(const double* partials, int n, Scalars* sc, int append_hist, cudaStream_t st);
+template <typename T>
+void launch_copy_norm(size_t nreal, const void* src, void* dst, double* partials, cudaStream_t st);
+template <typename T>
+void launch_scale_by_dev(size_t nreal, void* v, const double* scale, cudaStream_t st);
+template <typename T>
+void launch_axpy_norm(size_t nreal, double alpha, const void* x, void* y, double* partials, cudaStream_t st); // y = alpha*x (+norm of x)
+// partial complex dots <v_i, w>, i = 0..nb-1 (nb <= MDOT_NB): partials[block][2*nb]
+template <typename T>
+void launch_multi_dot(size_t nreal, int nb, const void* V, size_t vstride_real, const void* w, double* partials,
+                      cudaStream_t st);
+void launch_finalize_dots(const double* partials, int nblocks, int nb, Scalars* sc, int first, cudaStream_t st);
+// w += sum_i coef[i] v_i (complex coef on device, nb <= MDOT_NB); optional |w|^2 partials
+template <typename T>
+void launch_multi_axpy(size_t nreal, int nb, const void* V, size_t vstride_real, const double* coef, void* w,
+                       double* partials, cudaStream_t st);
+void launch_gmres_begin_cycle(Scalars* sc, cudaStream_t st);                 // g = beta e_1 (beta = sc->value)
+void launch_gmres_givens(Scalars* sc, int j, cudaStream_t st);               // after the norm of w is in sc->value
+void launch_gmres_solve(Scalars* sc, int m, cudaStream_t st);                // y = R^-1 g
+
+}  // namespace ddamg
