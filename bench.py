@@ -50,7 +50,7 @@ BYTES_BR = 1248         # kernel B': kernel B + b_e 96
 FLOP_PER_SITE = 1824    # 1320 (hop) + 504 (2 x 6x6 Hermitian mat-vec), per lattice site
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of kernel B' at config 5, from the
 # ncu --set full capture summarised in profiles/ (None until a capture exists)
-NCU_TRAFFIC_BYTES = {5: None, 3: None}
+NCU_TRAFFIC_BYTES = {5: 21.131e9, 3: None}     # profiles/r1_ncu_full_dslash.md
 CPU_SAMPLE = dict(L=16, T=32)
 
 
@@ -110,6 +110,23 @@ class ClockSampler:
         sm.sort()
         return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
                 "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# --------------------------------------------------------------------------- multi-rank host logic
+def max_over_ranks(ms: float, world: int, device="cpu") -> float:
+    """Timed-region length of the whole job = MAX over ranks (replicas run concurrently)."""
+    if world <= 1:
+        return float(ms)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_value(V: int, nu: int, world: int, ms_per_step: float) -> float:
+    """Whole-job site-sweeps/s: every rank sweeps its own replica of the V-site lattice nu times."""
+    return V * nu * world / (ms_per_step * 1e-3)
 
 
 # --------------------------------------------------------------------------- reference arm
@@ -261,11 +278,7 @@ def main():
             pairs.append((a, b))
         barrier()
         ms = sum(a.elapsed_time(b) for a, b in pairs)
-        if world > 1:
-            t = torch.tensor([ms], device=dev, dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms = float(t.item())
-        return ms
+        return max_over_ranks(ms, world, dev)
 
     # ---- the step: fused Richardson smoother nu = 4 (rows a2-a7)
     def prep_x(i):
@@ -292,7 +305,7 @@ def main():
     msB, nB = ctx.kernel_time_ms(1, reset=True)
     ctx.kernel_timing(False)
     ms_per_step = ms_total / K
-    value = V * NU * world / (ms_per_step * 1e-3)
+    value = job_value(V, NU, world, ms_per_step)
 
     peak, peak_src = _peaks()
     tB = msB / max(nB, 1) * 1e-3
@@ -353,7 +366,7 @@ def main():
         hout.copy_(x_e, non_blocking=True)
     ke = max(3, min(K, 10))
     ms_e2e = timed(e2e_step, ke, 2) / ke
-    e2e = {"value": V * NU * world / (ms_e2e * 1e-3), "unit": "site-sweeps/s", "ms_per_step": ms_e2e,
+    e2e = {"value": job_value(V, NU, world, ms_e2e), "unit": "site-sweeps/s", "ms_per_step": ms_e2e,
            "h2d_bytes_per_step": 2 * ctx.half_bytes, "d2h_bytes_per_step": ctx.half_bytes}
 
     line = {

@@ -46,8 +46,19 @@ __device__ __forceinline__ double block_sum(double v)
     return v;     // valid in thread 0
 }
 
+// Register budget per thread (ptxas trades registers for loads in flight; measured on B200,
+// 128 registers = 4 CTAs of 128 threads per SM is the optimum for both
+// the kernel-A class (EPI <= EPI_RHS_MINUS_HOP) and the kernel-B class).
+#ifndef DDAMG_MAXREG_A
+#define DDAMG_MAXREG_A 128
+#endif
+#ifndef DDAMG_MAXREG_B
+#define DDAMG_MAXREG_B 128
+#endif
+
 template <typename T, int EPI, bool NORM>
 __global__ void __launch_bounds__(DSLASH_THREADS)
+__maxnreg__(sizeof(T) == 4 ? (EPI <= EPI_RHS_MINUS_HOP ? DDAMG_MAXREG_A : DDAMG_MAXREG_B) : 255)
 dslash_kernel(const DslashArgs<T> a)
 {
     const int cb = blockIdx.x * DSLASH_THREADS + threadIdx.x;

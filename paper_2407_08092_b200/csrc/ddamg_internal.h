@@ -6,7 +6,10 @@
 
 namespace ddamg {
 
-constexpr int DSLASH_THREADS = 128;
+#ifndef DDAMG_DSLASH_THREADS
+#define DDAMG_DSLASH_THREADS 128
+#endif
+constexpr int DSLASH_THREADS = DDAMG_DSLASH_THREADS;
 constexpr int BLAS_THREADS = 256;
 constexpr int GMRES_KMAX = 64;          // largest cycle length m of GMRES(n, m)
 constexpr int HIST_MAX = 8192;         // residual-history entries kept on the device
