@@ -50,7 +50,7 @@ BYTES_BR = 1248         # kernel B': kernel B + b_e 96
 FLOP_PER_SITE = 1824    # 1320 (hop) + 504 (2 x 6x6 Hermitian mat-vec), per lattice site
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of kernel B' at config 5, from the
 # ncu --set full capture summarised in profiles/ (None until a capture exists)
-NCU_TRAFFIC_BYTES = {5: 21.131e9, 3: None}     # profiles/r1_ncu_full_dslash.md
+NCU_TRAFFIC_BYTES = {5: 21.274e9, 3: None}     # profiles/r1b_ncu_full_dslash.md
 CPU_SAMPLE = dict(L=16, T=32)
 
 
@@ -185,7 +185,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=5, choices=sorted(CONFIGS))
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--rows", default="all", help="'all' or 'main': skip the side measurements")
+    ap.add_argument("--rows", default="all", help="'all', 'main' (skip the side measurements) or 'multi_rhs' (main + multi-rhs rows)")
+    ap.add_argument("--nrhs", default="2,4,8", help="batch sizes of the multi-rhs rows")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
@@ -351,6 +352,36 @@ def main():
             rows["gmres_1x10"] = {"ms": ms, "ms_per_arnoldi_step": ms / kg}
         except Exception as e:     # e.g. Krylov basis does not fit
             rows["gmres_1x10"] = {"error": str(e)}
+
+    if args.rows in ("all", "multi_rhs"):
+        # ---- multi-rhs batched Richardson (NEXT-2): links + clover fetched once for nrhs rhs
+        rows["multi_rhs_richardson"] = {}
+        for nrhs in [int(t) for t in args.nrhs.split(",") if t]:
+            try:
+                Bb = torch.randn(nrhs * 12 * V, dtype=torch.float32, device=dev)
+                X0 = torch.randn(nrhs * 12 * V, dtype=torch.float32, device=dev)
+                Xb = torch.empty_like(X0)
+                ctx.kernel_timing(True)
+                ctx.kernel_time_ms(3, reset=True)
+                kb = max(3, min(K, 5))
+                ms = timed(lambda i: ctx.richardson_batch(nrhs, Bb, Xb, NU, c["omega"]), kb, 2,
+                           lambda i: Xb.copy_(X0)) / kb
+                ms3, n3 = ctx.kernel_time_ms(3, reset=False)
+                ms4, n4 = ctx.kernel_time_ms(4, reset=True)
+                ctx.kernel_timing(False)
+                bA = 192 + 864 / nrhs            # per (site, rhs): x_e neighbours 96 + write 96 + (links 576 + clover 288) / nrhs
+                bB = 384 + 864 / nrhs            # t_o 96 + x_e 96 + b_e 96 + write 96 + (576 + 288) / nrhs
+                tA3, tB4 = ms3 / max(n3, 1) * 1e-3, ms4 / max(n4, 1) * 1e-3
+                rows["multi_rhs_richardson"][str(nrhs)] = {
+                    "ms_per_call": ms, "rhs_site_sweeps_per_s": V * NU * nrhs / (ms * 1e-3),
+                    "speedup_vs_single_rhs": (V * NU * nrhs / (ms * 1e-3)) / (V * NU / (ms_per_step * 1e-3)),
+                    "kernel_A_ms": tA3 * 1e3, "kernel_A_model_GBps": bA * nrhs * Ve / tA3 / 1e9,
+                    "kernel_Bp_ms": tB4 * 1e3, "kernel_Bp_model_GBps": bB * nrhs * Ve / tB4 / 1e9,
+                    "model_bytes_per_rhs_site_sweep": bA + bB}
+                del Bb, X0, Xb
+                torch.cuda.empty_cache()
+            except Exception as e:
+                rows["multi_rhs_richardson"][str(nrhs)] = {"error": str(e)}
 
     # ---- e2e: HOST buffers, copies inside the timed region, through the public API
     hb = torch.empty_like(pool_b[0][0], device="cpu").pin_memory()

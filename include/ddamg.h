@@ -152,6 +152,36 @@ int ddamg_pack_spinor(ddamg_ctx* ctx, const void* nat, void* x_e, void* x_o);
 int ddamg_unpack_spinor(ddamg_ctx* ctx, const void* x_e, const void* x_o, void* nat);
 
 /*
+ * ---- Multi-rhs batching (PAPER.md:310-312 names "applying each block to
+ * many vectors" / multiple right-hand sides as the way to raise cache reuse).  The same D_S is
+ * applied to nrhs (1..32, V/2 * nrhs < 2^31) right-hand sides in one pass: links and clover
+ * blocks, 78 % of the bytes of a single-rhs pass, are fetched once per site for all of them.
+ * A BATCH is a DEVICE buffer of ddamg_batch_spinor_bytes(ctx, nrhs) = nrhs * half-spinor bytes
+ * holding nrhs native half spinors interleaved per site: plane j, vector index cb * nrhs + r
+ * (r = rhs index, fastest).  Callers build batches with ddamg_batch_interleave from nrhs
+ * native half spinors stored back to back (halves = [r][native half spinor]) and read them
+ * back with ddamg_batch_deinterleave; both are asynchronous, neither may alias.
+ * Every *_batch function computes, for each r independently, exactly what its single-rhs
+ * namesake computes (same arithmetic, same order: results are bit-identical per rhs).
+ */
+size_t ddamg_batch_spinor_bytes(ddamg_ctx* ctx, int nrhs);
+int ddamg_batch_interleave(ddamg_ctx* ctx, int nrhs, const void* halves, void* X);
+int ddamg_batch_deinterleave(ddamg_ctx* ctx, int nrhs, const void* X, void* halves);
+/* eq. 3 for every rhs:  Y_e[r] = D_S X_e[r].  Y_e must not alias X_e. */
+int ddamg_apply_schur_batch(ddamg_ctx* ctx, int nrhs, const void* X_e, void* Y_e);
+/*
+ * Alg. 4 (omega supplied) on every rhs, in place.  res_hist: HOST array of nu * nrhs doubles
+ * or NULL, res_hist[i * nrhs + r] = || B_e[r] - D_S X^(i)[r] ||_2.  zero_init != 0 starts from
+ * X = 0 (run as a full sweep on a zeroed batch; the result equals X = omega B bit for bit).
+ * EINVAL if nu < 0, nrhs out of range, nu * nrhs > 8192 with a history, or B_e aliases X_e.
+ */
+int ddamg_richardson_batch(ddamg_ctx* ctx, int nrhs, const void* B_e, void* X_e, int nu, double omega,
+                           int zero_init, double* res_hist);
+/* eq. 2 factors for every rhs (see ddamg_reconstruct_odd / ddamg_prepare_rhs). */
+int ddamg_reconstruct_odd_batch(ddamg_ctx* ctx, int nrhs, const void* B_o, const void* X_e, void* X_o);
+int ddamg_prepare_rhs_batch(ddamg_ctx* ctx, int nrhs, const void* B_e, const void* B_o, void* Bhat_e);
+
+/*
  * Debug / parity: the stored clover blocks as dense matrices, natural site order, DEVICE
  * buffers of V*2*6*6 complex numbers of the context precision ([n][block][row][col],
  * block 0 = spins 0,1, block 1 = spins 2,3, row = 3*(spin mod 2) + colour).
@@ -168,7 +198,8 @@ long long ddamg_launch_count(ddamg_ctx* ctx);
  * when enabled (on != 0) every hot-path kernel launch is bracketed by CUDA events on the
  * context's stream; ddamg_kernel_time_ms returns the accumulated device time (ms) and the
  * number of launches of kernel class `which` (0 = kernel A: A_oo^-1 H_oe, 1 = kernel B /
- * B': A_ee x - H_eo t with optional Richardson update) since the last reset, after
+ * B': A_ee x - H_eo t with optional Richardson update, 2 = eq.-2 factors, 3 / 4 = the
+ * multi-rhs forms of kernel A / kernel B, B') since the last reset, after
  * synchronising the stream.  Used by bench.py for the per-kernel roofline.
  */
 int ddamg_kernel_timing(ddamg_ctx* ctx, int on);

@@ -119,3 +119,18 @@ def power_iteration(apply, v0, iters: int) -> float:
         lam = _norm(w)
         v = w / lam
     return lam
+
+
+def richardson_multi(apply, B, X0, nu: int, omega: float):
+    """Multiple right-hand sides ("apply each block to many vectors",
+    multiple rhs): the same Alg. 4 run on every column independently.  ``B``, ``X0`` are
+    sequences of vectors; returns (list of x^(nu), hist) with hist[i][r] the residual norm
+    of rhs r before sweep i+1.  No new arithmetic: it calls :func:`richardson` per rhs, so
+    it inherits that function's pins.
+    """
+    xs, hists = [], []
+    for b, x0 in zip(B, X0):
+        x, h = richardson(apply, b, x0, nu, omega)
+        xs.append(x)
+        hists.append(h)
+    return xs, [[hists[r][i] for r in range(len(xs))] for i in range(nu)]

@@ -42,6 +42,13 @@ SYMBOLS = {
     "ddamg_pack_spinor": (_i, [_vp, _vp, _vp, _vp]),
     "ddamg_unpack_spinor": (_i, [_vp, _vp, _vp, _vp]),
     "ddamg_get_clover": (_i, [_vp, _vp, _vp]),
+    "ddamg_batch_spinor_bytes": (ctypes.c_size_t, [_vp, _i]),
+    "ddamg_batch_interleave": (_i, [_vp, _i, _vp, _vp]),
+    "ddamg_batch_deinterleave": (_i, [_vp, _i, _vp, _vp]),
+    "ddamg_apply_schur_batch": (_i, [_vp, _i, _vp, _vp]),
+    "ddamg_richardson_batch": (_i, [_vp, _i, _vp, _vp, _i, _d, _i, _dp]),
+    "ddamg_reconstruct_odd_batch": (_i, [_vp, _i, _vp, _vp, _vp]),
+    "ddamg_prepare_rhs_batch": (_i, [_vp, _i, _vp, _vp, _vp]),
     "ddamg_launch_count": (ctypes.c_longlong, [_vp]),
     "ddamg_kernel_timing": (_i, [_vp, _i]),
     "ddamg_kernel_time_ms": (_i, [_vp, _i, _dp, _llp, _i]),
@@ -204,6 +211,68 @@ class Ddamg:
         lam = ctypes.c_double(0.0)
         self._ck(self.lib.ddamg_power_iteration(self._h, _ptr(v_e), iters, ctypes.byref(lam)), "ddamg_power_iteration")
         return lam.value
+
+    # -- multi-rhs batching (NEXT-2) ------------------------------------------------
+    def batch_spinor(self, nrhs: int, zero: bool = False) -> torch.Tensor:
+        """A batch buffer: nrhs native half spinors interleaved per site (flat real tensor)."""
+        assert self.lib.ddamg_batch_spinor_bytes(self._h, nrhs) == nrhs * self.half_bytes
+        return (torch.zeros if zero else torch.empty)(nrhs * 12 * self.V, dtype=self.rdtype, device=self.device)
+
+    def _chk_batch(self, nrhs, *ts):
+        for t in ts:
+            assert t.is_cuda and t.dtype == self.rdtype and t.is_contiguous() and t.numel() == nrhs * 12 * self.V, \
+                "expected a batch of nrhs native half spinors of this context"
+
+    def batch_interleave(self, halves, X: Optional[torch.Tensor] = None) -> torch.Tensor:
+        """halves: list of native half spinors, or an (nrhs, 12 V) tensor of them -> batch."""
+        H = torch.stack(list(halves)) if not isinstance(halves, torch.Tensor) else halves
+        nrhs = H.shape[0]
+        H = H.contiguous().view(-1)
+        X = self.batch_spinor(nrhs) if X is None else X
+        self._chk_batch(nrhs, H, X)
+        self._ck(self.lib.ddamg_batch_interleave(self._h, nrhs, _ptr(H), _ptr(X)), "ddamg_batch_interleave")
+        return X
+
+    def batch_deinterleave(self, nrhs: int, X: torch.Tensor) -> torch.Tensor:
+        """batch -> (nrhs, 12 V) tensor whose rows are native half spinors."""
+        self._chk_batch(nrhs, X)
+        H = torch.empty(nrhs * 12 * self.V, dtype=self.rdtype, device=self.device)
+        self._ck(self.lib.ddamg_batch_deinterleave(self._h, nrhs, _ptr(X), _ptr(H)), "ddamg_batch_deinterleave")
+        return H.view(nrhs, 12 * self.V)
+
+    def apply_schur_batch(self, nrhs: int, X_e: torch.Tensor, Y_e: Optional[torch.Tensor] = None) -> torch.Tensor:
+        Y_e = self.batch_spinor(nrhs) if Y_e is None else Y_e
+        self._chk_batch(nrhs, X_e, Y_e)
+        self._ck(self.lib.ddamg_apply_schur_batch(self._h, nrhs, _ptr(X_e), _ptr(Y_e)), "ddamg_apply_schur_batch")
+        return Y_e
+
+    def richardson_batch(self, nrhs: int, B_e: torch.Tensor, X_e: torch.Tensor, nu: int, omega: float,
+                         zero_init: bool = False, history: bool = False):
+        """history -> list of nu lists of nrhs residual norms."""
+        self._chk_batch(nrhs, B_e, X_e)
+        hist = (ctypes.c_double * max(nu * nrhs, 1))() if history else None
+        self._ck(self.lib.ddamg_richardson_batch(self._h, nrhs, _ptr(B_e), _ptr(X_e), nu, omega, int(zero_init),
+                                                 hist), "ddamg_richardson_batch")
+        if not history:
+            return None
+        flat = list(hist)
+        return [flat[i * nrhs:(i + 1) * nrhs] for i in range(nu)]
+
+    def reconstruct_odd_batch(self, nrhs: int, B_o: torch.Tensor, X_e: torch.Tensor,
+                              X_o: Optional[torch.Tensor] = None) -> torch.Tensor:
+        X_o = self.batch_spinor(nrhs) if X_o is None else X_o
+        self._chk_batch(nrhs, B_o, X_e, X_o)
+        self._ck(self.lib.ddamg_reconstruct_odd_batch(self._h, nrhs, _ptr(B_o), _ptr(X_e), _ptr(X_o)),
+                 "ddamg_reconstruct_odd_batch")
+        return X_o
+
+    def prepare_rhs_batch(self, nrhs: int, B_e: torch.Tensor, B_o: torch.Tensor,
+                          Bhat_e: Optional[torch.Tensor] = None) -> torch.Tensor:
+        Bhat_e = self.batch_spinor(nrhs) if Bhat_e is None else Bhat_e
+        self._chk_batch(nrhs, B_e, B_o, Bhat_e)
+        self._ck(self.lib.ddamg_prepare_rhs_batch(self._h, nrhs, _ptr(B_e), _ptr(B_o), _ptr(Bhat_e)),
+                 "ddamg_prepare_rhs_batch")
+        return Bhat_e
 
     # -- accounting ---------------------------------------------------------------
     def launch_count(self) -> int:

@@ -28,6 +28,9 @@ struct ddamg_ctx {
     void* tmp_e;                // scratch half spinor (power iteration, final residual)
     void* krylov;               // (kcap + 1) half spinors
     int kcap;
+    void* tmp_batch;            // multi-rhs t_o (batch_cap half spinors)
+    double* partials_batch;     // multi-rhs reduction scratch
+    int batch_cap;
     double* partials;           // reduction scratch
     size_t partials_len;
     Scalars* sc;                // device scalars
@@ -119,6 +122,7 @@ extern "C" int ddamg_create(ddamg_ctx** out, int L, int T, double csw, double m0
     ctx->half_bytes = ctx->nreal * ctx->real_bytes;
     ctx->gauge = ctx->clov[0] = ctx->clov[1] = ctx->tmp_o = ctx->tmp_e = ctx->krylov = nullptr;
     ctx->kcap = 0;
+    ctx->tmp_batch = nullptr; ctx->partials_batch = nullptr; ctx->batch_cap = 0;
     ctx->partials = nullptr; ctx->sc = nullptr; ctx->host_hist = nullptr; ctx->singular = nullptr;
     ctx->have_gauge = ctx->have_clover = false;
     ctx->sticky = DDAMG_OK; ctx->launches = 0; ctx->timing = false;
@@ -157,6 +161,7 @@ extern "C" int ddamg_destroy(ddamg_ctx* ctx)
     for (auto& ev : ctx->events) { cudaEventDestroy(ev.a); cudaEventDestroy(ev.b); }
     cudaFree(ctx->gauge); cudaFree(ctx->clov[0]); cudaFree(ctx->clov[1]);
     cudaFree(ctx->tmp_o); cudaFree(ctx->tmp_e); cudaFree(ctx->krylov);
+    cudaFree(ctx->tmp_batch); cudaFree(ctx->partials_batch);
     cudaFree(ctx->partials); cudaFree(ctx->sc); cudaFree(ctx->singular);
     if (ctx->host_hist) cudaFreeHost(ctx->host_hist);
     cudaGetLastError();
@@ -249,8 +254,9 @@ extern "C" int ddamg_get_clover(ddamg_ctx* ctx, void* A_nat, void* Ainv_nat)
 // --------------------------------------------------------------------------- hot path
 // One fused hopping launch.  parity = parity of the output sites.
 static int dslash(ddamg_ctx* ctx, int epi, bool norm, int parity, const void* in, const void* own, const void* rhs,
-                  void* out, double omega, int which)
+                  void* out, double omega, int which, int nrhs = 1)
 {
+    double* partials = nrhs > 1 ? ctx->partials_batch : ctx->partials;
     ddamg_ctx::Ev ev;
     if (ctx->timing) {
         if (cudaEventCreate(&ev.a) != cudaSuccess || cudaEventCreate(&ev.b) != cudaSuccess)
@@ -260,10 +266,10 @@ static int dslash(ddamg_ctx* ctx, int epi, bool norm, int parity, const void* in
     }
     if (ctx->prec == DDAMG_F32)
         launch_dslash<float>(ctx->g, epi, norm, parity, in, gauge_block(ctx, parity), gauge_block(ctx, 1 - parity),
-                             ctx->clov[parity], own, rhs, out, omega, ctx->partials, ctx->stream);
+                             ctx->clov[parity], own, rhs, out, omega, partials, nrhs, ctx->stream);
     else
         launch_dslash<double>(ctx->g, epi, norm, parity, in, gauge_block(ctx, parity), gauge_block(ctx, 1 - parity),
-                              ctx->clov[parity], own, rhs, out, omega, ctx->partials, ctx->stream);
+                              ctx->clov[parity], own, rhs, out, omega, partials, nrhs, ctx->stream);
     if (ctx->timing) {
         cudaEventRecord(ev.b, ctx->stream);
         ctx->events.push_back(ev);
@@ -371,11 +377,122 @@ extern "C" int ddamg_prepare_rhs(ddamg_ctx* ctx, const void* b_e, const void* b_
     if (!b_e || !b_o || !bhat_e) return fail(ctx, DDAMG_EINVAL, "ddamg_prepare_rhs: NULL argument");
     int s = need_ready(ctx, "ddamg_prepare_rhs");
     if (s != DDAMG_OK) return s;
-    if (ctx->prec == DDAMG_F32) launch_clover_apply<float>(ctx->g, ctx->clov[1], b_o, ctx->tmp_o, ctx->stream);     // t_o = A_oo^-1 b_o
-    else launch_clover_apply<double>(ctx->g, ctx->clov[1], b_o, ctx->tmp_o, ctx->stream);
+    if (ctx->prec == DDAMG_F32) launch_clover_apply<float>(ctx->g, ctx->clov[1], b_o, ctx->tmp_o, 1, ctx->stream);     // t_o = A_oo^-1 b_o
+    else launch_clover_apply<double>(ctx->g, ctx->clov[1], b_o, ctx->tmp_o, 1, ctx->stream);
     s = after_launch(ctx);
     if (s != DDAMG_OK) return s;
     return dslash(ctx, EPI_RHS_MINUS_HOP, false, 0, ctx->tmp_o, nullptr, b_e, bhat_e, 0.0, 2);         // b_e - H_eo t_o
+}
+
+// --------------------------------------------------------------------------- multi-rhs (NEXT-2)
+// The same operator applied to nrhs right-hand sides per pass ("apply each
+// block to many vectors"): links and clover blocks are fetched once per site for all nrhs.
+static int batch_ready(ddamg_ctx* ctx, int nrhs, const char* who)
+{
+    if (nrhs < 1 || nrhs > NRHS_MAX) return fail(ctx, DDAMG_EINVAL, std::string(who) + ": nrhs must be 1..32");
+    if ((double)ctx->g.Vh * nrhs >= 2147483648.0) return fail(ctx, DDAMG_EINVAL, std::string(who) + ": V/2 * nrhs must be < 2^31");
+    int s = need_ready(ctx, who);
+    if (s != DDAMG_OK) return s;
+    if (nrhs > ctx->batch_cap) {
+        CK(cudaStreamSynchronize(ctx->stream));
+        cudaFree(ctx->tmp_batch); cudaFree(ctx->partials_batch);
+        ctx->tmp_batch = nullptr; ctx->partials_batch = nullptr; ctx->batch_cap = 0;
+        cudaError_t e = cudaMalloc(&ctx->tmp_batch, (size_t)nrhs * ctx->half_bytes);
+        if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->partials_batch, sizeof(double) * (size_t)dslash_grid(ctx->g, nrhs) * nrhs);
+        if (e != cudaSuccess) {
+            cudaGetLastError();
+            cudaFree(ctx->tmp_batch); ctx->tmp_batch = nullptr;
+            return fail(ctx, DDAMG_ENOMEM, std::string(who) + ": cannot allocate the multi-rhs workspace");
+        }
+        ctx->batch_cap = nrhs;
+    }
+    return DDAMG_OK;
+}
+
+extern "C" size_t ddamg_batch_spinor_bytes(ddamg_ctx* ctx, int nrhs)
+{
+    return (ctx && nrhs > 0) ? (size_t)nrhs * ctx->half_bytes : 0;
+}
+
+static int batch_interleave(ddamg_ctx* ctx, int nrhs, bool to_batch, void* halves, void* X, const char* who)
+{
+    ENTER(ctx);
+    if (!halves || !X || halves == X) return fail(ctx, DDAMG_EINVAL, std::string(who) + ": NULL or aliased arguments");
+    if (nrhs < 1 || nrhs > NRHS_MAX || (double)ctx->g.Vh * nrhs >= 2147483648.0)
+        return fail(ctx, DDAMG_EINVAL, std::string(who) + ": bad nrhs");
+    if (ctx->prec == DDAMG_F32) launch_batch_interleave<float>(ctx->g, nrhs, to_batch, halves, X, ctx->stream);
+    else launch_batch_interleave<double>(ctx->g, nrhs, to_batch, halves, X, ctx->stream);
+    return after_launch(ctx);
+}
+
+extern "C" int ddamg_batch_interleave(ddamg_ctx* ctx, int nrhs, const void* halves, void* X)
+{
+    return batch_interleave(ctx, nrhs, true, const_cast<void*>(halves), X, "ddamg_batch_interleave");
+}
+
+extern "C" int ddamg_batch_deinterleave(ddamg_ctx* ctx, int nrhs, const void* X, void* halves)
+{
+    return batch_interleave(ctx, nrhs, false, halves, const_cast<void*>(X), "ddamg_batch_deinterleave");
+}
+
+extern "C" int ddamg_apply_schur_batch(ddamg_ctx* ctx, int nrhs, const void* X_e, void* Y_e)
+{
+    ENTER(ctx);
+    if (!X_e || !Y_e || X_e == Y_e) return fail(ctx, DDAMG_EINVAL, "ddamg_apply_schur_batch: NULL or aliased arguments");
+    int s = batch_ready(ctx, nrhs, "ddamg_apply_schur_batch");
+    if (s != DDAMG_OK) return s;
+    s = dslash(ctx, EPI_CLOV_HOP, false, 1, X_e, nullptr, nullptr, ctx->tmp_batch, 0.0, 3, nrhs);
+    if (s != DDAMG_OK) return s;
+    return dslash(ctx, EPI_SCHUR, false, 0, ctx->tmp_batch, X_e, nullptr, Y_e, 0.0, 4, nrhs);
+}
+
+extern "C" int ddamg_richardson_batch(ddamg_ctx* ctx, int nrhs, const void* B_e, void* X_e, int nu, double omega,
+                                      int zero_init, double* res_hist)
+{
+    ENTER(ctx);
+    if (!B_e || !X_e || B_e == X_e || nu < 0) return fail(ctx, DDAMG_EINVAL, "ddamg_richardson_batch: bad arguments");
+    int s = batch_ready(ctx, nrhs, "ddamg_richardson_batch");
+    if (s != DDAMG_OK) return s;
+    const bool hist = res_hist != nullptr;
+    if (hist && (long long)nu * nrhs > HIST_MAX) return fail(ctx, DDAMG_EINVAL, "ddamg_richardson_batch: nu * nrhs exceeds the history capacity");
+    if (hist) { s = reset_hist(ctx); if (s != DDAMG_OK) return s; }
+    // x^(0) = 0 is run as a full sweep on a zeroed batch (bit-identical to x = omega b)
+    if (zero_init) CK(cudaMemsetAsync(X_e, 0, (size_t)nrhs * ctx->half_bytes, ctx->stream));
+    for (int i = 0; i < nu; ++i) {
+        s = dslash(ctx, EPI_CLOV_HOP, false, 1, X_e, nullptr, nullptr, ctx->tmp_batch, 0.0, 3, nrhs);
+        if (s != DDAMG_OK) return s;
+        s = dslash(ctx, EPI_RICHARDSON, hist, 0, ctx->tmp_batch, X_e, B_e, X_e, omega, 4, nrhs);
+        if (s != DDAMG_OK) return s;
+        if (hist) {
+            launch_finalize_norm_batch(nrhs > 1 ? ctx->partials_batch : ctx->partials, dslash_grid(ctx->g, nrhs), nrhs, ctx->sc, i * nrhs, ctx->stream);
+            s = after_launch(ctx);
+            if (s != DDAMG_OK) return s;
+        }
+    }
+    if (hist && nu > 0) return copy_hist(ctx, res_hist, nu * nrhs, nullptr);
+    return DDAMG_OK;
+}
+
+extern "C" int ddamg_reconstruct_odd_batch(ddamg_ctx* ctx, int nrhs, const void* B_o, const void* X_e, void* X_o)
+{
+    ENTER(ctx);
+    if (!B_o || !X_e || !X_o) return fail(ctx, DDAMG_EINVAL, "ddamg_reconstruct_odd_batch: NULL argument");
+    int s = batch_ready(ctx, nrhs, "ddamg_reconstruct_odd_batch");
+    if (s != DDAMG_OK) return s;
+    return dslash(ctx, EPI_CLOV_RHS_MINUS_HOP, false, 1, X_e, nullptr, B_o, X_o, 0.0, 2, nrhs);
+}
+
+extern "C" int ddamg_prepare_rhs_batch(ddamg_ctx* ctx, int nrhs, const void* B_e, const void* B_o, void* Bhat_e)
+{
+    ENTER(ctx);
+    if (!B_e || !B_o || !Bhat_e) return fail(ctx, DDAMG_EINVAL, "ddamg_prepare_rhs_batch: NULL argument");
+    int s = batch_ready(ctx, nrhs, "ddamg_prepare_rhs_batch");
+    if (s != DDAMG_OK) return s;
+    if (ctx->prec == DDAMG_F32) launch_clover_apply<float>(ctx->g, ctx->clov[1], B_o, ctx->tmp_batch, nrhs, ctx->stream);
+    else launch_clover_apply<double>(ctx->g, ctx->clov[1], B_o, ctx->tmp_batch, nrhs, ctx->stream);
+    s = after_launch(ctx);
+    if (s != DDAMG_OK) return s;
+    return dslash(ctx, EPI_RHS_MINUS_HOP, false, 0, ctx->tmp_batch, nullptr, B_e, Bhat_e, 0.0, 2, nrhs);
 }
 
 // --------------------------------------------------------------------------- GMRES

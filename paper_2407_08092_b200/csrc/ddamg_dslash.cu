@@ -26,7 +26,8 @@ struct DslashArgs {
     const T* rhs;            // b (EPI_RICHARDSON / RESIDUAL / *_RHS_*)
     T* out;
     T omega;
-    double* partials;        // per-block sum of |r|^2 (NORM) or nullptr
+    double* partials;        // per-block sum of |r|^2 (NORM) or nullptr; batch: [block][nrhs]
+    int nrhs;                // BATCH kernels: right-hand sides interleaved per site (else 1)
 };
 
 __device__ __forceinline__ double block_sum(double v)
@@ -56,17 +57,25 @@ __device__ __forceinline__ double block_sum(double v)
 #define DDAMG_MAXREG_B 128
 #endif
 
-template <typename T, int EPI, bool NORM>
+// BATCH (multi-rhs): one thread per (site, rhs), rhs fastest, so that the
+// nrhs threads of a site share every link / clover vector they load while all spinor planes
+// stay contiguous per warp (vector index cb * nrhs + r).
+template <typename T, int EPI, bool NORM, bool BATCH>
 __global__ void __launch_bounds__(DSLASH_THREADS)
 __maxnreg__(sizeof(T) == 4 ? (EPI <= EPI_RHS_MINUS_HOP ? DDAMG_MAXREG_A : DDAMG_MAXREG_B) : 255)
 dslash_kernel(const DslashArgs<T> a)
 {
-    const int cb = blockIdx.x * DSLASH_THREADS + threadIdx.x;
+    const int tid = blockIdx.x * DSLASH_THREADS + threadIdx.x;
+    const int nrhs = BATCH ? a.nrhs : 1;
+    const int cb = BATCH ? tid / nrhs : tid;
+    const int rr = BATCH ? tid - cb * nrhs : 0;
+    const int Vs = a.g.Vh * nrhs;          // vectors per spinor plane
+    const int sv = cb * nrhs + rr;         // this thread's vector index in a spinor plane (== tid)
     double nrm = 0.0;
     if (cb < a.g.Vh) {
         const Site s = site_of_cb(a.g, cb, a.parity);
         T acc[24];
-        hop_site<T>(a.g, cb, s, a.in, a.gauge_own, a.gauge_opp, acc);
+        hop_site<T>(a.g, cb, s, a.in, nrhs, rr, a.gauge_own, a.gauge_opp, acc);
         T res[24];
         if (EPI == EPI_CLOV_HOP) {
 #pragma unroll
@@ -74,25 +83,25 @@ dslash_kernel(const DslashArgs<T> a)
             clover_site_mul<T>(a.clov, a.g.Vh, cb, acc, res);
         } else if (EPI == EPI_CLOV_RHS_MINUS_HOP) {
             T b[24];
-            load_spinor<T, true>(a.rhs, a.g.Vh, cb, b);
+            load_spinor<T, true>(a.rhs, Vs, sv, b);
 #pragma unroll
             for (int i = 0; i < 24; ++i) acc[i] = b[i] + (T)0.5 * acc[i];
             clover_site_mul<T>(a.clov, a.g.Vh, cb, acc, res);
         } else if (EPI == EPI_RHS_MINUS_HOP) {
             T b[24];
-            load_spinor<T, true>(a.rhs, a.g.Vh, cb, b);
+            load_spinor<T, true>(a.rhs, Vs, sv, b);
 #pragma unroll
             for (int i = 0; i < 24; ++i) res[i] = b[i] + (T)0.5 * acc[i];
         } else {
             T x[24], ax[24];
-            load_spinor<T, true>(a.own, a.g.Vh, cb, x);
+            load_spinor<T, true>(a.own, Vs, sv, x);
             clover_site_mul<T>(a.clov, a.g.Vh, cb, x, ax);
             if (EPI == EPI_SCHUR) {
 #pragma unroll
                 for (int i = 0; i < 24; ++i) res[i] = ax[i] + (T)0.5 * acc[i];     // A x - H t
             } else {
                 T b[24];
-                load_spinor<T, true>(a.rhs, a.g.Vh, cb, b);
+                load_spinor<T, true>(a.rhs, Vs, sv, b);
 #pragma unroll
                 for (int i = 0; i < 24; ++i) {
                     const T r = b[i] - (ax[i] + (T)0.5 * acc[i]);
@@ -101,27 +110,44 @@ dslash_kernel(const DslashArgs<T> a)
                 }
             }
         }
-        store_spinor<T>(a.out, a.g.Vh, cb, res);
+        store_spinor<T>(a.out, Vs, sv, res);
     }
     if (NORM) {
-        const double tot = block_sum(nrm);
-        if (threadIdx.x == 0) a.partials[blockIdx.x] = tot;
+        if (BATCH) {
+            // per-rhs partial sums of this block: thread q < nrhs adds the entries of rhs q
+            __shared__ double per_thread[DSLASH_THREADS];
+            per_thread[threadIdx.x] = nrm;
+            __syncthreads();
+            if ((int)threadIdx.x < nrhs) {
+                const int first = (int)(((long long)blockIdx.x * DSLASH_THREADS) % nrhs);   // rhs of thread 0
+                int i = (int)threadIdx.x - first;
+                if (i < 0) i += nrhs;
+                double tot = 0.0;
+                for (; i < DSLASH_THREADS; i += nrhs) tot += per_thread[i];
+                a.partials[(size_t)blockIdx.x * nrhs + threadIdx.x] = tot;
+            }
+        } else {
+            const double tot = block_sum(nrm);
+            if (threadIdx.x == 0) a.partials[blockIdx.x] = tot;
+        }
     }
 }
 
 template <typename T, int EPI, bool NORM>
 static void launch(const DslashArgs<T>& a, cudaStream_t st)
 {
-    const int grid = (a.g.Vh + DSLASH_THREADS - 1) / DSLASH_THREADS;
-    dslash_kernel<T, EPI, NORM><<<grid, DSLASH_THREADS, 0, st>>>(a);
+    const int grid = dslash_grid(a.g, a.nrhs);
+    if (a.nrhs > 1) dslash_kernel<T, EPI, NORM, true><<<grid, DSLASH_THREADS, 0, st>>>(a);
+    else dslash_kernel<T, EPI, NORM, false><<<grid, DSLASH_THREADS, 0, st>>>(a);
 }
 
 template <typename T>
 void launch_dslash(const Geom& g, int epi, bool norm, int parity, const void* in, const void* gauge_own,
                    const void* gauge_opp, const void* clov, const void* own, const void* rhs, void* out,
-                   double omega, double* partials, cudaStream_t st)
+                   double omega, double* partials, int nrhs, cudaStream_t st)
 {
     DslashArgs<T> a;
+    a.nrhs = nrhs;
     a.g = g;
     a.parity = parity;
     a.in = (const T*)in;
@@ -150,32 +176,35 @@ void launch_dslash(const Geom& g, int epi, bool norm, int parity, const void* in
 }
 
 template void launch_dslash<float>(const Geom&, int, bool, int, const void*, const void*, const void*, const void*,
-                                   const void*, const void*, void*, double, double*, cudaStream_t);
+                                   const void*, const void*, void*, double, double*, int, cudaStream_t);
 template void launch_dslash<double>(const Geom&, int, bool, int, const void*, const void*, const void*, const void*,
-                                    const void*, const void*, void*, double, double*, cudaStream_t);
+                                    const void*, const void*, void*, double, double*, int, cudaStream_t);
 
 // out = Cl in on one parity (right factor of eq. 2: t_o = A_oo^-1 b_o)
 template <typename T>
 __global__ void __launch_bounds__(DSLASH_THREADS)
-clover_apply_kernel(Geom g, const T* __restrict__ clov, const T* __restrict__ in, T* __restrict__ out)
+clover_apply_kernel(Geom g, int nrhs, const T* __restrict__ clov, const T* __restrict__ in, T* __restrict__ out)
 {
-    const int cb = blockIdx.x * DSLASH_THREADS + threadIdx.x;
+    const int tid = blockIdx.x * DSLASH_THREADS + threadIdx.x;
+    const int cb = tid / nrhs;
     if (cb >= g.Vh) return;
     T v[24], res[24];
-    load_spinor<T, true>(in, g.Vh, cb, v);
+    load_spinor<T, true>(in, g.Vh * nrhs, tid, v);
     clover_site_mul<T>(clov, g.Vh, cb, v, res);
-    store_spinor<T>(out, g.Vh, cb, res);
+    store_spinor<T>(out, g.Vh * nrhs, tid, res);
 }
 
 template <typename T>
-void launch_clover_apply(const Geom& g, const void* clov, const void* in, void* out, cudaStream_t st)
+void launch_clover_apply(const Geom& g, const void* clov, const void* in, void* out, int nrhs, cudaStream_t st)
 {
-    const int grid = (g.Vh + DSLASH_THREADS - 1) / DSLASH_THREADS;
-    clover_apply_kernel<T><<<grid, DSLASH_THREADS, 0, st>>>(g, (const T*)clov, (const T*)in, (T*)out);
+    clover_apply_kernel<T><<<dslash_grid(g, nrhs), DSLASH_THREADS, 0, st>>>(g, nrhs, (const T*)clov, (const T*)in, (T*)out);
 }
-template void launch_clover_apply<float>(const Geom&, const void*, const void*, void*, cudaStream_t);
-template void launch_clover_apply<double>(const Geom&, const void*, const void*, void*, cudaStream_t);
+template void launch_clover_apply<float>(const Geom&, const void*, const void*, void*, int, cudaStream_t);
+template void launch_clover_apply<double>(const Geom&, const void*, const void*, void*, int, cudaStream_t);
 
-int dslash_grid(const Geom& g) { return (g.Vh + DSLASH_THREADS - 1) / DSLASH_THREADS; }
+int dslash_grid(const Geom& g, int nrhs)
+{
+    return (int)(((long long)g.Vh * nrhs + DSLASH_THREADS - 1) / DSLASH_THREADS);
+}
 
 }  // namespace ddamg

@@ -122,12 +122,16 @@ __device__ __forceinline__ void hop_dir(const T (&psi)[24], const T (&u)[18], T 
 
 // acc = sum over the 8 neighbours (WITHOUT the -1/2).  `in` is the opposite-parity spinor,
 // gauge_own / gauge_opp the 4-direction link blocks of this site's / the other parity.
+// Multi-rhs: `in` holds nrhs spinors interleaved per site (vector index
+// cb * nrhs + r, plane stride Vh * nrhs); links are indexed by site only, so the nrhs
+// adjacent threads of one site read the same link vectors (one DRAM fetch, L1 broadcast).
 template <typename T>
 __device__ __forceinline__ void hop_site(const Geom& g, int cb, const Site& s,
-                                         const T* __restrict__ in,
+                                         const T* __restrict__ in, const int nrhs, const int r,
                                          const T* __restrict__ gauge_own,
                                          const T* __restrict__ gauge_opp, T (&acc)[24])
 {
+    const int Vs = g.Vh * nrhs;                 // vectors per spinor plane
     const size_t lblk = (size_t)18 * g.Vh;      // reals per (parity, mu) link block
 #pragma unroll
     for (int i = 0; i < 24; ++i) acc[i] = 0;
@@ -138,10 +142,10 @@ __device__ __forceinline__ void hop_site(const Geom& g, int cb, const Site& s,
     nbs[4] = neighbour_cb<2, +1>(g, cb, s); nbs[5] = neighbour_cb<2, -1>(g, cb, s);
     nbs[6] = neighbour_cb<3, +1>(g, cb, s); nbs[7] = neighbour_cb<3, -1>(g, cb, s);
 #define DDAMG_HOP(MU)                                                        \
-    load_spinor<T>(in, g.Vh, nbs[2 * MU], psi);                              \
+    load_spinor<T>(in, Vs, nbs[2 * MU] * nrhs + r, psi);                     \
     load_link(gauge_own + MU * lblk, g.Vh, cb, u);                           \
     hop_dir<MU, true>(psi, u, acc);                                          \
-    load_spinor<T>(in, g.Vh, nbs[2 * MU + 1], psi);                          \
+    load_spinor<T>(in, Vs, nbs[2 * MU + 1] * nrhs + r, psi);                 \
     load_link(gauge_opp + MU * lblk, g.Vh, nbs[2 * MU + 1], u);              \
     hop_dir<MU, false>(psi, u, acc);
     DDAMG_HOP(0)

@@ -13,6 +13,7 @@ constexpr int DSLASH_THREADS = DDAMG_DSLASH_THREADS;
 constexpr int BLAS_THREADS = 256;
 constexpr int GMRES_KMAX = 64;          // largest cycle length m of GMRES(n, m)
 constexpr int HIST_MAX = 8192;         // residual-history entries kept on the device
+constexpr int NRHS_MAX = 32;            // right-hand sides per multi-rhs batch
 constexpr int MDOT_NB = 8;              // basis vectors handled per fused multi-dot / multi-axpy pass
 
 // epilogues of the fused hopping kernel (ddamg_dslash.cu)
@@ -28,10 +29,10 @@ enum {
 template <typename T>
 void launch_dslash(const Geom& g, int epi, bool norm, int parity, const void* in, const void* gauge_own,
                    const void* gauge_opp, const void* clov, const void* own, const void* rhs, void* out,
-                   double omega, double* partials, cudaStream_t st);
+                   double omega, double* partials, int nrhs, cudaStream_t st);
 template <typename T>
-void launch_clover_apply(const Geom& g, const void* clov, const void* in, void* out, cudaStream_t st);
-int dslash_grid(const Geom& g);
+void launch_clover_apply(const Geom& g, const void* clov, const void* in, void* out, int nrhs, cudaStream_t st);
+int dslash_grid(const Geom& g, int nrhs = 1);
 
 // ---- setup (ddamg_setup.cu)
 template <typename Tin, typename T>
@@ -40,6 +41,8 @@ template <typename T>
 void launch_pack_spinor(const Geom& g, const void* nat, void* x_e, void* x_o, cudaStream_t st);
 template <typename T>
 void launch_unpack_spinor(const Geom& g, const void* x_e, const void* x_o, void* nat, cudaStream_t st);
+template <typename T>
+void launch_batch_interleave(const Geom& g, int nrhs, bool to_batch, void* halves, void* X, cudaStream_t st);
 template <typename T>
 void launch_build_clover(const Geom& g, double csw, double m0, const void* gauge, void* clov_e, void* clov_o,
                          int* singular_flag, cudaStream_t st);
@@ -65,6 +68,7 @@ struct Scalars {
 int blas_grid(size_t nvec);
 // dst = sqrt(sum partials); stores into sc->value, optionally appends to sc->hist, sets sc->scale = 1/value
 void launch_finalize_norm(const double* partials, int n, Scalars* sc, int append_hist, cudaStream_t st);
+void launch_finalize_norm_batch(const double* partials, int nblocks, int nrhs, Scalars* sc, int offset, cudaStream_t st);
 template <typename T>
 void launch_copy_norm(size_t nreal, const void* src, void* dst, double* partials, cudaStream_t st);
 template <typename T>

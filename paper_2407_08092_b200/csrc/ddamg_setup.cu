@@ -121,6 +121,36 @@ template void launch_pack_spinor<double>(const Geom&, const void*, void*, void*,
 template void launch_unpack_spinor<float>(const Geom&, const void*, const void*, void*, cudaStream_t);
 template void launch_unpack_spinor<double>(const Geom&, const void*, const void*, void*, cudaStream_t);
 
+// ------------------------------------------------------------------ multi-rhs interleave
+// X[plane][cb * nrhs + r] = halves[r][plane][cb]  (TO_BATCH) or the inverse.  One thread per
+// vector of the batch; writes (TO_BATCH) / reads (inverse) of the batch are contiguous.
+template <typename T, bool TO_BATCH>
+__global__ void batch_interleave_kernel(int Vh, int nrhs, typename VecOf<T>::type* __restrict__ halves,
+                                        typename VecOf<T>::type* __restrict__ X)
+{
+    constexpr int NP = 24 / VecOf<T>::N;
+    const size_t per_plane = (size_t)Vh * nrhs;
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= per_plane * NP) return;
+    const int plane = (int)(i / per_plane);
+    const size_t rem = i - (size_t)plane * per_plane;
+    const int cb = (int)(rem / nrhs), r = (int)(rem - (size_t)cb * nrhs);
+    const size_t h = ((size_t)r * NP + plane) * Vh + cb;
+    if (TO_BATCH) X[i] = halves[h];
+    else halves[h] = X[i];
+}
+template <typename T>
+void launch_batch_interleave(const Geom& g, int nrhs, bool to_batch, void* halves, void* X, cudaStream_t st)
+{
+    using V = typename VecOf<T>::type;
+    const size_t n = (size_t)g.Vh * nrhs * (24 / VecOf<T>::N);
+    const unsigned grid = (unsigned)((n + 255) / 256);
+    if (to_batch) batch_interleave_kernel<T, true><<<grid, 256, 0, st>>>(g.Vh, nrhs, (V*)halves, (V*)X);
+    else batch_interleave_kernel<T, false><<<grid, 256, 0, st>>>(g.Vh, nrhs, (V*)halves, (V*)X);
+}
+template void launch_batch_interleave<float>(const Geom&, int, bool, void*, void*, cudaStream_t);
+template void launch_batch_interleave<double>(const Geom&, int, bool, void*, void*, cudaStream_t);
+
 // ------------------------------------------------------------------ a1: clover build
 struct M3 { double re[9], im[9]; };
 
