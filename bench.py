@@ -187,6 +187,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--rows", default="all", help="'all', 'main' (skip the side measurements) or 'multi_rhs' (main + multi-rhs rows)")
     ap.add_argument("--nrhs", default="2,4,8", help="batch sizes of the multi-rhs rows")
+    ap.add_argument("--batch-l2-bytes", type=float, default=None, help="override ddamg option batch_l2_bytes")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
@@ -356,6 +357,8 @@ def main():
     if args.rows in ("all", "multi_rhs"):
         # ---- multi-rhs batched Richardson (NEXT-2): links + clover fetched once for nrhs rhs
         rows["multi_rhs_richardson"] = {}
+        if args.batch_l2_bytes is not None:
+            ctx.set_option("batch_l2_bytes", args.batch_l2_bytes)
         for nrhs in [int(t) for t in args.nrhs.split(",") if t]:
             try:
                 Bb = torch.randn(nrhs * 12 * V, dtype=torch.float32, device=dev)

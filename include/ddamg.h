@@ -190,6 +190,17 @@ int ddamg_prepare_rhs_batch(ddamg_ctx* ctx, int nrhs, const void* B_e, const voi
  */
 int ddamg_get_clover(ddamg_ctx* ctx, void* A_nat, void* Ainv_nat);
 
+/*
+ * Tuning options (never change results, only the order in which sites are visited):
+ *   "batch_l2_bytes"  L2 budget (bytes, default 40e6) of the multi-rhs kernels' z-chunked
+ *                     traversal: CTAs visit the lattice in chunks of zc z-planes (zc = largest
+ *                     divisor of L with 3 * zc * one (z,t)-plane of batch spinors <= budget)
+ *                     so that t-neighbours are re-read from L2, not HBM.  0 = smallest chunks;
+ *                     a huge value = plain lexicographic order.
+ * EINVAL for an unknown name or a bad value.
+ */
+int ddamg_set_option(ddamg_ctx* ctx, const char* name, double value);
+
 /* Number of kernel launches this context has enqueued since creation (bench accounting). */
 long long ddamg_launch_count(ddamg_ctx* ctx);
 

@@ -49,6 +49,7 @@ SYMBOLS = {
     "ddamg_richardson_batch": (_i, [_vp, _i, _vp, _vp, _i, _d, _i, _dp]),
     "ddamg_reconstruct_odd_batch": (_i, [_vp, _i, _vp, _vp, _vp]),
     "ddamg_prepare_rhs_batch": (_i, [_vp, _i, _vp, _vp, _vp]),
+    "ddamg_set_option": (_i, [_vp, ctypes.c_char_p, _d]),
     "ddamg_launch_count": (ctypes.c_longlong, [_vp]),
     "ddamg_kernel_timing": (_i, [_vp, _i]),
     "ddamg_kernel_time_ms": (_i, [_vp, _i, _dp, _llp, _i]),
@@ -273,6 +274,9 @@ class Ddamg:
         self._ck(self.lib.ddamg_prepare_rhs_batch(self._h, nrhs, _ptr(B_e), _ptr(B_o), _ptr(Bhat_e)),
                  "ddamg_prepare_rhs_batch")
         return Bhat_e
+
+    def set_option(self, name: str, value: float):
+        self._ck(self.lib.ddamg_set_option(self._h, name.encode(), float(value)), "ddamg_set_option")
 
     # -- accounting ---------------------------------------------------------------
     def launch_count(self) -> int:

@@ -31,6 +31,7 @@ struct ddamg_ctx {
     void* tmp_batch;            // multi-rhs t_o (batch_cap half spinors)
     double* partials_batch;     // multi-rhs reduction scratch
     int batch_cap;
+    double batch_l2_bytes;      // L2 budget of the z-chunked multi-rhs traversal (option "batch_l2_bytes")
     double* partials;           // reduction scratch
     size_t partials_len;
     Scalars* sc;                // device scalars
@@ -122,7 +123,7 @@ extern "C" int ddamg_create(ddamg_ctx** out, int L, int T, double csw, double m0
     ctx->half_bytes = ctx->nreal * ctx->real_bytes;
     ctx->gauge = ctx->clov[0] = ctx->clov[1] = ctx->tmp_o = ctx->tmp_e = ctx->krylov = nullptr;
     ctx->kcap = 0;
-    ctx->tmp_batch = nullptr; ctx->partials_batch = nullptr; ctx->batch_cap = 0;
+    ctx->tmp_batch = nullptr; ctx->partials_batch = nullptr; ctx->batch_cap = 0; ctx->batch_l2_bytes = 40e6;
     ctx->partials = nullptr; ctx->sc = nullptr; ctx->host_hist = nullptr; ctx->singular = nullptr;
     ctx->have_gauge = ctx->have_clover = false;
     ctx->sticky = DDAMG_OK; ctx->launches = 0; ctx->timing = false;
@@ -266,10 +267,10 @@ static int dslash(ddamg_ctx* ctx, int epi, bool norm, int parity, const void* in
     }
     if (ctx->prec == DDAMG_F32)
         launch_dslash<float>(ctx->g, epi, norm, parity, in, gauge_block(ctx, parity), gauge_block(ctx, 1 - parity),
-                             ctx->clov[parity], own, rhs, out, omega, partials, nrhs, ctx->stream);
+                             ctx->clov[parity], own, rhs, out, omega, partials, nrhs, ctx->batch_l2_bytes, ctx->stream);
     else
         launch_dslash<double>(ctx->g, epi, norm, parity, in, gauge_block(ctx, parity), gauge_block(ctx, 1 - parity),
-                              ctx->clov[parity], own, rhs, out, omega, partials, nrhs, ctx->stream);
+                              ctx->clov[parity], own, rhs, out, omega, partials, nrhs, ctx->batch_l2_bytes, ctx->stream);
     if (ctx->timing) {
         cudaEventRecord(ev.b, ctx->stream);
         ctx->events.push_back(ev);
@@ -653,6 +654,19 @@ extern "C" int ddamg_power_iteration(ddamg_ctx* ctx, void* v_e, int iters, doubl
     CK(cudaMemcpyAsync(lambda_max, (char*)ctx->sc + offsetof(Scalars, value), sizeof(double), cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
     return DDAMG_OK;
+}
+
+// --------------------------------------------------------------------------- options
+extern "C" int ddamg_set_option(ddamg_ctx* ctx, const char* name, double value)
+{
+    ENTER(ctx);
+    if (!name) return fail(ctx, DDAMG_EINVAL, "ddamg_set_option: name is NULL");
+    if (strcmp(name, "batch_l2_bytes") == 0) {
+        if (!(value >= 0.0)) return fail(ctx, DDAMG_EINVAL, "ddamg_set_option: batch_l2_bytes must be >= 0");
+        ctx->batch_l2_bytes = value;
+        return DDAMG_OK;
+    }
+    return fail(ctx, DDAMG_EINVAL, std::string("ddamg_set_option: unknown option ") + name);
 }
 
 // --------------------------------------------------------------------------- kernel timing

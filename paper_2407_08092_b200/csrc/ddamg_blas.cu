@@ -181,26 +181,31 @@ void launch_multi_dot(size_t nreal, int nb, const void* V, size_t vstride_real, 
     const size_t nvec = nreal / VecOf<T>::N, vs = vstride_real / VecOf<T>::N;
     const int grid = blas_grid(nvec);
 #define MD(NB) case NB: multi_dot_kernel<T, NB><<<grid, BLAS_THREADS, 0, st>>>(nvec, (const VT*)V, vs, (const VT*)w, partials); break;
-    switch (nb) { MD(1) MD(2) MD(3) MD(4) MD(5) MD(6) MD(7) MD(8) }
+    switch (nb) { MD(1) MD(2) MD(3) MD(4) MD(5) MD(6) MD(7) MD(8) MD(9) MD(10) MD(11) MD(12) }
+    static_assert(MDOT_NB == 12, "one case per NB");
 #undef MD
 }
 template void launch_multi_dot<float>(size_t, int, const void*, size_t, const void*, double*, cudaStream_t);
 template void launch_multi_dot<double>(size_t, int, const void*, size_t, const void*, double*, cudaStream_t);
 
-// hcol[first .. first+nb-1] = sum over blocks; negh = -hcol
+// hcol[first .. first+nb-1] = sum over blocks; negh = -hcol.  One warp per real component,
+// lanes stride over the blocks, fixed shuffle tree: deterministic.
 __global__ void finalize_dots_kernel(const double* __restrict__ partials, int nblocks, int nb, Scalars* sc, int first)
 {
-    const int c = threadIdx.x;          // one thread per real component
+    const int c = threadIdx.x >> 5, lane = threadIdx.x & 31;
     if (c < 2 * nb) {
         double s = 0;
-        for (int b = 0; b < nblocks; ++b) s += partials[(size_t)b * 2 * nb + c];
-        sc->hcol[2 * first + c] = s;
-        sc->negh[2 * first + c] = -s;
+        for (int b = lane; b < nblocks; b += 32) s += partials[(size_t)b * 2 * nb + c];
+        s = warp_sum(s);
+        if (lane == 0) {
+            sc->hcol[2 * first + c] = s;
+            sc->negh[2 * first + c] = -s;
+        }
     }
 }
 void launch_finalize_dots(const double* partials, int nblocks, int nb, Scalars* sc, int first, cudaStream_t st)
 {
-    finalize_dots_kernel<<<1, 32, 0, st>>>(partials, nblocks, nb, sc, first);
+    finalize_dots_kernel<<<1, 32 * 2 * MDOT_NB, 0, st>>>(partials, nblocks, nb, sc, first);
 }
 
 // ------------------------------------------------------------------ w += sum_i coef_i v_i  (+ |w|^2)
@@ -243,7 +248,7 @@ void launch_multi_axpy(size_t nreal, int nb, const void* V, size_t vstride_real,
     const size_t nvec = nreal / VecOf<T>::N, vs = vstride_real / VecOf<T>::N;
     const int grid = blas_grid(nvec);
 #define MA(NB) case NB: multi_axpy_kernel<T, NB><<<grid, BLAS_THREADS, 0, st>>>(nvec, (const VT*)V, vs, coef, (VT*)w, partials); break;
-    switch (nb) { MA(1) MA(2) MA(3) MA(4) MA(5) MA(6) MA(7) MA(8) }
+    switch (nb) { MA(1) MA(2) MA(3) MA(4) MA(5) MA(6) MA(7) MA(8) MA(9) MA(10) MA(11) MA(12) }
 #undef MA
 }
 template void launch_multi_axpy<float>(size_t, int, const void*, size_t, const double*, void*, double*, cudaStream_t);

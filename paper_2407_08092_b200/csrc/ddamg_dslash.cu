@@ -28,6 +28,8 @@ struct DslashArgs {
     T omega;
     double* partials;        // per-block sum of |r|^2 (NORM) or nullptr; batch: [block][nrhs]
     int nrhs;                // BATCH kernels: right-hand sides interleaved per site (else 1)
+    int zc;                  // BATCH: z-chunk of the CTA traversal (0 = plain lexicographic order)
+    int cpp;                 // BATCH: CTAs per (z,t) plane = Lh * L * nrhs / DSLASH_THREADS (when zc > 0)
 };
 
 __device__ __forceinline__ double block_sum(double v)
@@ -65,7 +67,19 @@ __global__ void __launch_bounds__(DSLASH_THREADS)
 __maxnreg__(sizeof(T) == 4 ? (EPI <= EPI_RHS_MINUS_HOP ? DDAMG_MAXREG_A : DDAMG_MAXREG_B) : 255)
 dslash_kernel(const DslashArgs<T> a)
 {
-    const int tid = blockIdx.x * DSLASH_THREADS + threadIdx.x;
+    // BATCH: with nrhs spinors per site one time slice of neighbour spinors no longer fits L2
+    // (64^3: nrhs * 12.6 MB), so the t-1 neighbours would be re-fetched from HBM.  CTAs therefore
+    // walk the lattice in z-chunks: for each chunk of zc z-planes, t runs over the whole time
+    // extent before the next chunk starts, which keeps three t-slabs of the chunk L2-resident.
+    int blk = blockIdx.x;
+    if (BATCH && a.zc > 0) {
+        const int plane = blk / a.cpp, within = blk - plane * a.cpp;     // plane in chunked order
+        const int per_chunk = a.zc * a.g.T;
+        const int chunk = plane / per_chunk, rem = plane - chunk * per_chunk;
+        const int t = rem / a.zc, z = chunk * a.zc + (rem - t * a.zc);
+        blk = (t * a.g.L + z) * a.cpp + within;
+    }
+    const int tid = blk * DSLASH_THREADS + threadIdx.x;
     const int nrhs = BATCH ? a.nrhs : 1;
     const int cb = BATCH ? tid / nrhs : tid;
     const int rr = BATCH ? tid - cb * nrhs : 0;
@@ -119,12 +133,12 @@ dslash_kernel(const DslashArgs<T> a)
             per_thread[threadIdx.x] = nrm;
             __syncthreads();
             if ((int)threadIdx.x < nrhs) {
-                const int first = (int)(((long long)blockIdx.x * DSLASH_THREADS) % nrhs);   // rhs of thread 0
+                const int first = (int)(((long long)blk * DSLASH_THREADS) % nrhs);          // rhs of thread 0
                 int i = (int)threadIdx.x - first;
                 if (i < 0) i += nrhs;
                 double tot = 0.0;
                 for (; i < DSLASH_THREADS; i += nrhs) tot += per_thread[i];
-                a.partials[(size_t)blockIdx.x * nrhs + threadIdx.x] = tot;
+                a.partials[(size_t)blk * nrhs + threadIdx.x] = tot;
             }
         } else {
             const double tot = block_sum(nrm);
@@ -144,10 +158,25 @@ static void launch(const DslashArgs<T>& a, cudaStream_t st)
 template <typename T>
 void launch_dslash(const Geom& g, int epi, bool norm, int parity, const void* in, const void* gauge_own,
                    const void* gauge_opp, const void* clov, const void* own, const void* rhs, void* out,
-                   double omega, double* partials, int nrhs, cudaStream_t st)
+                   double omega, double* partials, int nrhs, double batch_l2_bytes, cudaStream_t st)
 {
     DslashArgs<T> a;
     a.nrhs = nrhs;
+    a.zc = 0;
+    a.cpp = 0;
+    const long long plane_threads = (long long)g.Lh * g.L * nrhs;
+    if (nrhs > 1 && plane_threads % DSLASH_THREADS == 0) {
+        // largest divisor zc of L whose three t-slabs of spinors (zc planes each) fit the L2 budget
+        const double plane_bytes = (double)g.Lh * g.L * nrhs * 24 * sizeof(T);
+        int zc = 0;
+        for (int d = 1; d <= g.L; ++d)
+            if (g.L % d == 0 && 3.0 * d * plane_bytes <= batch_l2_bytes) zc = d;
+        if (zc == 0) zc = 1;
+        if (zc < g.L) {
+            a.zc = zc;
+            a.cpp = (int)(plane_threads / DSLASH_THREADS);
+        }
+    }
     a.g = g;
     a.parity = parity;
     a.in = (const T*)in;
@@ -176,9 +205,9 @@ void launch_dslash(const Geom& g, int epi, bool norm, int parity, const void* in
 }
 
 template void launch_dslash<float>(const Geom&, int, bool, int, const void*, const void*, const void*, const void*,
-                                   const void*, const void*, void*, double, double*, int, cudaStream_t);
+                                   const void*, const void*, void*, double, double*, int, double, cudaStream_t);
 template void launch_dslash<double>(const Geom&, int, bool, int, const void*, const void*, const void*, const void*,
-                                    const void*, const void*, void*, double, double*, int, cudaStream_t);
+                                    const void*, const void*, void*, double, double*, int, double, cudaStream_t);
 
 // out = Cl in on one parity (right factor of eq. 2: t_o = A_oo^-1 b_o)
 template <typename T>

@@ -14,7 +14,7 @@ constexpr int BLAS_THREADS = 256;
 constexpr int GMRES_KMAX = 64;          // largest cycle length m of GMRES(n, m)
 constexpr int HIST_MAX = 8192;         // residual-history entries kept on the device
 constexpr int NRHS_MAX = 32;            // right-hand sides per multi-rhs batch
-constexpr int MDOT_NB = 8;              // basis vectors handled per fused multi-dot / multi-axpy pass
+constexpr int MDOT_NB = 12;             // basis vectors handled per fused multi-dot / multi-axpy pass
 
 // epilogues of the fused hopping kernel (ddamg_dslash.cu)
 enum {
@@ -29,7 +29,7 @@ enum {
 template <typename T>
 void launch_dslash(const Geom& g, int epi, bool norm, int parity, const void* in, const void* gauge_own,
                    const void* gauge_opp, const void* clov, const void* own, const void* rhs, void* out,
-                   double omega, double* partials, int nrhs, cudaStream_t st);
+                   double omega, double* partials, int nrhs, double batch_l2_bytes, cudaStream_t st);
 template <typename T>
 void launch_clover_apply(const Geom& g, const void* clov, const void* in, void* out, int nrhs, cudaStream_t st);
 int dslash_grid(const Geom& g, int nrhs = 1);

@@ -120,3 +120,29 @@ def test_batch_error_codes():
     fresh = dd.Ddamg(4, 4, 1.0, 0.0, 1, dd.F32)
     assert fresh.lib.ddamg_apply_schur_batch(fresh._h, 2, vp(X), vp(Y)) == dd.binding.ESTATE
     assert lib.ddamg_apply_schur_batch(h, 2, vp(X), vp(Y)) == dd.binding.OK
+
+
+@pytest.mark.parametrize("budget", [0.0, 3 * 2 * 4 * 8 * 4 * 96.0, 1e12])
+def test_batch_z_chunked_traversal_is_bit_identical(budget):
+    """The z-chunked CTA order (option batch_l2_bytes) only permutes which CTA does which sites:
+    results, including the per-rhs residual history, are bit-identical to the single-rhs path.
+    8^3 x 6, nrhs = 4: one (z,t) plane = 4 * 8 * 4 threads = 1 CTA, so chunking is active for
+    budget 0 (zc = 1) and for a budget of two planes (zc = 2), and off for the huge one."""
+    p = make_pair(3, "f32", 8, 6)
+    nrhs, nu, omega = 4, 3, 0.9
+    _, bh = _spinors(p, nrhs, 7500)
+    _, xh = _spinors(p, nrhs, 7600)
+    p.ctx.set_option("batch_l2_bytes", budget)
+    B_e = p.ctx.batch_interleave([h[0] for h in bh])
+    X_e = p.ctx.batch_interleave([h[0] for h in xh])
+    Y = p.ctx.batch_deinterleave(nrhs, p.ctx.apply_schur_batch(nrhs, X_e))
+    hist = p.ctx.richardson_batch(nrhs, B_e, X_e, nu, omega, history=True)
+    got = p.ctx.batch_deinterleave(nrhs, X_e)
+    for r in range(nrhs):
+        assert torch.equal(Y[r], p.ctx.apply_schur(xh[r][0]))
+        x1 = xh[r][0].clone()
+        h1 = p.ctx.richardson(bh[r][0], x1, nu, omega, history=True)
+        assert torch.equal(got[r], x1)
+        assert np.allclose([hist[i][r] for i in range(nu)], h1, rtol=1e-13, atol=0)
+    with pytest.raises(Exception):
+        p.ctx.set_option("no_such_option", 1.0)
