@@ -134,4 +134,4 @@ class WilsonClover:
         return M
 
 
-from .iterations import richardson, richardson_multi, gmres, power_iteration  # noqa: E402,F401
+from .iterations import richardson, richardson_multi, gmres, gcr, fgmres, power_iteration  # noqa: E402,F401

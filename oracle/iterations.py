@@ -134,3 +134,116 @@ def richardson_multi(apply, B, X0, nu: int, omega: float):
         xs.append(x)
         hists.append(h)
     return xs, [[hists[r][i] for r in range(len(xs))] for i in range(nu)]
+
+
+def gcr(apply, b, x0, k: int, cycles: int, tol: float = 0.0):
+    """Alg. 3 (PAPER.md:113-131 and the algorithm box after it): GCR(n = cycles, m = k) on D x = b.
+
+    Followed line by line: p_1 = r, z_1 = D p_1; for each step delta_k = (z_k, z_k),
+    alpha = (r, z_k)/delta_k, x += alpha p_k, r -= alpha z_k, w = D r,
+    beta_j = -(w, z_j)/delta_j, p_{k+1} = r + sum beta_j p_j, z_{k+1} = w + sum beta_j z_j.
+    Inner products are conjugate-linear in the direction vector z (reading R8): (a, z) = z^H a.
+    The D r / p_{k+1} / z_{k+1} of the last step of a cycle are never used and are skipped.
+    History (same layout as ``gmres``, R13): the true ||b - D x|| at the start of every cycle,
+    then ||r|| after each of the k updates of line 8 (the recursively updated residual), and
+    the true residual norm at the end.  With tol > 0 (R10) stop as soon as ||r|| <= tol ||b||.
+    """
+    x = np.array(x0, dtype=np.complex128, copy=True)
+    bnorm = _norm(b)
+    hist = []
+    done = False
+    for _ in range(cycles):
+        r = b - apply(x)                                   # line 2
+        hist.append(_norm(r))
+        if tol > 0.0 and hist[-1] <= tol * bnorm:          # line 3
+            done = True
+            break
+        P = [r.copy()]                                     # line 4: p_1 = r
+        Z = [apply(P[0])]                                  #         z_1 = D p_1
+        delta = []
+        for j in range(k):                                 # line 5
+            delta.append(np.vdot(Z[j], Z[j]).real)         # line 6
+            alpha = np.vdot(Z[j], r) / delta[j]            # line 7: (r, z_k) / delta_k
+            x = x + alpha * P[j]                           # line 8
+            r = r - alpha * Z[j]                           # line 9
+            hist.append(_norm(r))
+            if tol > 0.0 and hist[-1] <= tol * bnorm:
+                break
+            if j == k - 1:
+                break
+            w = apply(r)                                   # line 10
+            p_new = r.copy()
+            z_new = w.copy()
+            for i in range(j + 1):                         # line 11
+                beta = -np.vdot(Z[i], w) / delta[i]        # line 12
+                p_new = p_new + beta * P[i]                # line 13
+                z_new = z_new + beta * Z[i]                # line 14
+            P.append(p_new)
+            Z.append(z_new)
+    if not done:
+        hist.append(_norm(b - apply(x)))
+    return x, hist
+
+
+def fgmres(apply, precond, b, x0, k: int, cycles: int, tol: float = 0.0, return_basis: bool = False):
+    """Flexible GMRES(n = cycles, m = k): the outer solver of DD-alphaAMG (PAPER.md:77,
+    "FGMRES ... preconditioned by" the multigrid cycle; here by the smoother alone).
+
+    The paper prints no algorithm for it; this is Alg. 2 with the one change that makes GMRES
+    flexible (reading R19): the Krylov vector is preconditioned before the operator is
+    applied, z_j = M(v_j), w = D z_j, the z_j are kept, and the update is x += Z_m y.
+    ``precond`` may be any (even non-linear) map.  History layout as in ``gmres``.
+    """
+    x = np.array(x0, dtype=np.complex128, copy=True)
+    bnorm = _norm(b)
+    hist = []
+    Zs = None
+    done = False
+    for _ in range(cycles):
+        r = b - apply(x)
+        beta = _norm(r)
+        hist.append(beta)
+        if tol > 0.0 and beta <= tol * bnorm:
+            done = True
+            break
+        V = [r / beta]
+        Zs = []
+        H = np.zeros((k + 1, k), dtype=np.complex128)
+        cs = np.zeros(k, dtype=np.complex128)
+        sn = np.zeros(k, dtype=np.complex128)
+        g = np.zeros(k + 1, dtype=np.complex128)
+        g[0] = beta
+        m = 0
+        for j in range(k):
+            Zs.append(precond(V[j]))                       # z_j = M v_j
+            w = apply(Zs[j])                               # w = D z_j
+            for i in range(j + 1):
+                H[i, j] = np.vdot(V[i], w)
+                w = w - H[i, j] * V[i]
+            H[j + 1, j] = _norm(w)
+            V.append(w / H[j + 1, j] if H[j + 1, j].real > 0.0 else np.zeros_like(w))
+            for i in range(j):
+                t = cs[i] * H[i, j] + sn[i] * H[i + 1, j]
+                H[i + 1, j] = -np.conj(sn[i]) * H[i, j] + np.conj(cs[i]) * H[i + 1, j]
+                H[i, j] = t
+            a, c = H[j, j], H[j + 1, j]
+            d = np.sqrt(abs(a) ** 2 + abs(c) ** 2)
+            cs[j], sn[j] = np.conj(a) / d, np.conj(c) / d
+            H[j, j] = cs[j] * a + sn[j] * c
+            H[j + 1, j] = 0.0
+            g[j + 1] = -np.conj(sn[j]) * g[j]
+            g[j] = cs[j] * g[j]
+            hist.append(abs(g[j + 1]))
+            m = j + 1
+            if tol > 0.0 and abs(g[j + 1]) <= tol * bnorm:
+                break
+        y = np.zeros(m, dtype=np.complex128)
+        for i in range(m - 1, -1, -1):
+            y[i] = (g[i] - np.dot(H[i, i + 1:m], y[i + 1:m])) / H[i, i]
+        for i in range(m):
+            x = x + y[i] * Zs[i]                           # x += Z_m y
+    if not done:
+        hist.append(_norm(b - apply(x)))
+    if return_basis:
+        return x, hist, Zs
+    return x, hist
