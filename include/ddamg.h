@@ -134,6 +134,17 @@ int ddamg_richardson(ddamg_ctx* ctx, const void* b_e, void* x_e, int nu, double 
 int ddamg_gmres_oe(ddamg_ctx* ctx, const void* b_e, void* x_e, int k, int cycles, double tol,
                    int zero_init, double* res_hist, int* n_hist);
 
+/*
+ * Alg. 3: GCR(n = cycles, m = k) on D_S x_e = b_e -- SURVEY.md NEXT-4.
+ * Arguments, history layout (cycles*(k+1)+1 entries: true residual at each cycle start, the
+ * recursively updated ||r|| after each of the k steps, true residual at the end), tol and
+ * error behaviour as ddamg_gmres_oe.  Mathematically equivalent to GMRES but
+ * keeps 2k+1 half spinors (p_j, z_j = D_S p_j, r) and does one D_S application per step;
+ * lines 11-14 run as one fused pass that also yields delta_{k+1} and (r, z_{k+1}).
+ */
+int ddamg_gcr_oe(ddamg_ctx* ctx, const void* b_e, void* x_e, int k, int cycles, double tol,
+                 int zero_init, double* res_hist, int* n_hist);
+
 /* eq. 2, left factor:  x_o = A_oo^-1 (b_o - H_oe x_e). */
 int ddamg_reconstruct_odd(ddamg_ctx* ctx, const void* b_o, const void* x_e, void* x_o);
 

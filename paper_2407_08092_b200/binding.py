@@ -36,6 +36,7 @@ SYMBOLS = {
     "ddamg_apply_schur": (_i, [_vp, _vp, _vp]),
     "ddamg_richardson": (_i, [_vp, _vp, _vp, _i, _d, _i, _dp]),
     "ddamg_gmres_oe": (_i, [_vp, _vp, _vp, _i, _i, _d, _i, _dp, _ip]),
+    "ddamg_gcr_oe": (_i, [_vp, _vp, _vp, _i, _i, _d, _i, _dp, _ip]),
     "ddamg_reconstruct_odd": (_i, [_vp, _vp, _vp, _vp]),
     "ddamg_prepare_rhs": (_i, [_vp, _vp, _vp, _vp]),
     "ddamg_power_iteration": (_i, [_vp, _vp, _i, _dp]),
@@ -193,6 +194,16 @@ class Ddamg:
         nh = ctypes.c_int(0)
         self._ck(self.lib.ddamg_gmres_oe(self._h, _ptr(b_e), _ptr(x_e), k, cycles, tol, int(zero_init), hist,
                                          ctypes.byref(nh)), "ddamg_gmres_oe")
+        return list(hist)[:nh.value]
+
+    def gcr_oe(self, b_e: torch.Tensor, x_e: torch.Tensor, k: int, cycles: int, tol: float = 0.0,
+               zero_init: bool = False):
+        self._chk_half(b_e, x_e)
+        n = cycles * (k + 1) + 1
+        hist = (ctypes.c_double * n)()
+        nh = ctypes.c_int(0)
+        self._ck(self.lib.ddamg_gcr_oe(self._h, _ptr(b_e), _ptr(x_e), k, cycles, tol, int(zero_init), hist,
+                                       ctypes.byref(nh)), "ddamg_gcr_oe")
         return list(hist)[:nh.value]
 
     def reconstruct_odd(self, b_o: torch.Tensor, x_e: torch.Tensor, x_o: Optional[torch.Tensor] = None):

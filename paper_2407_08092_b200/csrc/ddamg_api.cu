@@ -622,6 +622,134 @@ extern "C" int ddamg_gmres_oe(ddamg_ctx* ctx, const void* b_e, void* x_e, int k,
     return gmres_impl<double>(ctx, b_e, x_e, k, cycles, tol, zero_init, res_hist, n_hist);
 }
 
+// --------------------------------------------------------------------------- GCR (NEXT-4)
+static int ensure_krylov(ddamg_ctx* ctx, int nvec, const char* who)
+{
+    if (nvec <= ctx->kcap + 1) return DDAMG_OK;
+    CK(cudaStreamSynchronize(ctx->stream));
+    cudaFree(ctx->krylov);
+    ctx->krylov = nullptr; ctx->kcap = 0;
+    cudaError_t e = cudaMalloc(&ctx->krylov, (size_t)nvec * ctx->half_bytes);
+    if (e != cudaSuccess) { cudaGetLastError(); return fail(ctx, DDAMG_ENOMEM, std::string(who) + ": cannot allocate the Krylov vectors"); }
+    ctx->kcap = nvec - 1;
+    return DDAMG_OK;
+}
+
+template <typename T>
+static int gcr_impl(ddamg_ctx* ctx, const void* b_e, void* x_e, int k, int cycles, double tol, int zero_init,
+                    double* res_hist, int* n_hist)
+{
+    cudaStream_t st = ctx->stream;
+    const size_t nreal = ctx->nreal;
+    const int vecN = (int)(16 / ctx->real_bytes);
+    const int bgrid = blas_grid(nreal / vecN);
+    const int dgrid = dslash_grid(ctx->g);
+    char* base = (char*)ctx->krylov;
+    auto P = [&](int j) { return (void*)(base + (size_t)j * ctx->half_bytes); };
+    auto Z = [&](int j) { return (void*)(base + (size_t)(k + j) * ctx->half_bytes); };
+    void* r = (void*)(base + (size_t)(2 * k) * ctx->half_bytes);
+    double* alpha = (double*)((char*)ctx->sc + offsetof(Scalars, alpha));
+    double* beta = (double*)((char*)ctx->sc + offsetof(Scalars, negh));
+    int s = reset_hist(ctx);
+    if (s != DDAMG_OK) return s;
+    double bnorm = 0.0;
+    auto last_hist = [&](double* v) -> int {
+        int nh = 0;
+        CK(cudaMemcpyAsync(&nh, (char*)ctx->sc + offsetof(Scalars, nhist), sizeof(int), cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+        CK(cudaMemcpyAsync(v, (char*)ctx->sc + offsetof(Scalars, hist) + sizeof(double) * (nh - 1), sizeof(double), cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+        return DDAMG_OK;
+    };
+    if (tol > 0.0) {
+        launch_copy_norm<T>(nreal, b_e, r, ctx->partials, st);
+        launch_finalize_norm(ctx->partials, bgrid, ctx->sc, 0, st);
+        s = after_launch(ctx, 2); if (s != DDAMG_OK) return s;
+        CK(cudaMemcpyAsync(&bnorm, (char*)ctx->sc + offsetof(Scalars, value), sizeof(double), cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+    }
+    if (zero_init) CK(cudaMemsetAsync(x_e, 0, ctx->half_bytes, st));
+    bool converged = false;
+    for (int c = 0; c < cycles && !converged; ++c) {
+        // line 2: r = b - D_S x
+        if (zero_init && c == 0) {
+            launch_copy_norm<T>(nreal, b_e, r, ctx->partials, st);
+            s = after_launch(ctx); if (s != DDAMG_OK) return s;
+            launch_finalize_norm(ctx->partials, bgrid, ctx->sc, 1, st);
+        } else {
+            s = dslash(ctx, EPI_CLOV_HOP, false, 1, x_e, nullptr, nullptr, ctx->tmp_o, 0.0, 0);
+            if (s != DDAMG_OK) return s;
+            s = dslash(ctx, EPI_RESIDUAL, true, 0, ctx->tmp_o, x_e, b_e, r, 0.0, 1);
+            if (s != DDAMG_OK) return s;
+            launch_finalize_norm(ctx->partials, dgrid, ctx->sc, 1, st);
+        }
+        s = after_launch(ctx); if (s != DDAMG_OK) return s;
+        if (tol > 0.0) {
+            double v = 0.0;
+            s = last_hist(&v); if (s != DDAMG_OK) return s;
+            if (v <= tol * bnorm) { converged = true; break; }
+        }
+        // line 4: z_1 = D_S r (p_1 = r is written by the form pass, which also gives delta_1, <z_1, r>)
+        s = schur(ctx, r, Z(0));
+        if (s != DDAMG_OK) return s;
+        launch_gcr_form<T>(nreal, 0, nullptr, nullptr, nreal, nullptr, Z(0), r, P(0), 1, ctx->partials, st);
+        s = after_launch(ctx); if (s != DDAMG_OK) return s;
+        for (int j = 0; j < k; ++j) {
+            launch_gcr_alpha(ctx->partials, bgrid, ctx->sc, j, st);                       // lines 6-7
+            launch_gcr_update<T>(nreal, alpha, P(j), Z(j), x_e, r, ctx->partials, st);    // lines 8-9
+            launch_finalize_norm(ctx->partials, bgrid, ctx->sc, 1, st);
+            s = after_launch(ctx, 3); if (s != DDAMG_OK) return s;
+            if (tol > 0.0) {
+                double v = 0.0;
+                s = last_hist(&v); if (s != DDAMG_OK) return s;
+                if (v <= tol * bnorm) { converged = true; break; }
+            }
+            if (j == k - 1) break;
+            s = schur(ctx, r, Z(j + 1));                                                   // line 10: w = D_S r
+            if (s != DDAMG_OK) return s;
+            for (int i0 = 0; i0 <= j; i0 += MDOT_NB) {                                     // line 12
+                const int nb = (j + 1 - i0) < MDOT_NB ? (j + 1 - i0) : MDOT_NB;
+                launch_multi_dot<T>(nreal, nb, Z(i0), nreal, Z(j + 1), ctx->partials, st);
+                launch_finalize_dots(ctx->partials, bgrid, nb, ctx->sc, i0, st);
+                launch_gcr_beta(ctx->sc, i0, nb, st);
+                s = after_launch(ctx, 3); if (s != DDAMG_OK) return s;
+            }
+            for (int i0 = 0; i0 <= j; i0 += MDOT_NB) {                                     // lines 13-14
+                const int nb = (j + 1 - i0) < MDOT_NB ? (j + 1 - i0) : MDOT_NB;
+                const bool last = i0 + MDOT_NB > j;
+                launch_gcr_form<T>(nreal, nb, Z(i0), P(i0), nreal, beta + 2 * i0, Z(j + 1), r, P(j + 1), i0 == 0,
+                                   last ? ctx->partials : nullptr, st);
+                s = after_launch(ctx); if (s != DDAMG_OK) return s;
+            }
+        }
+    }
+    if (!converged) {
+        s = dslash(ctx, EPI_CLOV_HOP, false, 1, x_e, nullptr, nullptr, ctx->tmp_o, 0.0, 0);
+        if (s != DDAMG_OK) return s;
+        s = dslash(ctx, EPI_RESIDUAL, true, 0, ctx->tmp_o, x_e, b_e, r, 0.0, 1);
+        if (s != DDAMG_OK) return s;
+        launch_finalize_norm(ctx->partials, dgrid, ctx->sc, 1, st);
+        s = after_launch(ctx); if (s != DDAMG_OK) return s;
+    }
+    return copy_hist(ctx, res_hist, cycles * (k + 1) + 1, n_hist);
+}
+
+extern "C" int ddamg_gcr_oe(ddamg_ctx* ctx, const void* b_e, void* x_e, int k, int cycles, double tol, int zero_init,
+                            double* res_hist, int* n_hist)
+{
+    ENTER(ctx);
+    if (!b_e || !x_e || b_e == x_e || k < 1 || cycles < 1 || tol < 0.0)
+        return fail(ctx, DDAMG_EINVAL, "ddamg_gcr_oe: bad arguments");
+    if (k > GMRES_KMAX) return fail(ctx, DDAMG_EINVAL, "ddamg_gcr_oe: k exceeds 64");
+    if ((long long)cycles * (k + 1) + 1 > HIST_MAX) return fail(ctx, DDAMG_EINVAL, "ddamg_gcr_oe: history too long");
+    int s = need_ready(ctx, "ddamg_gcr_oe");
+    if (s != DDAMG_OK) return s;
+    s = ensure_krylov(ctx, 2 * k + 1, "ddamg_gcr_oe");
+    if (s != DDAMG_OK) return s;
+    if (ctx->prec == DDAMG_F32) return gcr_impl<float>(ctx, b_e, x_e, k, cycles, tol, zero_init, res_hist, n_hist);
+    return gcr_impl<double>(ctx, b_e, x_e, k, cycles, tol, zero_init, res_hist, n_hist);
+}
+
 // --------------------------------------------------------------------------- power iteration
 extern "C" int ddamg_power_iteration(ddamg_ctx* ctx, void* v_e, int iters, double* lambda_max)
 {

@@ -254,6 +254,150 @@ void launch_multi_axpy(size_t nreal, int nb, const void* V, size_t vstride_real,
 template void launch_multi_axpy<float>(size_t, int, const void*, size_t, const double*, void*, double*, cudaStream_t);
 template void launch_multi_axpy<double>(size_t, int, const void*, size_t, const double*, void*, double*, cudaStream_t);
 
+// ------------------------------------------------------------------ GCR (Alg. 3)
+// lines 11-14 in one pass:  z = w + sum_j beta_j z_j  (in place on w),  p = r + sum_j beta_j p_j,
+// plus the partial sums the next step needs: |z|^2 (line 6) and <z, r> (line 7).
+// NB = 0 is the start of a cycle: p_1 = r, z_1 = D p_1 untouched, same partial sums.
+template <typename T, int NB>
+__global__ void __launch_bounds__(BLAS_THREADS)
+gcr_form_kernel(size_t nvec, const typename VecOf<T>::type* __restrict__ Z0,
+                const typename VecOf<T>::type* __restrict__ P0, size_t vstride,
+                const double* __restrict__ coef, typename VecOf<T>::type* __restrict__ z_io,
+                const typename VecOf<T>::type* __restrict__ r, typename VecOf<T>::type* __restrict__ p_out,
+                int init_p, double* __restrict__ partials)
+{
+    constexpr int N = VecOf<T>::N;
+    double cr[NB > 0 ? NB : 1], ci[NB > 0 ? NB : 1];
+#pragma unroll
+    for (int b = 0; b < NB; ++b) { cr[b] = coef[2 * b]; ci[b] = coef[2 * b + 1]; }
+    double acc[3] = { 0.0, 0.0, 0.0 };
+    for (size_t i = (size_t)blockIdx.x * BLAS_THREADS + threadIdx.x; i < nvec; i += (size_t)gridDim.x * BLAS_THREADS) {
+        double zr[N], pr[N], rr[N];
+        cvt(z_io[i], zr);
+        cvt(r[i], rr);
+        if (init_p) {
+#pragma unroll
+            for (int c = 0; c < N; ++c) pr[c] = rr[c];
+        } else {
+            cvt(p_out[i], pr);
+        }
+#pragma unroll
+        for (int b = 0; b < NB; ++b) {
+            double zv[N], pv[N];
+            cvt(Z0[(size_t)b * vstride + i], zv);
+            cvt(P0[(size_t)b * vstride + i], pv);
+#pragma unroll
+            for (int c = 0; c < N; c += 2) {
+                zr[c] += cr[b] * zv[c] - ci[b] * zv[c + 1];
+                zr[c + 1] += cr[b] * zv[c + 1] + ci[b] * zv[c];
+                pr[c] += cr[b] * pv[c] - ci[b] * pv[c + 1];
+                pr[c + 1] += cr[b] * pv[c + 1] + ci[b] * pv[c];
+            }
+        }
+        T zo[N], po[N];
+#pragma unroll
+        for (int c = 0; c < N; ++c) { zo[c] = (T)zr[c]; po[c] = (T)pr[c]; }
+        if (NB > 0) z_io[i] = pack(zo);
+        p_out[i] = pack(po);
+        if (partials) {
+#pragma unroll
+            for (int c = 0; c < N; c += 2) {              // conj(z) * r
+                const double a = zo[c], bq = zo[c + 1];
+                acc[0] += a * a + bq * bq;
+                acc[1] += a * rr[c] + bq * rr[c + 1];
+                acc[2] += a * rr[c + 1] - bq * rr[c];
+            }
+        }
+    }
+    if (partials) block_sum_n<3>(acc, partials + (size_t)blockIdx.x * 3);
+}
+template <typename T>
+void launch_gcr_form(size_t nreal, int nb, const void* Z0, const void* P0, size_t vstride_real, const double* coef,
+                     void* z_io, const void* r, void* p_out, int init_p, double* partials, cudaStream_t st)
+{
+    using VT = typename VecOf<T>::type;
+    const size_t nvec = nreal / VecOf<T>::N, vs = vstride_real / VecOf<T>::N;
+    const int grid = blas_grid(nvec);
+#define GF(NB) case NB: gcr_form_kernel<T, NB><<<grid, BLAS_THREADS, 0, st>>>(nvec, (const VT*)Z0, (const VT*)P0, vs, coef, (VT*)z_io, (const VT*)r, (VT*)p_out, init_p, partials); break;
+    switch (nb) { GF(0) GF(1) GF(2) GF(3) GF(4) GF(5) GF(6) GF(7) GF(8) GF(9) GF(10) GF(11) GF(12) }
+#undef GF
+}
+template void launch_gcr_form<float>(size_t, int, const void*, const void*, size_t, const double*, void*, const void*, void*, int, double*, cudaStream_t);
+template void launch_gcr_form<double>(size_t, int, const void*, const void*, size_t, const double*, void*, const void*, void*, int, double*, cudaStream_t);
+
+// lines 6-7: delta_j = sum |z|^2, alpha = <z, r> / delta_j  (partials[block][3] from gcr_form)
+__global__ void gcr_alpha_kernel(const double* __restrict__ partials, int nblocks, Scalars* sc, int j)
+{
+    const int c = threadIdx.x >> 5, lane = threadIdx.x & 31;       // 3 warps, one per component
+    __shared__ double tot[3];
+    double s = 0;
+    for (int b = lane; b < nblocks; b += 32) s += partials[(size_t)b * 3 + c];
+    s = warp_sum(s);
+    if (lane == 0) tot[c] = s;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        const double d = tot[0];
+        sc->delta[j] = d;
+        sc->alpha[0] = d > 0.0 ? tot[1] / d : 0.0;
+        sc->alpha[1] = d > 0.0 ? tot[2] / d : 0.0;
+    }
+}
+void launch_gcr_alpha(const double* partials, int nblocks, Scalars* sc, int j, cudaStream_t st)
+{
+    gcr_alpha_kernel<<<1, 96, 0, st>>>(partials, nblocks, sc, j);
+}
+
+// line 12: beta_i = -<z_i, w> / delta_i for i = first..first+nb-1 (hcol holds the dots) -> sc->negh
+__global__ void gcr_beta_kernel(Scalars* sc, int first, int nb)
+{
+    const int i = first + threadIdx.x;
+    if ((int)threadIdx.x < nb) {
+        const double d = sc->delta[i];
+        sc->negh[2 * i] = d > 0.0 ? -sc->hcol[2 * i] / d : 0.0;
+        sc->negh[2 * i + 1] = d > 0.0 ? -sc->hcol[2 * i + 1] / d : 0.0;
+    }
+}
+void launch_gcr_beta(Scalars* sc, int first, int nb, cudaStream_t st) { gcr_beta_kernel<<<1, 32, 0, st>>>(sc, first, nb); }
+
+// lines 8-9:  x += alpha p,  r -= alpha z,  partial |r|^2
+template <typename T>
+__global__ void __launch_bounds__(BLAS_THREADS)
+gcr_update_kernel(size_t nvec, const double* __restrict__ alpha, const typename VecOf<T>::type* __restrict__ p,
+                  const typename VecOf<T>::type* __restrict__ z, typename VecOf<T>::type* __restrict__ x,
+                  typename VecOf<T>::type* __restrict__ r, double* __restrict__ partials)
+{
+    constexpr int N = VecOf<T>::N;
+    const double ar = alpha[0], ai = alpha[1];
+    double acc[1] = { 0.0 };
+    for (size_t i = (size_t)blockIdx.x * BLAS_THREADS + threadIdx.x; i < nvec; i += (size_t)gridDim.x * BLAS_THREADS) {
+        double xv[N], rv[N], pv[N], zv[N];
+        cvt(x[i], xv); cvt(r[i], rv); cvt(p[i], pv); cvt(z[i], zv);
+        T xo[N], ro[N];
+#pragma unroll
+        for (int c = 0; c < N; c += 2) {
+            xo[c] = (T)(xv[c] + ar * pv[c] - ai * pv[c + 1]);
+            xo[c + 1] = (T)(xv[c + 1] + ar * pv[c + 1] + ai * pv[c]);
+            ro[c] = (T)(rv[c] - (ar * zv[c] - ai * zv[c + 1]));
+            ro[c + 1] = (T)(rv[c + 1] - (ar * zv[c + 1] + ai * zv[c]));
+        }
+#pragma unroll
+        for (int c = 0; c < N; ++c) acc[0] += (double)ro[c] * (double)ro[c];
+        x[i] = pack(xo);
+        r[i] = pack(ro);
+    }
+    block_sum_n<1>(acc, partials + blockIdx.x);
+}
+template <typename T>
+void launch_gcr_update(size_t nreal, const double* alpha, const void* p, const void* z, void* x, void* r,
+                       double* partials, cudaStream_t st)
+{
+    using VT = typename VecOf<T>::type;
+    const size_t nvec = nreal / VecOf<T>::N;
+    gcr_update_kernel<T><<<blas_grid(nvec), BLAS_THREADS, 0, st>>>(nvec, alpha, (const VT*)p, (const VT*)z, (VT*)x, (VT*)r, partials);
+}
+template void launch_gcr_update<float>(size_t, const double*, const void*, const void*, void*, void*, double*, cudaStream_t);
+template void launch_gcr_update<double>(size_t, const double*, const void*, const void*, void*, void*, double*, cudaStream_t);
+
 // ------------------------------------------------------------------ small dense part (1 thread)
 __global__ void gmres_begin_cycle_kernel(Scalars* sc)
 {

@@ -60,6 +60,8 @@ struct Scalars {
     double y[GMRES_KMAX * 2];                           // least-squares solution
     double hcol[(GMRES_KMAX + 1) * 2];                  // current column h_{1..j,j}
     double negh[(GMRES_KMAX + 1) * 2];                  // -hcol (axpy coefficients)
+    double delta[GMRES_KMAX];                           // GCR: delta_j = (z_j, z_j)
+    double alpha[2];                                    // GCR: alpha of the current step
     double scale;                                       // 1/beta or 1/h_{j+1,j}
     double value;                                       // last reduced norm
     int nhist;
@@ -83,6 +85,15 @@ void launch_finalize_dots(const double* partials, int nblocks, int nb, Scalars* 
 // w += sum_i coef[i] v_i (complex coef on device, nb <= MDOT_NB); optional |w|^2 partials
 template <typename T>
 void launch_multi_axpy(size_t nreal, int nb, const void* V, size_t vstride_real, const double* coef, void* w,
+                       double* partials, cudaStream_t st);
+// GCR (Alg. 3)
+template <typename T>
+void launch_gcr_form(size_t nreal, int nb, const void* Z0, const void* P0, size_t vstride_real, const double* coef,
+                     void* z_io, const void* r, void* p_out, int init_p, double* partials, cudaStream_t st);
+void launch_gcr_alpha(const double* partials, int nblocks, Scalars* sc, int j, cudaStream_t st);
+void launch_gcr_beta(Scalars* sc, int first, int nb, cudaStream_t st);
+template <typename T>
+void launch_gcr_update(size_t nreal, const double* alpha, const void* p, const void* z, void* x, void* r,
                        double* partials, cudaStream_t st);
 void launch_gmres_begin_cycle(Scalars* sc, cudaStream_t st);                 // g = beta e_1 (beta = sc->value)
 void launch_gmres_givens(Scalars* sc, int j, cudaStream_t st);               // after the norm of w is in sc->value
