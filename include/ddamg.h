@@ -60,6 +60,7 @@ enum {
 };
 enum { DDAMG_F32 = 0, DDAMG_F64 = 1 };
 enum { DDAMG_BC_PERIODIC = 0, DDAMG_BC_ANTIPERIODIC_T = 1 };
+enum { DDAMG_SMOOTHER_RICHARDSON = 0, DDAMG_SMOOTHER_GMRES = 1, DDAMG_SMOOTHER_GCR = 2 };
 
 /* Library version string, e.g. "ddamg-b200 0.1 (sm_100a)". Never NULL. */
 const char* ddamg_version(void);
@@ -144,6 +145,30 @@ int ddamg_gmres_oe(ddamg_ctx* ctx, const void* b_e, void* x_e, int k, int cycles
  */
 int ddamg_gcr_oe(ddamg_ctx* ctx, const void* b_e, void* x_e, int k, int cycles, double tol,
                  int zero_init, double* res_hist, int* n_hist);
+
+/*
+ * The full operator of eq. 1 on both parities:
+ *   y_e = A_ee x_e + H_eo x_o,   y_o = A_oo x_o + H_oe x_e.
+ * Builds and keeps A_oo itself on first use (the Schur path stores only A_oo^-1).
+ * No output may alias an input.
+ */
+int ddamg_apply_full(ddamg_ctx* ctx, const void* x_e, const void* x_o, void* y_e, void* y_o);
+
+/*
+ * Outer solver: flexible GMRES(n = cycles, m = k) on the full system
+ * D x = b (PAPER.md:77 names FGMRES as DD-alphaAMG's outer solver), preconditioned by ONE
+ * odd-even smoother call per Krylov vector and nothing else (no coarse grid):
+ *   z = M v:  bhat_e = v_e - H_eo A_oo^-1 v_o;  z_e = smoother on D_S z_e = bhat_e from z_e = 0;
+ *             z_o = A_oo^-1 (v_o - H_oe z_e)                                   (eq. 2)
+ *   smoother = DDAMG_SMOOTHER_RICHARDSON: s_n sweeps with weight omega (s_m ignored)
+ *              DDAMG_SMOOTHER_GMRES / _GCR: (n = s_n cycles, m = s_m) without tolerance
+ * The paper prints no FGMRES algorithm; reading R19: Alg. 2 with z_j = M v_j,
+ * w = D z_j, x += Z_m y.  History layout, tol, zero_init as ddamg_gmres_oe (norms over both
+ * parities).  x_e / x_o: initial guess in, solution out.  Keeps 2k+1 full-lattice vectors.
+ */
+int ddamg_fgmres(ddamg_ctx* ctx, const void* b_e, const void* b_o, void* x_e, void* x_o, int k, int cycles,
+                 double tol, int smoother, int s_n, int s_m, double omega, int zero_init, double* res_hist,
+                 int* n_hist);
 
 /* eq. 2, left factor:  x_o = A_oo^-1 (b_o - H_oe x_e). */
 int ddamg_reconstruct_odd(ddamg_ctx* ctx, const void* b_o, const void* x_e, void* x_o);

@@ -18,6 +18,7 @@ LIB_PATH = os.path.join(HERE, "libddamg.so")
 OK, EINVAL, ENOMEM, ESTATE, ECUDA, ESINGULAR = 0, -1, -2, -3, -4, -5
 F32, F64 = 0, 1
 BC_PERIODIC, BC_ANTIPERIODIC_T = 0, 1
+SMOOTHER_RICHARDSON, SMOOTHER_GMRES, SMOOTHER_GCR = 0, 1, 2
 
 _STATUS = {0: "DDAMG_OK", -1: "DDAMG_EINVAL", -2: "DDAMG_ENOMEM", -3: "DDAMG_ESTATE",
            -4: "DDAMG_ECUDA", -5: "DDAMG_ESINGULAR"}
@@ -37,6 +38,8 @@ SYMBOLS = {
     "ddamg_richardson": (_i, [_vp, _vp, _vp, _i, _d, _i, _dp]),
     "ddamg_gmres_oe": (_i, [_vp, _vp, _vp, _i, _i, _d, _i, _dp, _ip]),
     "ddamg_gcr_oe": (_i, [_vp, _vp, _vp, _i, _i, _d, _i, _dp, _ip]),
+    "ddamg_apply_full": (_i, [_vp, _vp, _vp, _vp, _vp]),
+    "ddamg_fgmres": (_i, [_vp, _vp, _vp, _vp, _vp, _i, _i, _d, _i, _i, _i, _d, _i, _dp, _ip]),
     "ddamg_reconstruct_odd": (_i, [_vp, _vp, _vp, _vp]),
     "ddamg_prepare_rhs": (_i, [_vp, _vp, _vp, _vp]),
     "ddamg_power_iteration": (_i, [_vp, _vp, _i, _dp]),
@@ -204,6 +207,23 @@ class Ddamg:
         nh = ctypes.c_int(0)
         self._ck(self.lib.ddamg_gcr_oe(self._h, _ptr(b_e), _ptr(x_e), k, cycles, tol, int(zero_init), hist,
                                        ctypes.byref(nh)), "ddamg_gcr_oe")
+        return list(hist)[:nh.value]
+
+    def apply_full(self, x_e: torch.Tensor, x_o: torch.Tensor):
+        """(y_e, y_o) = D (x_e, x_o), the full Wilson-clover operator."""
+        y_e, y_o = self.half_spinor(), self.half_spinor()
+        self._chk_half(x_e, x_o)
+        self._ck(self.lib.ddamg_apply_full(self._h, _ptr(x_e), _ptr(x_o), _ptr(y_e), _ptr(y_o)), "ddamg_apply_full")
+        return y_e, y_o
+
+    def fgmres(self, b_e, b_o, x_e, x_o, k: int, cycles: int, tol: float = 0.0, smoother: int = SMOOTHER_RICHARDSON,
+               s_n: int = 4, s_m: int = 1, omega: float = 1.0, zero_init: bool = True):
+        self._chk_half(b_e, b_o, x_e, x_o)
+        n = cycles * (k + 1) + 1
+        hist = (ctypes.c_double * n)()
+        nh = ctypes.c_int(0)
+        self._ck(self.lib.ddamg_fgmres(self._h, _ptr(b_e), _ptr(b_o), _ptr(x_e), _ptr(x_o), k, cycles, tol, smoother,
+                                       s_n, s_m, omega, int(zero_init), hist, ctypes.byref(nh)), "ddamg_fgmres")
         return list(hist)[:nh.value]
 
     def reconstruct_odd(self, b_o: torch.Tensor, x_e: torch.Tensor, x_o: Optional[torch.Tensor] = None):

@@ -28,6 +28,10 @@ struct ddamg_ctx {
     void* tmp_e;                // scratch half spinor (power iteration, final residual)
     void* krylov;               // (kcap + 1) half spinors
     int kcap;
+    void* clov_oo;              // A itself on odd sites (built lazily: only the full operator D needs it)
+    Scalars* sc2;               // device scalars of the outer FGMRES (the inner smoother uses sc)
+    void* fgm_basis;            // outer FGMRES: (fgm_cap + 1) V + fgm_cap Z full-lattice vectors
+    int fgm_cap;
     void* tmp_batch;            // multi-rhs t_o (batch_cap half spinors)
     double* partials_batch;     // multi-rhs reduction scratch
     int batch_cap;
@@ -37,7 +41,7 @@ struct ddamg_ctx {
     Scalars* sc;                // device scalars
     double* host_hist;          // pinned
     int* singular;              // device flag
-    bool have_gauge, have_clover;
+    bool have_gauge, have_clover, have_clov_oo;
     int sticky;                 // DDAMG_OK or DDAMG_ECUDA
     long long launches;
     std::string err;
@@ -123,16 +127,17 @@ extern "C" int ddamg_create(ddamg_ctx** out, int L, int T, double csw, double m0
     ctx->half_bytes = ctx->nreal * ctx->real_bytes;
     ctx->gauge = ctx->clov[0] = ctx->clov[1] = ctx->tmp_o = ctx->tmp_e = ctx->krylov = nullptr;
     ctx->kcap = 0;
+    ctx->clov_oo = nullptr; ctx->sc2 = nullptr; ctx->fgm_basis = nullptr; ctx->fgm_cap = 0;
     ctx->tmp_batch = nullptr; ctx->partials_batch = nullptr; ctx->batch_cap = 0; ctx->batch_l2_bytes = 40e6;
     ctx->partials = nullptr; ctx->sc = nullptr; ctx->host_hist = nullptr; ctx->singular = nullptr;
-    ctx->have_gauge = ctx->have_clover = false;
+    ctx->have_gauge = ctx->have_clover = ctx->have_clov_oo = false;
     ctx->sticky = DDAMG_OK; ctx->launches = 0; ctx->timing = false;
 
     const size_t gauge_bytes = (size_t)2 * 4 * 18 * ctx->g.Vh * ctx->real_bytes;
     const size_t clov_bytes = (size_t)72 * ctx->g.Vh * ctx->real_bytes;
     const int dgrid = dslash_grid(ctx->g);
     const int bgrid = blas_grid(ctx->nreal / 2);
-    ctx->partials_len = (size_t)(dgrid > bgrid * 2 * MDOT_NB ? dgrid : bgrid * 2 * MDOT_NB);
+    ctx->partials_len = (size_t)(2 * dgrid > bgrid * 2 * MDOT_NB ? 2 * dgrid : bgrid * 2 * MDOT_NB);
     cudaError_t e = cudaSuccess;
     if (e == cudaSuccess) e = cudaMalloc(&ctx->gauge, gauge_bytes);
     if (e == cudaSuccess) e = cudaMalloc(&ctx->clov[0], clov_bytes);
@@ -163,6 +168,7 @@ extern "C" int ddamg_destroy(ddamg_ctx* ctx)
     cudaFree(ctx->gauge); cudaFree(ctx->clov[0]); cudaFree(ctx->clov[1]);
     cudaFree(ctx->tmp_o); cudaFree(ctx->tmp_e); cudaFree(ctx->krylov);
     cudaFree(ctx->tmp_batch); cudaFree(ctx->partials_batch);
+    cudaFree(ctx->clov_oo); cudaFree(ctx->sc2); cudaFree(ctx->fgm_basis);
     cudaFree(ctx->partials); cudaFree(ctx->sc); cudaFree(ctx->singular);
     if (ctx->host_hist) cudaFreeHost(ctx->host_hist);
     cudaGetLastError();
@@ -202,6 +208,7 @@ extern "C" int ddamg_load_gauge(ddamg_ctx* ctx, const void* U, int u_prec, int o
     if (s != DDAMG_OK) return s;
     ctx->have_gauge = true;
     ctx->have_clover = false;
+    ctx->have_clov_oo = false;
     return DDAMG_OK;
 }
 
@@ -211,9 +218,9 @@ extern "C" int ddamg_build_clover(ddamg_ctx* ctx)
     if (!ctx->have_gauge) return fail(ctx, DDAMG_ESTATE, "ddamg_build_clover: no gauge field loaded");
     CK(cudaMemsetAsync(ctx->singular, 0, sizeof(int), ctx->stream));
     if (ctx->prec == DDAMG_F32)
-        launch_build_clover<float>(ctx->g, ctx->csw, ctx->m0, ctx->gauge, ctx->clov[0], ctx->clov[1], ctx->singular, ctx->stream);
+        launch_build_clover<float>(ctx->g, ctx->csw, ctx->m0, ctx->gauge, ctx->clov[0], ctx->clov[1], nullptr, ctx->singular, ctx->stream);
     else
-        launch_build_clover<double>(ctx->g, ctx->csw, ctx->m0, ctx->gauge, ctx->clov[0], ctx->clov[1], ctx->singular, ctx->stream);
+        launch_build_clover<double>(ctx->g, ctx->csw, ctx->m0, ctx->gauge, ctx->clov[0], ctx->clov[1], nullptr, ctx->singular, ctx->stream);
     int s = after_launch(ctx);
     if (s != DDAMG_OK) return s;
     int flag = 0;
@@ -255,9 +262,11 @@ extern "C" int ddamg_get_clover(ddamg_ctx* ctx, void* A_nat, void* Ainv_nat)
 // --------------------------------------------------------------------------- hot path
 // One fused hopping launch.  parity = parity of the output sites.
 static int dslash(ddamg_ctx* ctx, int epi, bool norm, int parity, const void* in, const void* own, const void* rhs,
-                  void* out, double omega, int which, int nrhs = 1)
+                  void* out, double omega, int which, int nrhs = 1, size_t partials_offset = 0,
+                  const void* clov_override = nullptr)
 {
-    double* partials = nrhs > 1 ? ctx->partials_batch : ctx->partials;
+    double* partials = (nrhs > 1 ? ctx->partials_batch : ctx->partials) + partials_offset;
+    const void* clov = clov_override ? clov_override : ctx->clov[parity];
     ddamg_ctx::Ev ev;
     if (ctx->timing) {
         if (cudaEventCreate(&ev.a) != cudaSuccess || cudaEventCreate(&ev.b) != cudaSuccess)
@@ -267,10 +276,10 @@ static int dslash(ddamg_ctx* ctx, int epi, bool norm, int parity, const void* in
     }
     if (ctx->prec == DDAMG_F32)
         launch_dslash<float>(ctx->g, epi, norm, parity, in, gauge_block(ctx, parity), gauge_block(ctx, 1 - parity),
-                             ctx->clov[parity], own, rhs, out, omega, partials, nrhs, ctx->batch_l2_bytes, ctx->stream);
+                             clov, own, rhs, out, omega, partials, nrhs, ctx->batch_l2_bytes, ctx->stream);
     else
         launch_dslash<double>(ctx->g, epi, norm, parity, in, gauge_block(ctx, parity), gauge_block(ctx, 1 - parity),
-                              ctx->clov[parity], own, rhs, out, omega, partials, nrhs, ctx->batch_l2_bytes, ctx->stream);
+                              clov, own, rhs, out, omega, partials, nrhs, ctx->batch_l2_bytes, ctx->stream);
     if (ctx->timing) {
         cudaEventRecord(ev.b, ctx->stream);
         ctx->events.push_back(ev);
@@ -748,6 +757,216 @@ extern "C" int ddamg_gcr_oe(ddamg_ctx* ctx, const void* b_e, void* x_e, int k, i
     if (s != DDAMG_OK) return s;
     if (ctx->prec == DDAMG_F32) return gcr_impl<float>(ctx, b_e, x_e, k, cycles, tol, zero_init, res_hist, n_hist);
     return gcr_impl<double>(ctx, b_e, x_e, k, cycles, tol, zero_init, res_hist, n_hist);
+}
+
+// --------------------------------------------------------------------------- full operator, outer FGMRES (NEXT-4)
+// D = A + H on both parities needs A_oo itself (the Schur path stores only its inverse).
+static int ensure_full(ddamg_ctx* ctx, const char* who)
+{
+    int s = need_ready(ctx, who);
+    if (s != DDAMG_OK) return s;
+    if (ctx->have_clov_oo) return DDAMG_OK;
+    if (!ctx->clov_oo) {
+        cudaError_t e = cudaMalloc(&ctx->clov_oo, (size_t)72 * ctx->g.Vh * ctx->real_bytes);
+        if (e != cudaSuccess) { cudaGetLastError(); ctx->clov_oo = nullptr; return fail(ctx, DDAMG_ENOMEM, std::string(who) + ": cannot allocate A_oo"); }
+    }
+    if (ctx->prec == DDAMG_F32)
+        launch_build_clover<float>(ctx->g, ctx->csw, ctx->m0, ctx->gauge, nullptr, nullptr, ctx->clov_oo, ctx->singular, ctx->stream);
+    else
+        launch_build_clover<double>(ctx->g, ctx->csw, ctx->m0, ctx->gauge, nullptr, nullptr, ctx->clov_oo, ctx->singular, ctx->stream);
+    s = after_launch(ctx);
+    if (s != DDAMG_OK) return s;
+    ctx->have_clov_oo = true;
+    return DDAMG_OK;
+}
+
+// (y_e, y_o) = D (x_e, x_o)
+static int apply_full(ddamg_ctx* ctx, const void* x_e, const void* x_o, void* y_e, void* y_o)
+{
+    int s = dslash(ctx, EPI_FULL, false, 0, x_o, x_e, nullptr, y_e, 0.0, 5);
+    if (s != DDAMG_OK) return s;
+    return dslash(ctx, EPI_FULL, false, 1, x_e, x_o, nullptr, y_o, 0.0, 5, 1, 0, ctx->clov_oo);
+}
+
+extern "C" int ddamg_apply_full(ddamg_ctx* ctx, const void* x_e, const void* x_o, void* y_e, void* y_o)
+{
+    ENTER(ctx);
+    if (!x_e || !x_o || !y_e || !y_o || x_e == y_e || x_o == y_o || x_e == y_o || x_o == y_e)
+        return fail(ctx, DDAMG_EINVAL, "ddamg_apply_full: NULL or aliased arguments");
+    int s = ensure_full(ctx, "ddamg_apply_full");
+    if (s != DDAMG_OK) return s;
+    return apply_full(ctx, x_e, x_o, y_e, y_o);
+}
+
+// z = M v: one odd-even smoother call (eq. 2) from a zero initial guess
+static int smoother_call(ddamg_ctx* ctx, int smoother, int s_n, int s_m, double omega, const void* v_e, const void* v_o,
+                         void* z_e, void* z_o)
+{
+    int s = ddamg_prepare_rhs(ctx, v_e, v_o, ctx->tmp_e);
+    if (s != DDAMG_OK) return s;
+    switch (smoother) {
+    case DDAMG_SMOOTHER_RICHARDSON: s = ddamg_richardson(ctx, ctx->tmp_e, z_e, s_n, omega, 1, nullptr); break;
+    case DDAMG_SMOOTHER_GMRES: s = ddamg_gmres_oe(ctx, ctx->tmp_e, z_e, s_m, s_n, 0.0, 1, nullptr, nullptr); break;
+    case DDAMG_SMOOTHER_GCR: s = ddamg_gcr_oe(ctx, ctx->tmp_e, z_e, s_m, s_n, 0.0, 1, nullptr, nullptr); break;
+    default: return fail(ctx, DDAMG_EINVAL, "ddamg_fgmres: unknown smoother");
+    }
+    if (s != DDAMG_OK) return s;
+    return ddamg_reconstruct_odd(ctx, v_o, z_e, z_o);
+}
+
+static int copy_hist_from(ddamg_ctx* ctx, Scalars* sc, double* dst, int n, int* n_out)
+{
+    CK(cudaMemcpyAsync(ctx->host_hist, (char*)sc + offsetof(Scalars, hist), sizeof(double) * n, cudaMemcpyDeviceToHost, ctx->stream));
+    int nh = 0;
+    CK(cudaMemcpyAsync(&nh, (char*)sc + offsetof(Scalars, nhist), sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    if (nh > n) nh = n;
+    if (dst) memcpy(dst, ctx->host_hist, sizeof(double) * nh);
+    if (n_out) *n_out = nh;
+    return DDAMG_OK;
+}
+
+template <typename T>
+static int fgmres_impl(ddamg_ctx* ctx, const void* b_e, const void* b_o, void* x_e, void* x_o, int k, int cycles, double tol,
+                       int smoother, int s_n, int s_m, double omega, int zero_init, double* res_hist, int* n_hist)
+{
+    cudaStream_t st = ctx->stream;
+    Scalars* sc = ctx->sc2;
+    const size_t nhalf = ctx->nreal, nfull = 2 * ctx->nreal;
+    const size_t full_bytes = 2 * ctx->half_bytes;
+    const int vecN = (int)(16 / ctx->real_bytes);
+    const int bgrid = blas_grid(nfull / vecN);
+    const int dgrid = dslash_grid(ctx->g);
+    char* base = (char*)ctx->fgm_basis;
+    auto Ve = [&](int j) { return (void*)(base + (size_t)j * full_bytes); };                       // v_j, even half
+    auto Vo = [&](int j) { return (void*)(base + (size_t)j * full_bytes + ctx->half_bytes); };
+    auto Ze = [&](int j) { return (void*)(base + (size_t)(k + 1 + j) * full_bytes); };             // z_j = M v_j
+    auto Zo = [&](int j) { return (void*)(base + (size_t)(k + 1 + j) * full_bytes + ctx->half_bytes); };
+    double* coef_y = (double*)((char*)sc + offsetof(Scalars, y));
+    double* coef_negh = (double*)((char*)sc + offsetof(Scalars, negh));
+    double* scale = (double*)((char*)sc + offsetof(Scalars, scale));
+    double* value = (double*)((char*)sc + offsetof(Scalars, value));
+    CK(cudaMemsetAsync((char*)sc + offsetof(Scalars, nhist), 0, sizeof(int), st));
+    int s;
+    // r = b - D x into v_0, ||r|| appended to the history
+    auto residual = [&]() -> int {
+        int q = dslash(ctx, EPI_FULL_RESIDUAL, true, 0, x_o, x_e, b_e, Ve(0), 0.0, 5);
+        if (q != DDAMG_OK) return q;
+        q = dslash(ctx, EPI_FULL_RESIDUAL, true, 1, x_e, x_o, b_o, Vo(0), 0.0, 5, 1, (size_t)dgrid, ctx->clov_oo);
+        if (q != DDAMG_OK) return q;
+        launch_finalize_norm(ctx->partials, 2 * dgrid, sc, 1, st);
+        return after_launch(ctx);
+    };
+    double bnorm = 0.0;
+    {   // ||b|| (the tolerance is relative to it)
+        launch_copy_norm<T>(nhalf, b_e, Ve(0), ctx->partials, st);
+        launch_copy_norm<T>(nhalf, b_o, Vo(0), ctx->partials + blas_grid(nhalf / vecN), st);
+        launch_finalize_norm(ctx->partials, 2 * blas_grid(nhalf / vecN), sc, 0, st);
+        s = after_launch(ctx, 3); if (s != DDAMG_OK) return s;
+        if (tol > 0.0) {
+            CK(cudaMemcpyAsync(&bnorm, value, sizeof(double), cudaMemcpyDeviceToHost, st));
+            CK(cudaStreamSynchronize(st));
+        }
+    }
+    if (zero_init) {
+        CK(cudaMemsetAsync(x_e, 0, ctx->half_bytes, st));
+        CK(cudaMemsetAsync(x_o, 0, ctx->half_bytes, st));
+    }
+    bool converged = false;
+    for (int c = 0; c < cycles && !converged; ++c) {
+        if (zero_init && c == 0) {
+            // r = b: v_0 already holds b and sc->value its norm
+            launch_finalize_norm(ctx->partials, 2 * blas_grid(nhalf / vecN), sc, 1, st);
+            s = after_launch(ctx); if (s != DDAMG_OK) return s;
+        } else {
+            s = residual(); if (s != DDAMG_OK) return s;
+        }
+        launch_gmres_begin_cycle(sc, st);
+        launch_scale_by_dev<T>(nfull, Ve(0), scale, st);
+        s = after_launch(ctx, 2); if (s != DDAMG_OK) return s;
+        if (tol > 0.0) {
+            double beta = 0.0;
+            CK(cudaMemcpyAsync(&beta, value, sizeof(double), cudaMemcpyDeviceToHost, st));
+            CK(cudaStreamSynchronize(st));
+            if (beta <= tol * bnorm) { converged = true; break; }
+        }
+        int m = 0;
+        for (int j = 0; j < k; ++j) {
+            s = smoother_call(ctx, smoother, s_n, s_m, omega, Ve(j), Vo(j), Ze(j), Zo(j));      // z_j = M v_j
+            if (s != DDAMG_OK) return s;
+            s = apply_full(ctx, Ze(j), Zo(j), Ve(j + 1), Vo(j + 1));                             // w = D z_j
+            if (s != DDAMG_OK) return s;
+            for (int i0 = 0; i0 <= j; i0 += MDOT_NB) {
+                const int nb = (j + 1 - i0) < MDOT_NB ? (j + 1 - i0) : MDOT_NB;
+                launch_multi_dot<T>(nfull, nb, Ve(i0), nfull, Ve(j + 1), ctx->partials, st);
+                launch_finalize_dots(ctx->partials, bgrid, nb, sc, i0, st);
+                s = after_launch(ctx, 2); if (s != DDAMG_OK) return s;
+            }
+            for (int i0 = 0; i0 <= j; i0 += MDOT_NB) {
+                const int nb = (j + 1 - i0) < MDOT_NB ? (j + 1 - i0) : MDOT_NB;
+                const bool last = i0 + MDOT_NB > j;
+                launch_multi_axpy<T>(nfull, nb, Ve(i0), nfull, coef_negh + 2 * i0, Ve(j + 1), last ? ctx->partials : nullptr, st);
+                s = after_launch(ctx); if (s != DDAMG_OK) return s;
+            }
+            launch_finalize_norm(ctx->partials, bgrid, sc, 0, st);
+            launch_gmres_givens(sc, j, st);
+            launch_scale_by_dev<T>(nfull, Ve(j + 1), scale, st);
+            s = after_launch(ctx, 3); if (s != DDAMG_OK) return s;
+            m = j + 1;
+            if (tol > 0.0) {
+                int nh = 0;
+                CK(cudaMemcpyAsync(&nh, (char*)sc + offsetof(Scalars, nhist), sizeof(int), cudaMemcpyDeviceToHost, st));
+                CK(cudaStreamSynchronize(st));
+                double est = 0.0;
+                CK(cudaMemcpyAsync(&est, (char*)sc + offsetof(Scalars, hist) + sizeof(double) * (nh - 1), sizeof(double), cudaMemcpyDeviceToHost, st));
+                CK(cudaStreamSynchronize(st));
+                if (est <= tol * bnorm) break;
+            }
+        }
+        launch_gmres_solve(sc, m, st);
+        s = after_launch(ctx); if (s != DDAMG_OK) return s;
+        for (int i0 = 0; i0 < m; i0 += MDOT_NB) {                                                  // x += Z_m y
+            const int nb = (m - i0) < MDOT_NB ? (m - i0) : MDOT_NB;
+            launch_multi_axpy<T>(nhalf, nb, Ze(i0), nfull, coef_y + 2 * i0, x_e, nullptr, st);
+            launch_multi_axpy<T>(nhalf, nb, Zo(i0), nfull, coef_y + 2 * i0, x_o, nullptr, st);
+            s = after_launch(ctx, 2); if (s != DDAMG_OK) return s;
+        }
+    }
+    if (!converged) { s = residual(); if (s != DDAMG_OK) return s; }
+    return copy_hist_from(ctx, sc, res_hist, cycles * (k + 1) + 1, n_hist);
+}
+
+extern "C" int ddamg_fgmres(ddamg_ctx* ctx, const void* b_e, const void* b_o, void* x_e, void* x_o, int k, int cycles,
+                            double tol, int smoother, int s_n, int s_m, double omega, int zero_init, double* res_hist,
+                            int* n_hist)
+{
+    ENTER(ctx);
+    if (!b_e || !b_o || !x_e || !x_o || b_e == x_e || b_o == x_o || k < 1 || cycles < 1 || tol < 0.0 || s_n < 1)
+        return fail(ctx, DDAMG_EINVAL, "ddamg_fgmres: bad arguments");
+    if (smoother != DDAMG_SMOOTHER_RICHARDSON && (s_m < 1 || s_m > GMRES_KMAX))
+        return fail(ctx, DDAMG_EINVAL, "ddamg_fgmres: bad inner cycle length");
+    if (smoother < DDAMG_SMOOTHER_RICHARDSON || smoother > DDAMG_SMOOTHER_GCR)
+        return fail(ctx, DDAMG_EINVAL, "ddamg_fgmres: unknown smoother");
+    if (k > GMRES_KMAX) return fail(ctx, DDAMG_EINVAL, "ddamg_fgmres: k exceeds 64");
+    if ((long long)cycles * (k + 1) + 1 > HIST_MAX) return fail(ctx, DDAMG_EINVAL, "ddamg_fgmres: history too long");
+    int s = ensure_full(ctx, "ddamg_fgmres");
+    if (s != DDAMG_OK) return s;
+    if (!ctx->sc2) {
+        cudaError_t e = cudaMalloc((void**)&ctx->sc2, sizeof(Scalars));
+        if (e != cudaSuccess) { cudaGetLastError(); ctx->sc2 = nullptr; return fail(ctx, DDAMG_ENOMEM, "ddamg_fgmres: scalars"); }
+        CK(cudaMemsetAsync(ctx->sc2, 0, sizeof(Scalars), ctx->stream));
+    }
+    if (k > ctx->fgm_cap) {
+        CK(cudaStreamSynchronize(ctx->stream));
+        cudaFree(ctx->fgm_basis);
+        ctx->fgm_basis = nullptr; ctx->fgm_cap = 0;
+        cudaError_t e = cudaMalloc(&ctx->fgm_basis, (size_t)(2 * k + 1) * 2 * ctx->half_bytes);
+        if (e != cudaSuccess) { cudaGetLastError(); return fail(ctx, DDAMG_ENOMEM, "ddamg_fgmres: cannot allocate the V and Z bases"); }
+        ctx->fgm_cap = k;
+    }
+    if (ctx->prec == DDAMG_F32)
+        return fgmres_impl<float>(ctx, b_e, b_o, x_e, x_o, k, cycles, tol, smoother, s_n, s_m, omega, zero_init, res_hist, n_hist);
+    return fgmres_impl<double>(ctx, b_e, b_o, x_e, x_o, k, cycles, tol, smoother, s_n, s_m, omega, zero_init, res_hist, n_hist);
 }
 
 // --------------------------------------------------------------------------- power iteration

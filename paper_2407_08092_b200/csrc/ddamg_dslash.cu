@@ -6,6 +6,8 @@
 //              out = b_e - (A_ee x_e - H_eo t_o)  (+ ||out||^2)  EPI_RESIDUAL      (GMRES line 2)
 //              x_o = A_oo^-1 (b_o - H_oe x_e)                    EPI_CLOV_RHS_MINUS_HOP (eq. 2 left)
 //              bhat_e = b_e - H_eo t_o                           EPI_RHS_MINUS_HOP (eq. 2 right)
+//              y_p = A_pp x_p + H_pq x_q  (one parity of D x)    EPI_FULL          (outer FGMRES)
+//              out = b_p - (A_pp x_p + H_pq x_q)  (+ ||out||^2)  EPI_FULL_RESIDUAL
 //
 // One thread per output site; consecutive threads = consecutive checkerboard indices, so
 // every plane access of a warp is one contiguous 512-byte (16-byte vectors) run.
@@ -110,15 +112,18 @@ dslash_kernel(const DslashArgs<T> a)
             T x[24], ax[24];
             load_spinor<T, true>(a.own, Vs, sv, x);
             clover_site_mul<T>(a.clov, a.g.Vh, cb, x, ax);
-            if (EPI == EPI_SCHUR) {
+            // H = -1/2 acc:  Schur forms subtract H t (+1/2 acc), the full operator adds H x (-1/2 acc)
+            constexpr bool FULL = (EPI == EPI_FULL || EPI == EPI_FULL_RESIDUAL);
+            const T hs = FULL ? (T)(-0.5) : (T)0.5;
+            if (EPI == EPI_SCHUR || EPI == EPI_FULL) {
 #pragma unroll
-                for (int i = 0; i < 24; ++i) res[i] = ax[i] + (T)0.5 * acc[i];     // A x - H t
+                for (int i = 0; i < 24; ++i) res[i] = ax[i] + hs * acc[i];     // A x - H t   or   A x + H x'
             } else {
                 T b[24];
                 load_spinor<T, true>(a.rhs, Vs, sv, b);
 #pragma unroll
                 for (int i = 0; i < 24; ++i) {
-                    const T r = b[i] - (ax[i] + (T)0.5 * acc[i]);
+                    const T r = b[i] - (ax[i] + hs * acc[i]);
                     if (NORM) nrm += (double)r * (double)r;
                     res[i] = (EPI == EPI_RICHARDSON) ? x[i] + a.omega * r : r;
                 }
@@ -200,6 +205,11 @@ void launch_dslash(const Geom& g, int epi, bool norm, int parity, const void* in
     case EPI_RESIDUAL:
         if (norm) launch<T, EPI_RESIDUAL, true>(a, st);
         else launch<T, EPI_RESIDUAL, false>(a, st);
+        break;
+    case EPI_FULL: launch<T, EPI_FULL, false>(a, st); break;
+    case EPI_FULL_RESIDUAL:
+        if (norm) launch<T, EPI_FULL_RESIDUAL, true>(a, st);
+        else launch<T, EPI_FULL_RESIDUAL, false>(a, st);
         break;
     }
 }

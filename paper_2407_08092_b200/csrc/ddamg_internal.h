@@ -23,7 +23,9 @@ enum {
     EPI_RHS_MINUS_HOP = 2,       // out = rhs - H in                        prepare_rhs
     EPI_SCHUR = 3,               // out = Cl own - H in                     kernel B
     EPI_RICHARDSON = 4,          // r = rhs - (Cl own - H in); out = own + w r   kernel B'
-    EPI_RESIDUAL = 5             // out = rhs - (Cl own - H in)
+    EPI_RESIDUAL = 5,            // out = rhs - (Cl own - H in)
+    EPI_FULL = 6,                // out = Cl own + H in                     one parity of D = A + H
+    EPI_FULL_RESIDUAL = 7        // out = rhs - (Cl own + H in)             one parity of b - D x
 };
 
 template <typename T>
@@ -45,7 +47,7 @@ template <typename T>
 void launch_batch_interleave(const Geom& g, int nrhs, bool to_batch, void* halves, void* X, cudaStream_t st);
 template <typename T>
 void launch_build_clover(const Geom& g, double csw, double m0, const void* gauge, void* clov_e, void* clov_o,
-                         int* singular_flag, cudaStream_t st);
+                         void* clov_o_plain, int* singular_flag, cudaStream_t st);
 template <typename T>
 void launch_get_clover(const Geom& g, const void* clov_e, const void* clov_o, void* A_nat, void* Ainv_nat,
                        cudaStream_t st);

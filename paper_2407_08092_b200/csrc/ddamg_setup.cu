@@ -267,11 +267,15 @@ __device__ bool invert6(double (&mr)[6][6], double (&mi)[6][6])
 
 template <typename T>
 __global__ void build_clover_kernel(Geom g, double csw, double m0, const T* __restrict__ gauge,
-                                    T* __restrict__ clov_e, T* __restrict__ clov_o, int* singular)
+                                    T* __restrict__ clov_e, T* __restrict__ clov_o, T* __restrict__ clov_o_plain,
+                                    int* singular)
 {
+    // clov_e: A on even sites; clov_o: A^-1 on odd sites; clov_o_plain: A itself on odd sites
+    // (needed only by the full operator D = A + H).  A NULL output skips that part.
     const int idx = blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= 2 * g.Vh) return;
     const int parity = idx / g.Vh, cb = idx % g.Vh;
+    if (parity == 0 && !clov_e) return;
     const Coord x = coord_of(g, cb, parity);
     // dense blocks, index 3*s + c
     double ur[6][6], ui[6][6], lr[6][6], li[6][6];
@@ -310,14 +314,22 @@ __global__ void build_clover_kernel(Geom g, double csw, double m0, const T* __re
                 }
             }
     }
-    if (parity == 1) {
-        const bool ok1 = invert6(ur, ui);
-        const bool ok2 = invert6(lr, li);
-        if (!(ok1 && ok2)) atomicOr(singular, 1);
-    }
-    T* dst = parity ? clov_o : clov_e;
     T c[36];
-    for (int blk = 0; blk < 2; ++blk) {
+    for (int pass = 0; pass < 2; ++pass) {
+      // pass 0: the block itself (even sites -> clov_e, odd sites -> clov_o_plain);
+      // pass 1: odd sites only, the inverse -> clov_o
+      T* dst;
+      if (pass == 0) {
+          dst = parity ? clov_o_plain : clov_e;
+      } else {
+          if (parity == 0 || !clov_o) break;
+          const bool ok1 = invert6(ur, ui);
+          const bool ok2 = invert6(lr, li);
+          if (!(ok1 && ok2)) atomicOr(singular, 1);
+          dst = clov_o;
+      }
+      if (!dst) continue;
+      for (int blk = 0; blk < 2; ++blk) {
         double (&mr)[6][6] = blk ? lr : ur;
         double (&mi)[6][6] = blk ? li : ui;
         for (int i = 0; i < 6; ++i) c[i] = (T)mr[i][i];
@@ -329,19 +341,20 @@ __global__ void build_clover_kernel(Geom g, double csw, double m0, const T* __re
                 c[k + 1] = (T)(0.5 * (mi[i][j] - mi[j][i]));
             }
         store_clover_block<T>(dst, g.Vh, cb, blk, c);
+      }
     }
 }
 
 template <typename T>
 void launch_build_clover(const Geom& g, double csw, double m0, const void* gauge, void* clov_e, void* clov_o,
-                         int* singular_flag, cudaStream_t st)
+                         void* clov_o_plain, int* singular_flag, cudaStream_t st)
 {
     const int n = 2 * g.Vh;
     build_clover_kernel<T><<<(n + 63) / 64, 64, 0, st>>>(g, csw, m0, (const T*)gauge, (T*)clov_e, (T*)clov_o,
-                                                          singular_flag);
+                                                          (T*)clov_o_plain, singular_flag);
 }
-template void launch_build_clover<float>(const Geom&, double, double, const void*, void*, void*, int*, cudaStream_t);
-template void launch_build_clover<double>(const Geom&, double, double, const void*, void*, void*, int*, cudaStream_t);
+template void launch_build_clover<float>(const Geom&, double, double, const void*, void*, void*, void*, int*, cudaStream_t);
+template void launch_build_clover<double>(const Geom&, double, double, const void*, void*, void*, void*, int*, cudaStream_t);
 
 // ------------------------------------------------------------------ debug: dense clover out
 template <typename T>
