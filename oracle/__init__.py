@@ -6,8 +6,8 @@ Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline``
 
 The operator arithmetic lives in ``oracle/wilson_clover.c`` (plain C, natural
 layout, full 4x4 spin matrices); this file is the ctypes marshalling around
-it.  The two iterations (Richardson, Alg. 4; GMRES, Alg. 2) are written out
-step by step in ``oracle/iterations.py``.
+it.  The iterations (Richardson, Alg. 4; GMRES, Alg. 2; GCR, Alg. 3; FGMRES) are
+written out step by step in ``oracle/iterations.py``, SAP (Alg. 1) in ``oracle/sap.py``.
 
 Parity status: every function is pinned by ``tests/test_oracle_*.py`` against
 closed forms / invariants / dense linear algebra; the only *unpinned* items
@@ -83,11 +83,14 @@ class WilsonClover:
         self.odd = (self.par == 1)[..., None, None]
 
     # -- pieces ------------------------------------------------------------
-    def hop(self, psi, sel: int = 2) -> np.ndarray:
-        """(H psi) on even (sel=0), odd (sel=1) or all (sel=2) sites; 0 elsewhere."""
+    def hop(self, psi, sel: int = 2, Ubc=None) -> np.ndarray:
+        """(H psi) on even (sel=0), odd (sel=1) or all (sel=2) sites; 0 elsewhere.
+        ``Ubc``: link field to use instead of this operator's own (SAP's block-diagonal
+        operator is the hopping term of a link field with the inter-block links zeroed)."""
         psi = _c(psi)
+        links = self.Ubc if Ubc is None else _c(Ubc)
         out = np.empty(self.shape, dtype=np.complex128)
-        lib().oracle_hop(self.L, self.T, _p(self.Ubc), _p(psi), _p(out), int(sel))
+        lib().oracle_hop(self.L, self.T, _p(links), _p(psi), _p(out), int(sel))
         return out
 
     def site_matvec(self, M, psi, sel: int = 2) -> np.ndarray:
@@ -135,3 +138,4 @@ class WilsonClover:
 
 
 from .iterations import richardson, richardson_multi, gmres, gcr, fgmres, power_iteration  # noqa: E402,F401
+from .sap import sap, BlockOperators, block_index, cut_links, minimal_residual  # noqa: E402,F401
