@@ -170,6 +170,30 @@ int ddamg_fgmres(ddamg_ctx* ctx, const void* b_e, const void* b_o, void* x_e, vo
                  double tol, int smoother, int s_n, int s_m, double omega, int zero_init, double* res_hist,
                  int* n_hist);
 
+/*
+ * Alg. 1: SAP(n, m) on the full system D x = b -- SURVEY.md NEXT-3.
+ * The lattice is cut into 4-D blocks of block[0..3] = (Bx, By, Bz, Bt) sites, coloured
+ * red/black by the parity of the sum of their block coordinates.  Each of the
+ * n outer iterations computes r = b - D x (line 2), approximately solves D_k e_k = r_k on every
+ * red block and adds e_k to x_k (lines 4-6), recomputes r (line 7) and does the same on the
+ * black blocks (lines 8-10).  D_k = P_k D P_k^T (hops leaving the block dropped).  The block
+ * solve is m Minimal Residual iterations with block-local odd-even preconditioning
+ * (PAPER.md:179): rhat_e = r_e - H^k_eo A_oo^-1 r_o; e = 0, rho = rhat_e, m times
+ * { q = D^k_S rho; alpha = <q,rho>/<q,q>; e += alpha rho; rho -= alpha q };
+ * e_o = A_oo^-1 (r_o - H^k_oe e)  (readings R20-R24).  All dot products are
+ * block-local; one CTA per block, the block's links staged in shared memory.
+ *   block      HOST array of 4 ints; each even, dividing L (L, L, T) with an EVEN quotient, at
+ *              most 512 sites per block, links of one block must fit in shared memory
+ *              (fp32: up to 512 sites, fp64: up to 256 sites) -- else EINVAL
+ *   x_e, x_o   in: x^(0) (ignored if zero_init != 0); out: x^(n).  In place.
+ *   res_hist   HOST array of n+1 doubles or NULL: ||b - D x^(i)||_2 for i = 0..n (the first n
+ *              are the residuals of line 2; the last costs one extra residual).  NULL skips
+ *              the reductions and the stream synchronisation.
+ * m = 0 leaves x unchanged.  Builds and keeps A_oo on first use (as ddamg_apply_full).
+ */
+int ddamg_sap(ddamg_ctx* ctx, const void* b_e, const void* b_o, void* x_e, void* x_o, int n, int m,
+              const int* block, int zero_init, double* res_hist);
+
 /* eq. 2, left factor:  x_o = A_oo^-1 (b_o - H_oe x_e). */
 int ddamg_reconstruct_odd(ddamg_ctx* ctx, const void* b_o, const void* x_e, void* x_o);
 
@@ -246,7 +270,8 @@ long long ddamg_launch_count(ddamg_ctx* ctx);
  * context's stream; ddamg_kernel_time_ms returns the accumulated device time (ms) and the
  * number of launches of kernel class `which` (0 = kernel A: A_oo^-1 H_oe, 1 = kernel B /
  * B': A_ee x - H_eo t with optional Richardson update, 2 = eq.-2 factors, 3 / 4 = the
- * multi-rhs forms of kernel A / kernel B, B') since the last reset, after
+ * multi-rhs forms of kernel A / kernel B, B', 5 = one parity of the full operator /
+ * residual, 6 = SAP block-solve kernel) since the last reset, after
  * synchronising the stream.  Used by bench.py for the per-kernel roofline.
  */
 int ddamg_kernel_timing(ddamg_ctx* ctx, int on);

@@ -40,6 +40,7 @@ SYMBOLS = {
     "ddamg_gcr_oe": (_i, [_vp, _vp, _vp, _i, _i, _d, _i, _dp, _ip]),
     "ddamg_apply_full": (_i, [_vp, _vp, _vp, _vp, _vp]),
     "ddamg_fgmres": (_i, [_vp, _vp, _vp, _vp, _vp, _i, _i, _d, _i, _i, _i, _d, _i, _dp, _ip]),
+    "ddamg_sap": (_i, [_vp, _vp, _vp, _vp, _vp, _i, _i, _ip, _i, _dp]),
     "ddamg_reconstruct_odd": (_i, [_vp, _vp, _vp, _vp]),
     "ddamg_prepare_rhs": (_i, [_vp, _vp, _vp, _vp]),
     "ddamg_power_iteration": (_i, [_vp, _vp, _i, _dp]),
@@ -225,6 +226,16 @@ class Ddamg:
         self._ck(self.lib.ddamg_fgmres(self._h, _ptr(b_e), _ptr(b_o), _ptr(x_e), _ptr(x_o), k, cycles, tol, smoother,
                                        s_n, s_m, omega, int(zero_init), hist, ctypes.byref(nh)), "ddamg_fgmres")
         return list(hist)[:nh.value]
+
+    def sap(self, b_e, b_o, x_e, x_o, n: int, m: int, block=(4, 4, 4, 4), zero_init: bool = False,
+            history: bool = False):
+        """Alg. 1: SAP(n, m) on D x = b, in place on (x_e, x_o); history = ||b - D x^(i)||, i = 0..n."""
+        self._chk_half(b_e, b_o, x_e, x_o)
+        blk = (ctypes.c_int * 4)(*[int(v) for v in block])
+        hist = (ctypes.c_double * (n + 1))() if history else None
+        self._ck(self.lib.ddamg_sap(self._h, _ptr(b_e), _ptr(b_o), _ptr(x_e), _ptr(x_o), n, m, blk, int(zero_init),
+                                    hist), "ddamg_sap")
+        return list(hist) if history else None
 
     def reconstruct_odd(self, b_o: torch.Tensor, x_e: torch.Tensor, x_o: Optional[torch.Tensor] = None):
         x_o = self.half_spinor() if x_o is None else x_o

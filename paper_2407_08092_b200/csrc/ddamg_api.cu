@@ -969,6 +969,93 @@ extern "C" int ddamg_fgmres(ddamg_ctx* ctx, const void* b_e, const void* b_o, vo
     return fgmres_impl<double>(ctx, b_e, b_o, x_e, x_o, k, cycles, tol, smoother, s_n, s_m, omega, zero_init, res_hist, n_hist);
 }
 
+// --------------------------------------------------------------------------- SAP (NEXT-3)
+// Alg. 1.  Per outer iteration and colour: the global residual r = b - D x
+// (lines 2 / 7) with the fused full-operator kernels, then one launch of the block-solve
+// kernel over all blocks of that colour (lines 4-6 / 8-10).
+static int sap_geometry(ddamg_ctx* ctx, const int* block, SapGeom* sg, const char* who)
+{
+    const int ext[4] = { ctx->g.L, ctx->g.L, ctx->g.L, ctx->g.T };
+    long long vb = 1;
+    for (int mu = 0; mu < 4; ++mu) {
+        const int B = block[mu];
+        if (B < 2 || (B & 1) || ext[mu] % B != 0 || ((ext[mu] / B) & 1))
+            return fail(ctx, DDAMG_EINVAL, std::string(who) + ": block extents must be even and divide the lattice extents with an even quotient");
+        sg->B[mu] = B;
+        sg->nb[mu] = ext[mu] / B;
+        vb *= B;
+    }
+    if (vb / 2 > SAP_MAX_THREADS) return fail(ctx, DDAMG_EINVAL, std::string(who) + ": blocks of more than 512 sites are not supported");
+    sg->Bxh = sg->B[0] / 2;
+    sg->Vbh = (int)(vb / 2);
+    sg->nbxh = sg->nb[0] / 2;
+    int dev = 0, optin = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) != cudaSuccess)
+        return check_cuda(ctx, cudaGetLastError(), "cudaDeviceGetAttribute");
+    if (sap_smem_bytes(*sg, ctx->real_bytes) > (size_t)optin)
+        return fail(ctx, DDAMG_EINVAL, std::string(who) + ": the block's links do not fit in shared memory at this precision");
+    return DDAMG_OK;
+}
+
+extern "C" int ddamg_sap(ddamg_ctx* ctx, const void* b_e, const void* b_o, void* x_e, void* x_o, int n, int m,
+                         const int* block, int zero_init, double* res_hist)
+{
+    ENTER(ctx);
+    if (!b_e || !b_o || !x_e || !x_o || !block || b_e == x_e || b_o == x_o || n < 0 || m < 0)
+        return fail(ctx, DDAMG_EINVAL, "ddamg_sap: bad arguments");
+    if (res_hist && n + 1 > HIST_MAX) return fail(ctx, DDAMG_EINVAL, "ddamg_sap: n exceeds the history capacity");
+    int s = ensure_full(ctx, "ddamg_sap");
+    if (s != DDAMG_OK) return s;
+    SapGeom sg;
+    s = sap_geometry(ctx, block, &sg, "ddamg_sap");
+    if (s != DDAMG_OK) return s;
+    cudaStream_t st = ctx->stream;
+    const bool hist = res_hist != nullptr;
+    const bool f32 = ctx->prec == DDAMG_F32;
+    const int dgrid = dslash_grid(ctx->g);
+    if (hist) { s = reset_hist(ctx); if (s != DDAMG_OK) return s; }
+    if (zero_init) {
+        CK(cudaMemsetAsync(x_e, 0, ctx->half_bytes, st));
+        CK(cudaMemsetAsync(x_o, 0, ctx->half_bytes, st));
+    }
+    // r = b - D x into (tmp_e, tmp_o); with a history also ||r||
+    auto residual = [&](bool norm) -> int {
+        int q = dslash(ctx, EPI_FULL_RESIDUAL, norm, 0, x_o, x_e, b_e, ctx->tmp_e, 0.0, 5);
+        if (q != DDAMG_OK) return q;
+        q = dslash(ctx, EPI_FULL_RESIDUAL, norm, 1, x_e, x_o, b_o, ctx->tmp_o, 0.0, 5, 1, (size_t)dgrid, ctx->clov_oo);
+        if (q != DDAMG_OK) return q;
+        if (norm) { launch_finalize_norm(ctx->partials, 2 * dgrid, ctx->sc, 1, st); q = after_launch(ctx); }
+        return q;
+    };
+    auto blocks = [&](int colour) -> int {
+        if (m == 0) return DDAMG_OK;                       // zero Minimal Residual iterations: e_k = 0
+        ddamg_ctx::Ev ev;
+        if (ctx->timing) {
+            if (cudaEventCreate(&ev.a) != cudaSuccess || cudaEventCreate(&ev.b) != cudaSuccess)
+                return check_cuda(ctx, cudaGetLastError(), "cudaEventCreate");
+            ev.which = 6;
+            cudaEventRecord(ev.a, st);
+        }
+        cudaError_t e = f32
+            ? launch_sap_blocks<float>(ctx->g, sg, colour, m, ctx->gauge, ctx->clov[0], ctx->clov[1], ctx->tmp_e, ctx->tmp_o, x_e, x_o, st)
+            : launch_sap_blocks<double>(ctx->g, sg, colour, m, ctx->gauge, ctx->clov[0], ctx->clov[1], ctx->tmp_e, ctx->tmp_o, x_e, x_o, st);
+        if (e != cudaSuccess) return check_cuda(ctx, e, "sap_block_kernel attributes");
+        if (ctx->timing) { cudaEventRecord(ev.b, st); ctx->events.push_back(ev); }
+        return after_launch(ctx);
+    };
+    for (int i = 0; i < n; ++i) {
+        s = residual(hist); if (s != DDAMG_OK) return s;             // line 2
+        s = blocks(0); if (s != DDAMG_OK) return s;                  // lines 4-6: red blocks
+        s = residual(false); if (s != DDAMG_OK) return s;            // line 7
+        s = blocks(1); if (s != DDAMG_OK) return s;                  // lines 8-10: black blocks
+    }
+    if (hist) {
+        s = residual(true); if (s != DDAMG_OK) return s;             // final true residual
+        return copy_hist(ctx, res_hist, n + 1, nullptr);
+    }
+    return DDAMG_OK;
+}
+
 // --------------------------------------------------------------------------- power iteration
 extern "C" int ddamg_power_iteration(ddamg_ctx* ctx, void* v_e, int iters, double* lambda_max)
 {

@@ -95,15 +95,16 @@ __device__ __forceinline__ void store_link(double* __restrict__ blk, int Vh, int
     for (int k = 0; k < 9; ++k) p[(size_t)k * Vh] = pack(&u[2 * k]);
 }
 
-// 36 reals of clover block b (0/1) of one site
-template <typename T>
+// 36 reals of clover block b (0/1) of one site.  STREAM: read once per kernel (evict-first);
+// !STREAM: re-read by the same CTA (SAP block solves), keep it cacheable.
+template <typename T, bool STREAM = true>
 __device__ __forceinline__ void load_clover_block(const T* __restrict__ base, int Vh, int cb, int b, T (&c)[36])
 {
     using V = typename VecOf<T>::type;
     constexpr int N = VecOf<T>::N;
     const V* p = reinterpret_cast<const V*>(base) + (size_t)b * (36 / N) * Vh + cb;
 #pragma unroll
-    for (int k = 0; k < 36 / N; ++k) unpack(ld_stream(p + (size_t)k * Vh), &c[k * N]);
+    for (int k = 0; k < 36 / N; ++k) unpack(STREAM ? ld_stream(p + (size_t)k * Vh) : ld_reuse(p + (size_t)k * Vh), &c[k * N]);
 }
 template <typename T>
 __device__ __forceinline__ void store_clover_block(T* __restrict__ base, int Vh, int cb, int b, const T (&c)[36])

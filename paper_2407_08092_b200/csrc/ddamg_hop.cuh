@@ -185,14 +185,14 @@ __device__ __forceinline__ void clover_block_mul(const T (&c)[36], const T* __re
 }
 
 // out = Cl(x) v for the two blocks of one site (upper: reals 0..11, lower: 12..23)
-template <typename T>
+template <typename T, bool STREAM = true>
 __device__ __forceinline__ void clover_site_mul(const T* __restrict__ clov, int Vh, int cb,
                                                 const T (&v)[24], T (&out)[24])
 {
     T c[36];
-    load_clover_block<T>(clov, Vh, cb, 0, c);
+    load_clover_block<T, STREAM>(clov, Vh, cb, 0, c);
     clover_block_mul<T>(c, &v[0], &out[0]);
-    load_clover_block<T>(clov, Vh, cb, 1, c);
+    load_clover_block<T, STREAM>(clov, Vh, cb, 1, c);
     clover_block_mul<T>(c, &v[12], &out[12]);
 }
 

@@ -15,6 +15,7 @@ constexpr int GMRES_KMAX = 64;          // largest cycle length m of GMRES(n, m)
 constexpr int HIST_MAX = 8192;         // residual-history entries kept on the device
 constexpr int NRHS_MAX = 32;            // right-hand sides per multi-rhs batch
 constexpr int MDOT_NB = 12;             // basis vectors handled per fused multi-dot / multi-axpy pass
+constexpr int SAP_MAX_THREADS = 256;    // SAP: sites per parity of one domain-decomposition block (<= 512-site blocks)
 
 // epilogues of the fused hopping kernel (ddamg_dslash.cu)
 enum {
@@ -35,6 +36,20 @@ void launch_dslash(const Geom& g, int epi, bool norm, int parity, const void* in
 template <typename T>
 void launch_clover_apply(const Geom& g, const void* clov, const void* in, void* out, int nrhs, cudaStream_t st);
 int dslash_grid(const Geom& g, int nrhs = 1);
+
+// ---- SAP block solves (ddamg_sap.cu)
+struct SapGeom {
+    int B[4];            // block extents (each even, dividing the lattice extent with an even quotient)
+    int Bxh;             // B[0] / 2
+    int Vbh;             // sites per parity of one block
+    int nb[4];           // blocks per direction
+    int nbxh;            // nb[0] / 2
+};
+size_t sap_smem_bytes(const SapGeom& sg, size_t real_bytes);
+template <typename T>
+cudaError_t launch_sap_blocks(const Geom& g, const SapGeom& sg, int colour, int m, const void* gauge,
+                              const void* clov_e, const void* clov_oinv, const void* r_e, const void* r_o,
+                              void* x_e, void* x_o, cudaStream_t st);
 
 // ---- setup (ddamg_setup.cu)
 template <typename Tin, typename T>

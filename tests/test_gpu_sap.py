@@ -1,0 +1,91 @@
+"""GPU parity of SAP(n, m) (Alg. 1) vs the oracle.
+
+The oracle (oracle/sap.py) recomputes r = b - D x before each colour and runs the per-block
+odd-even Minimal Residual with numpy on full-lattice vectors; the CUDA path does the block
+solves with one CTA per block out of shared memory.  Same seeded inputs, element by element.
+"""
+import ctypes
+
+import numpy as np
+import pytest
+import torch
+
+from helpers import rel_l2
+from test_gpu_parity import make_pair, _mods
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.mark.parametrize("cfg,prec,L,T,block,n,m", [
+    (1, "f64", 4, 4, (2, 2, 2, 2), 2, 3),        # config 1, smallest blocks (8 of 32 lanes active)
+    (1, "f32", 4, 4, (2, 2, 2, 2), 2, 3),
+    (4, "f32", 8, 8, (4, 4, 4, 4), 3, 4),        # the paper's SAP(3,4) on 4^4 blocks (Tables 1, 2, 6)
+    (4, "f64", 8, 8, (4, 4, 4, 4), 3, 4),
+    (3, "f32", 8, 16, (4, 2, 4, 4), 2, 4),       # anisotropic block, ragged last warp (64 of 64), 4 blocks along t
+    (2, "f64", 8, 8, (2, 4, 2, 4), 1, 5),
+    (3, "f32", 8, 16, (4, 4, 4, 8), 1, 2),       # 512-site blocks: 256 threads, the fp32 maximum
+    (2, "f32", 16, 16, (4, 4, 4, 4), 2, 4),      # 256 blocks: several CTAs per SM wave
+    (1, "f32", 4, 8, (2, 2, 2, 4), 2, 1),        # m = 1
+])
+def test_sap_matches_oracle(cfg, prec, L, T, block, n, m):
+    oracle, _ = _mods()
+    p = make_pair(cfg, prec, L, T)
+    b_np, b_d = p.spinor(9000 + cfg)
+    x_np, x_d = p.spinor(9050 + cfg)
+    b_e, b_o = p.ctx.pack(b_d)
+    x_e, x_o = p.ctx.pack(x_d)
+    hist = p.ctx.sap(b_e, b_o, x_e, x_o, n, m, block, zero_init=False, history=True)
+    x_ref, h_ref = oracle.sap(p.ora, b_np, x_np, n, m, block)
+    assert len(hist) == n + 1
+    tol_h = 1e-10 if p.f64 else 1e-4
+    for a, r in zip(hist, h_ref):
+        assert abs(a - r) <= tol_h * r, (hist, h_ref)
+    assert rel_l2(p.to_np(x_e, x_o), x_ref) <= (1e-11 if p.f64 else 2e-5)
+    # zero initial guess, no history (asynchronous path): bit-identical to the history path
+    y_e, y_o = p.ctx.half_spinor(), p.ctx.half_spinor()
+    y_e.fill_(7.0); y_o.fill_(-3.0)                                   # must be ignored
+    p.ctx.sap(b_e, b_o, y_e, y_o, n, m, block, zero_init=True)
+    z_e, z_o = p.ctx.half_spinor(zero=True), p.ctx.half_spinor(zero=True)
+    h0 = p.ctx.sap(b_e, b_o, z_e, z_o, n, m, block, zero_init=False, history=True)
+    assert torch.equal(y_e, z_e) and torch.equal(y_o, z_o)
+    x0_ref, h0_ref = oracle.sap(p.ora, b_np, np.zeros_like(b_np), n, m, block)
+    assert rel_l2(p.to_np(y_e, y_o), x0_ref) <= (1e-11 if p.f64 else 2e-5)
+    assert abs(h0[0] - np.linalg.norm(b_np)) <= (1e-12 if p.f64 else 1e-6) * h0[0]
+    assert all(abs(a - r) <= tol_h * r for a, r in zip(h0, h0_ref))
+
+
+def test_sap_smooths_and_m0_is_identity():
+    """SAP(n, 4) reduces the residual every iteration; SAP(n, 0) leaves x untouched."""
+    p = make_pair(4, "f32", 8, 8)
+    b_np, b_d = p.spinor(9101)
+    b_e, b_o = p.ctx.pack(b_d)
+    x_e, x_o = p.ctx.half_spinor(zero=True), p.ctx.half_spinor(zero=True)
+    hist = p.ctx.sap(b_e, b_o, x_e, x_o, 4, 4, (4, 4, 4, 4), history=True)
+    assert all(hist[i + 1] < 0.7 * hist[i] for i in range(4)), hist
+    keep_e, keep_o = x_e.clone(), x_o.clone()
+    h = p.ctx.sap(b_e, b_o, x_e, x_o, 2, 0, (4, 4, 4, 4), history=True)
+    assert torch.equal(keep_e, x_e) and torch.equal(keep_o, x_o)
+    assert h[0] == h[1] == h[2] and abs(h[0] - hist[-1]) <= 1e-5 * hist[-1]
+
+
+def test_sap_error_codes():
+    _, dd = _mods()
+    E = dd.binding
+    p = make_pair(1, "f64", 8, 8)
+    b = [p.ctx.half_spinor(zero=True) for _ in range(4)]
+    vp = lambda t: ctypes.c_void_p(t.data_ptr())
+    lib, h = p.ctx.lib, p.ctx._h
+    blk = lambda *v: (ctypes.c_int * 4)(*v)
+    call = lambda block, n=1, m=1, xe=b[2]: lib.ddamg_sap(h, vp(b[0]), vp(b[1]), vp(xe), vp(b[3]), n, m, block, 0, None)
+    assert call(blk(4, 4, 4, 4)) == E.OK
+    assert call(blk(8, 4, 4, 4)) == E.EINVAL          # one block along x
+    assert call(blk(3, 4, 4, 4)) == E.EINVAL          # odd extent
+    assert call(blk(4, 4, 4, 4), n=-1) == E.EINVAL
+    assert call(blk(4, 4, 4, 4), m=-1) == E.EINVAL
+    assert call(blk(4, 4, 4, 4), xe=b[0]) == E.EINVAL  # x_e aliases b_e
+    assert call(None) == E.EINVAL
+    p2 = make_pair(1, "f64", 8, 16)
+    c = [p2.ctx.half_spinor(zero=True) for _ in range(4)]
+    # 512-site blocks in fp64: 295 KB of links, more than a CTA's shared memory
+    assert p2.ctx.lib.ddamg_sap(p2.ctx._h, vp(c[0]), vp(c[1]), vp(c[2]), vp(c[3]), 1, 1, blk(4, 4, 4, 8), 0, None) == E.EINVAL
+    assert b"shared memory" in p2.ctx.lib.ddamg_last_error(p2.ctx._h)
