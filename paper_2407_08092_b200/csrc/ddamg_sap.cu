@@ -1,8 +1,9 @@
 // ddamg_sap.cu -- the block solves of SAP(n, m) (Alg. 1).
 //
 // One CTA per domain-decomposition block of one colour (Alg. 1 lines 4-6 / 8-10): given the
-// global residual r = b - D x (lines 2 / 7, computed by the fused full-operator kernel of
-// ddamg_dslash.cu) it runs m Minimal Residual iterations on the block system D_k e_k = r_k with
+// global residual r = b - D x (lines 2 / 7, computed by the streaming full-operator kernel of
+// ddamg_dslash.cu, which runs at the HBM roofline; evaluating it inside this low-occupancy
+// kernel was measured 1.6x slower) it runs m Minimal Residual iterations on D_k e_k = r_k with
 // block-local odd-even preconditioning ("each of the domain decomposition blocks"
 // is reordered and "minimal residual is used for solving the linear systems with the Schur
 // complement of each block") and adds e_k to x_k:
@@ -33,7 +34,7 @@ struct SapArgs {
     const T* gauge;          // [parity][mu] link blocks
     const T* clov_e;         // A_ee
     const T* clov_oinv;      // A_oo^-1
-    const T* r_e;            // global residual
+    const T* r_e;            // global residual r = b - D x
     const T* r_o;
     T* x_e;                  // iterate, updated in place on the blocks of this colour
     T* x_o;
@@ -159,116 +160,122 @@ __global__ void __launch_bounds__(SAP_MAX_THREADS, 1) sap_block_kernel(const Sap
     const int cx = 2 * cxh + ((cy + cz + ct + a.colour) & 1);
     const int ox = cx * sg.B[0], oy = cy * sg.B[1], oz = cz * sg.B[2], ot = ct * sg.B[3];
 
-    LSite se, so;
-    int cb_e = 0, cb_o = 0;                                    // global checkerboard indices of the two sites
+    LSite ls[2];                                               // this thread's even / odd site in the block
+    int cbg[2] = { 0, 0 };                                     // and their global checkerboard indices
+    T rho[24], e[24];
     if (active) {
-        se = lsite_of(sg, tid, 0);
-        so = lsite_of(sg, tid, 1);
-        cb_e = ((ox + se.lx) >> 1) + a.g.Lh * ((oy + se.ly) + a.g.L * ((oz + se.lz) + a.g.L * (ot + se.lt)));
-        cb_o = ((ox + so.lx) >> 1) + a.g.Lh * ((oy + so.ly) + a.g.L * ((oz + so.lz) + a.g.L * (ot + so.lt)));
+#pragma unroll
+        for (int p = 0; p < 2; ++p) {
+            ls[p] = lsite_of(sg, tid, p);
+            cbg[p] = ((ox + ls[p].lx) >> 1) + a.g.Lh * ((oy + ls[p].ly) + a.g.L * ((oz + ls[p].lz) + a.g.L * (ot + ls[p].lt)));
+        }
+    }
+    const int sblk = 4 * 18 * n;                               // one parity's four link blocks in shared memory
+    if (active) {
         // ---- stage the block's links (each is read once from HBM per launch)
         const size_t gblk = (size_t)18 * a.g.Vh;
         T u[18];
-#pragma unroll
-        for (int mu = 0; mu < 4; ++mu) {
-            load_link(a.gauge + (size_t)(0 * 4 + mu) * gblk, a.g.Vh, cb_e, u);
-            sts_link(links + (0 * 4 + mu) * 18 * n, n, tid, u);
-            load_link(a.gauge + (size_t)(1 * 4 + mu) * gblk, a.g.Vh, cb_o, u);
-            sts_link(links + (1 * 4 + mu) * 18 * n, n, tid, u);
+#pragma unroll 1
+        for (int pm = 0; pm < 8; ++pm) {                       // (parity, mu)
+            load_link(a.gauge + (size_t)pm * gblk, a.g.Vh, cbg[pm >> 2], u);
+            sts_link(links + pm * 18 * n, n, tid, u);
         }
-        // ---- eq. 2 right factor, odd half: t_o = A_oo^-1 r_o
+        // ---- eq. 2 right factor, odd half: t_o = A_oo^-1 r_o;  rho starts as r_e
         T v[24], t[24];
-        load_spinor<T, true>(a.r_o, a.g.Vh, cb_o, v);
-        clover_site_mul<T, false>(a.clov_oinv, a.g.Vh, cb_o, v, t);
+        load_spinor<T, false>(a.r_o, a.g.Vh, cbg[1], v);
+        clover_site_mul<T, false>(a.clov_oinv, a.g.Vh, cbg[1], v, t);
         sts_spinor<T>(S_o, n, tid, t);
+        load_spinor<T, true>(a.r_e, a.g.Vh, cbg[0], rho);
     }
     __syncthreads();
-    const T* links_e = links;
-    const T* links_o = links + 4 * 18 * n;
-    T rho[24], e[24];
-    if (active) {
-        // rho = rhat_e = r_e - H^k_eo t_o  (H = -1/2 acc)
+
+    // ---- the block solve as 2m+2 half steps, one copy of the block hopping code:
+    //   hs = 0        even:  rho = rhat_e = r_e - H^k_eo t_o;  e = 0
+    //   hs odd < last odd :  t_o = A_oo^-1 H^k_oe rho
+    //   hs even > 0   even:  q = A_ee rho - H^k_eo t_o;  alpha = <q,rho>/<q,q>;  e += alpha rho;  rho -= alpha q
+    //   hs = 2m+1     odd :  e_o = A_oo^-1 (r_o - H^k_oe e);  x += e
+    const int last = 2 * a.m + 1;
+#pragma unroll 1
+    for (int hs = 0; hs <= last; ++hs) {
+        const int par = hs & 1;
         T acc[24];
-        hop_block<T>(sg, tid, se, S_o, links_e, links_o, acc);
-        load_spinor<T, true>(a.r_e, a.g.Vh, cb_e, rho);
+        if (active)
+            hop_block<T>(sg, tid, ls[par], par ? S_e : S_o, links + par * sblk, links + (1 - par) * sblk, acc);
+        if (par) {
+            if (active) {
+                T v[24], t[24];
+                if (hs == last) {
+                    load_spinor<T, false>(a.r_o, a.g.Vh, cbg[1], v);
 #pragma unroll
-        for (int i = 0; i < 24; ++i) {
-            rho[i] = rho[i] + (T)0.5 * acc[i];
-            e[i] = 0;
-        }
-        sts_spinor<T>(S_e, n, tid, rho);
-    }
-    __syncthreads();
-    for (int it = 0; it < a.m; ++it) {
-        if (active) {
-            // t_o = A_oo^-1 H^k_oe rho
-            T acc[24], t[24];
-            hop_block<T>(sg, tid, so, S_e, links_o, links_e, acc);
+                    for (int i = 0; i < 24; ++i) v[i] = v[i] + (T)0.5 * acc[i];          // r_o - H e
+                } else {
 #pragma unroll
-            for (int i = 0; i < 24; ++i) acc[i] *= (T)(-0.5);
-            clover_site_mul<T, false>(a.clov_oinv, a.g.Vh, cb_o, acc, t);
-            sts_spinor<T>(S_o, n, tid, t);
-        }
-        __syncthreads();
-        T q[24];
-        double nr = 0.0, ni = 0.0, dd = 0.0;
-        if (active) {
-            // q = D^k_S rho = A_ee rho - H^k_eo t_o
-            T acc[24];
-            hop_block<T>(sg, tid, se, S_o, links_e, links_o, acc);
-            clover_site_mul<T, false>(a.clov_e, a.g.Vh, cb_e, rho, q);
+                    for (int i = 0; i < 24; ++i) v[i] = (T)(-0.5) * acc[i];              // H rho
+                }
+                clover_site_mul<T, false>(a.clov_oinv, a.g.Vh, cbg[1], v, t);
+                if (hs == last) {
+                    load_spinor<T, true>(a.x_o, a.g.Vh, cbg[1], v);
 #pragma unroll
-            for (int i = 0; i < 24; ++i) q[i] = q[i] + (T)0.5 * acc[i];
-            // <q, rho> = q^H rho and <q, q>, this site's share
+                    for (int i = 0; i < 24; ++i) v[i] += t[i];
+                    store_spinor<T>(a.x_o, a.g.Vh, cbg[1], v);
+                    load_spinor<T, true>(a.x_e, a.g.Vh, cbg[0], v);
 #pragma unroll
-            for (int c = 0; c < 12; ++c) {
-                const double qr = q[2 * c], qi = q[2 * c + 1], pr = rho[2 * c], pi = rho[2 * c + 1];
-                nr += qr * pr + qi * pi;
-                ni += qr * pi - qi * pr;
-                dd += qr * qr + qi * qi;
+                    for (int i = 0; i < 24; ++i) v[i] += e[i];
+                    store_spinor<T>(a.x_e, a.g.Vh, cbg[0], v);
+                } else {
+                    sts_spinor<T>(S_o, n, tid, t);
+                }
+            }
+        } else if (hs == 0) {
+            if (active) {
+#pragma unroll
+                for (int i = 0; i < 24; ++i) {
+                    rho[i] = rho[i] + (T)0.5 * acc[i];
+                    e[i] = 0;
+                }
+                sts_spinor<T>(S_e, n, tid, rho);
+            }
+        } else {
+            T q[24];
+            double nr = 0.0, ni = 0.0, dd = 0.0;
+            if (active) {
+                clover_site_mul<T, false>(a.clov_e, a.g.Vh, cbg[0], rho, q);
+#pragma unroll
+                for (int i = 0; i < 24; ++i) q[i] = q[i] + (T)0.5 * acc[i];
+                // <q, rho> = q^H rho and <q, q>, this site's share
+#pragma unroll
+                for (int c = 0; c < 12; ++c) {
+                    const double qr = q[2 * c], qi = q[2 * c + 1], pr = rho[2 * c], pi = rho[2 * c + 1];
+                    nr += qr * pr + qi * pi;
+                    ni += qr * pi - qi * pr;
+                    dd += qr * qr + qi * qi;
+                }
+            }
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                nr += __shfl_xor_sync(0xffffffffu, nr, o);
+                ni += __shfl_xor_sync(0xffffffffu, ni, o);
+                dd += __shfl_xor_sync(0xffffffffu, dd, o);
+            }
+            if (lane == 0) { red[3 * warp] = nr; red[3 * warp + 1] = ni; red[3 * warp + 2] = dd; }
+            __syncthreads();
+            nr = ni = dd = 0.0;
+            for (int w = 0; w < nwarps; ++w) { nr += red[3 * w]; ni += red[3 * w + 1]; dd += red[3 * w + 2]; }
+            const T ar = dd > 0.0 ? (T)(nr / dd) : (T)0, ai = dd > 0.0 ? (T)(ni / dd) : (T)0;
+            if (active) {
+#pragma unroll
+                for (int c = 0; c < 12; ++c) {
+                    const T pr = rho[2 * c], pi = rho[2 * c + 1];
+                    e[2 * c] += ar * pr - ai * pi;                     // e += alpha rho
+                    e[2 * c + 1] += ar * pi + ai * pr;
+                    rho[2 * c] -= ar * q[2 * c] - ai * q[2 * c + 1];   // rho -= alpha q
+                    rho[2 * c + 1] -= ar * q[2 * c + 1] + ai * q[2 * c];
+                }
+                if (hs + 1 < last) sts_spinor<T>(S_e, n, tid, rho);
+                else sts_spinor<T>(S_e, n, tid, e);
             }
         }
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-            nr += __shfl_xor_sync(0xffffffffu, nr, o);
-            ni += __shfl_xor_sync(0xffffffffu, ni, o);
-            dd += __shfl_xor_sync(0xffffffffu, dd, o);
-        }
-        if (lane == 0) { red[3 * warp] = nr; red[3 * warp + 1] = ni; red[3 * warp + 2] = dd; }
         __syncthreads();
-        nr = ni = dd = 0.0;
-        for (int w = 0; w < nwarps; ++w) { nr += red[3 * w]; ni += red[3 * w + 1]; dd += red[3 * w + 2]; }
-        const T ar = dd > 0.0 ? (T)(nr / dd) : (T)0, ai = dd > 0.0 ? (T)(ni / dd) : (T)0;
-        if (active) {
-#pragma unroll
-            for (int c = 0; c < 12; ++c) {
-                const T pr = rho[2 * c], pi = rho[2 * c + 1];
-                e[2 * c] += ar * pr - ai * pi;                   // e += alpha rho
-                e[2 * c + 1] += ar * pi + ai * pr;
-                rho[2 * c] -= ar * q[2 * c] - ai * q[2 * c + 1];   // rho -= alpha q
-                rho[2 * c + 1] -= ar * q[2 * c + 1] + ai * q[2 * c];
-            }
-            if (it + 1 < a.m) sts_spinor<T>(S_e, n, tid, rho);
-            else sts_spinor<T>(S_e, n, tid, e);
-        }
-        __syncthreads();
-    }
-    if (active) {
-        // eq. 2 left factor: e_o = A_oo^-1 (r_o - H^k_oe e);  x += e
-        T acc[24], v[24], eo[24];
-        hop_block<T>(sg, tid, so, S_e, links_o, links_e, acc);
-        load_spinor<T, true>(a.r_o, a.g.Vh, cb_o, v);
-#pragma unroll
-        for (int i = 0; i < 24; ++i) v[i] = v[i] + (T)0.5 * acc[i];
-        clover_site_mul<T, false>(a.clov_oinv, a.g.Vh, cb_o, v, eo);
-        load_spinor<T, true>(a.x_o, a.g.Vh, cb_o, v);
-#pragma unroll
-        for (int i = 0; i < 24; ++i) v[i] += eo[i];
-        store_spinor<T>(a.x_o, a.g.Vh, cb_o, v);
-        load_spinor<T, true>(a.x_e, a.g.Vh, cb_e, v);
-#pragma unroll
-        for (int i = 0; i < 24; ++i) v[i] += e[i];
-        store_spinor<T>(a.x_e, a.g.Vh, cb_e, v);
     }
 }
 
