@@ -60,7 +60,7 @@ enum {
 };
 enum { DDAMG_F32 = 0, DDAMG_F64 = 1 };
 enum { DDAMG_BC_PERIODIC = 0, DDAMG_BC_ANTIPERIODIC_T = 1 };
-enum { DDAMG_SMOOTHER_RICHARDSON = 0, DDAMG_SMOOTHER_GMRES = 1, DDAMG_SMOOTHER_GCR = 2 };
+enum { DDAMG_SMOOTHER_RICHARDSON = 0, DDAMG_SMOOTHER_GMRES = 1, DDAMG_SMOOTHER_GCR = 2, DDAMG_SMOOTHER_SAP = 3 };
 
 /* Library version string, e.g. "ddamg-b200 0.1 (sm_100a)". Never NULL. */
 const char* ddamg_version(void);
@@ -162,6 +162,9 @@ int ddamg_apply_full(ddamg_ctx* ctx, const void* x_e, const void* x_o, void* y_e
  *             z_o = A_oo^-1 (v_o - H_oe z_e)                                   (eq. 2)
  *   smoother = DDAMG_SMOOTHER_RICHARDSON: s_n sweeps with weight omega (s_m ignored)
  *              DDAMG_SMOOTHER_GMRES / _GCR: (n = s_n cycles, m = s_m) without tolerance
+ *              DDAMG_SMOOTHER_SAP: z = SAP(s_n, s_m) on D z = v from z = 0 (Alg. 1; acts on the
+ *              full system, no eq.-2 wrapper; block extents from the "sap_block_*" options,
+ *              default 4^4 as in Table 6; s_m = 0 is rejected)
  * The paper prints no FGMRES algorithm; reading R19: Alg. 2 with z_j = M v_j,
  * w = D z_j, x += Z_m y.  History layout, tol, zero_init as ddamg_gmres_oe (norms over both
  * parities).  x_e / x_o: initial guess in, solution out.  Keeps 2k+1 full-lattice vectors.
@@ -251,12 +254,15 @@ int ddamg_prepare_rhs_batch(ddamg_ctx* ctx, int nrhs, const void* B_e, const voi
 int ddamg_get_clover(ddamg_ctx* ctx, void* A_nat, void* Ainv_nat);
 
 /*
- * Tuning options (never change results, only the order in which sites are visited):
+ * Options:
  *   "batch_l2_bytes"  L2 budget (bytes, default 40e6) of the multi-rhs kernels' z-chunked
  *                     traversal: CTAs visit the lattice in chunks of zc z-planes (zc = largest
  *                     divisor of L with 3 * zc * one (z,t)-plane of batch spinors <= budget)
  *                     so that t-neighbours are re-read from L2, not HBM.  0 = smallest chunks;
- *                     a huge value = plain lexicographic order.
+ *                     a huge value = plain lexicographic order.  Never changes results.
+ *   "sap_block_x", "sap_block_y", "sap_block_z", "sap_block_t"
+ *                     block extents SAP uses as the FGMRES smoother (even integers >= 2,
+ *                     default 4; checked against the lattice when the smoother runs).
  * EINVAL for an unknown name or a bad value.
  */
 int ddamg_set_option(ddamg_ctx* ctx, const char* name, double value);

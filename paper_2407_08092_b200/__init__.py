@@ -7,6 +7,6 @@ libddamg.so in-tree.  There is no CPU fallback and this package never imports ``
 from .binding import (  # noqa: F401
     Ddamg, DdamgError, load_library, SYMBOLS, LIB_PATH,
     OK, EINVAL, ENOMEM, ESTATE, ECUDA, ESINGULAR, F32, F64, BC_PERIODIC, BC_ANTIPERIODIC_T,
-    SMOOTHER_RICHARDSON, SMOOTHER_GMRES, SMOOTHER_GCR,
+    SMOOTHER_RICHARDSON, SMOOTHER_GMRES, SMOOTHER_GCR, SMOOTHER_SAP,
 )
 from .build import build_library  # noqa: F401

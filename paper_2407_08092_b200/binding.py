@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(HERE, "libddamg.so")
 OK, EINVAL, ENOMEM, ESTATE, ECUDA, ESINGULAR = 0, -1, -2, -3, -4, -5
 F32, F64 = 0, 1
 BC_PERIODIC, BC_ANTIPERIODIC_T = 0, 1
-SMOOTHER_RICHARDSON, SMOOTHER_GMRES, SMOOTHER_GCR = 0, 1, 2
+SMOOTHER_RICHARDSON, SMOOTHER_GMRES, SMOOTHER_GCR, SMOOTHER_SAP = 0, 1, 2, 3
 
 _STATUS = {0: "DDAMG_OK", -1: "DDAMG_EINVAL", -2: "DDAMG_ENOMEM", -3: "DDAMG_ESTATE",
            -4: "DDAMG_ECUDA", -5: "DDAMG_ESINGULAR"}

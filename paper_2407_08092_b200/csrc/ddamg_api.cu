@@ -36,6 +36,7 @@ struct ddamg_ctx {
     double* partials_batch;     // multi-rhs reduction scratch
     int batch_cap;
     double batch_l2_bytes;      // L2 budget of the z-chunked multi-rhs traversal (option "batch_l2_bytes")
+    int sap_block[4];           // SAP block extents used when SAP is the FGMRES smoother (options "sap_block_x".."_t")
     double* partials;           // reduction scratch
     size_t partials_len;
     Scalars* sc;                // device scalars
@@ -129,6 +130,7 @@ extern "C" int ddamg_create(ddamg_ctx** out, int L, int T, double csw, double m0
     ctx->kcap = 0;
     ctx->clov_oo = nullptr; ctx->sc2 = nullptr; ctx->fgm_basis = nullptr; ctx->fgm_cap = 0;
     ctx->tmp_batch = nullptr; ctx->partials_batch = nullptr; ctx->batch_cap = 0; ctx->batch_l2_bytes = 40e6;
+    for (int mu = 0; mu < 4; ++mu) ctx->sap_block[mu] = 4;
     ctx->partials = nullptr; ctx->sc = nullptr; ctx->host_hist = nullptr; ctx->singular = nullptr;
     ctx->have_gauge = ctx->have_clover = ctx->have_clov_oo = false;
     ctx->sticky = DDAMG_OK; ctx->launches = 0; ctx->timing = false;
@@ -802,6 +804,8 @@ extern "C" int ddamg_apply_full(ddamg_ctx* ctx, const void* x_e, const void* x_o
 static int smoother_call(ddamg_ctx* ctx, int smoother, int s_n, int s_m, double omega, const void* v_e, const void* v_o,
                          void* z_e, void* z_o)
 {
+    if (smoother == DDAMG_SMOOTHER_SAP)      // z = SAP(s_n, s_m) on D z = v from z = 0 (acts on the full system, no eq. 2 wrapper)
+        return ddamg_sap(ctx, v_e, v_o, z_e, z_o, s_n, s_m, ctx->sap_block, 1, nullptr);
     int s = ddamg_prepare_rhs(ctx, v_e, v_o, ctx->tmp_e);
     if (s != DDAMG_OK) return s;
     switch (smoother) {
@@ -943,9 +947,10 @@ extern "C" int ddamg_fgmres(ddamg_ctx* ctx, const void* b_e, const void* b_o, vo
     ENTER(ctx);
     if (!b_e || !b_o || !x_e || !x_o || b_e == x_e || b_o == x_o || k < 1 || cycles < 1 || tol < 0.0 || s_n < 1)
         return fail(ctx, DDAMG_EINVAL, "ddamg_fgmres: bad arguments");
-    if (smoother != DDAMG_SMOOTHER_RICHARDSON && (s_m < 1 || s_m > GMRES_KMAX))
+    if ((smoother == DDAMG_SMOOTHER_GMRES || smoother == DDAMG_SMOOTHER_GCR) && (s_m < 1 || s_m > GMRES_KMAX))
         return fail(ctx, DDAMG_EINVAL, "ddamg_fgmres: bad inner cycle length");
-    if (smoother < DDAMG_SMOOTHER_RICHARDSON || smoother > DDAMG_SMOOTHER_GCR)
+    if (smoother == DDAMG_SMOOTHER_SAP && s_m < 1) return fail(ctx, DDAMG_EINVAL, "ddamg_fgmres: SAP needs at least one Minimal Residual iteration");
+    if (smoother < DDAMG_SMOOTHER_RICHARDSON || smoother > DDAMG_SMOOTHER_SAP)
         return fail(ctx, DDAMG_EINVAL, "ddamg_fgmres: unknown smoother");
     if (k > GMRES_KMAX) return fail(ctx, DDAMG_EINVAL, "ddamg_fgmres: k exceeds 64");
     if ((long long)cycles * (k + 1) + 1 > HIST_MAX) return fail(ctx, DDAMG_EINVAL, "ddamg_fgmres: history too long");
@@ -1100,6 +1105,14 @@ extern "C" int ddamg_set_option(ddamg_ctx* ctx, const char* name, double value)
         ctx->batch_l2_bytes = value;
         return DDAMG_OK;
     }
+    static const char* const sap_names[4] = { "sap_block_x", "sap_block_y", "sap_block_z", "sap_block_t" };
+    for (int mu = 0; mu < 4; ++mu)
+        if (strcmp(name, sap_names[mu]) == 0) {
+            const int B = (int)value;
+            if ((double)B != value || B < 2 || (B & 1)) return fail(ctx, DDAMG_EINVAL, "ddamg_set_option: SAP block extents must be even integers >= 2");
+            ctx->sap_block[mu] = B;
+            return DDAMG_OK;
+        }
     return fail(ctx, DDAMG_EINVAL, std::string("ddamg_set_option: unknown option ") + name);
 }
 

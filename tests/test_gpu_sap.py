@@ -89,3 +89,42 @@ def test_sap_error_codes():
     # 512-site blocks in fp64: 295 KB of links, more than a CTA's shared memory
     assert p2.ctx.lib.ddamg_sap(p2.ctx._h, vp(c[0]), vp(c[1]), vp(c[2]), vp(c[3]), 1, 1, blk(4, 4, 4, 8), 0, None) == E.EINVAL
     assert b"shared memory" in p2.ctx.lib.ddamg_last_error(p2.ctx._h)
+
+
+@pytest.mark.parametrize("cfg,prec,L,T,block,k,s_n,s_m", [
+    (1, "f64", 4, 4, (2, 2, 2, 2), 5, 2, 3),
+    (4, "f32", 8, 8, (4, 4, 4, 4), 6, 1, 4),
+])
+def test_fgmres_with_sap_smoother_matches_oracle(cfg, prec, L, T, block, k, s_n, s_m):
+    """Outer FGMRES preconditioned by z = SAP(s_n, s_m) v from z = 0: the paper's default solver
+    configuration (Table 6) minus the coarse grid.  SAP is a fixed linear map, so the oracle's
+    FGMRES with the oracle's SAP as preconditioner is the reference."""
+    from test_gpu_parity import _check_history
+    oracle, dd = _mods()
+    p = make_pair(cfg, prec, L, T)
+    for name, B in zip(("sap_block_x", "sap_block_y", "sap_block_z", "sap_block_t"), block):
+        p.ctx.set_option(name, B)
+    b_np, b_d = p.spinor(9200 + cfg)
+    b_e, b_o = p.ctx.pack(b_d)
+    x_e, x_o = p.ctx.half_spinor(), p.ctx.half_spinor()
+    hist = p.ctx.fgmres(b_e, b_o, x_e, x_o, k, 1, 0.0, dd.SMOOTHER_SAP, s_n, s_m, 0.0, zero_init=True)
+    M = lambda v: oracle.sap(p.ora, v, np.zeros_like(v), s_n, s_m, block)[0]
+    x_ref, h_ref = oracle.fgmres(p.ora.apply_D, M, b_np, np.zeros_like(b_np), k, 1)
+    _check_history(hist, h_ref, np.linalg.norm(b_np), p.f64)
+    assert rel_l2(p.to_np(x_e, x_o), x_ref) <= (1e-8 if p.f64 else 1e-4)
+    assert hist[-1] < 1e-2 * hist[0]                       # SAP-preconditioned FGMRES converges fast
+
+
+def test_sap_options_error_codes():
+    _, dd = _mods()
+    p = make_pair(1, "f32")
+    with pytest.raises(dd.DdamgError):
+        p.ctx.set_option("sap_block_x", 3)
+    with pytest.raises(dd.DdamgError):
+        p.ctx.set_option("sap_block_q", 4)
+    b_e, b_o, x_e, x_o = (p.ctx.half_spinor(zero=True) for _ in range(4))
+    # default 4^4 blocks do not two-colour a 4^4 lattice: the smoother reports it
+    with pytest.raises(dd.DdamgError):
+        p.ctx.fgmres(b_e, b_o, x_e, x_o, 2, 1, 0.0, dd.SMOOTHER_SAP, 1, 1, 0.0)
+    with pytest.raises(dd.DdamgError):
+        p.ctx.fgmres(b_e, b_o, x_e, x_o, 2, 1, 0.0, dd.SMOOTHER_SAP, 1, 0, 0.0)
