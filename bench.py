@@ -52,6 +52,9 @@ FLOP_PER_SITE = 1824    # 1320 (hop) + 504 (2 x 6x6 Hermitian mat-vec), per latt
 # ncu --set full capture summarised in profiles/ (None until a capture exists)
 NCU_TRAFFIC_BYTES = {5: 21.274e9, 3: None}     # profiles/r1b_ncu_full_dslash.md
 CPU_SAMPLE = dict(L=16, T=32)
+# SAP(n, m) row: the paper's smoother parameters (Tables 1, 2, 6) on 4^4 blocks
+SAP_N, SAP_M, SAP_BLOCK = 3, 4, (4, 4, 4, 4)
+SAP_HOP_FLOP = 990      # in-block hopping sum: on a 4^4 block 6 of the 8 neighbours are inside on average (1320 * 6/8)
 
 
 def _peaks():
@@ -353,6 +356,32 @@ def main():
             rows["gmres_1x10"] = {"ms": ms, "ms_per_arnoldi_step": ms / kg}
         except Exception as e:     # e.g. Krylov basis does not fit
             rows["gmres_1x10"] = {"error": str(e)}
+        # ---- SAP(3,4) on 4^4 blocks (NEXT-3; the smoother of the paper's Tables 2 and 6)
+        try:
+            xs_e, xs_o = ctx.half_spinor(), ctx.half_spinor()
+            ctx.kernel_timing(True)
+            ctx.kernel_time_ms(6, reset=True)
+            ksap = 3
+            ms = timed(lambda i: ctx.sap(pool_b[i % NPOOL][0], pool_b[i % NPOOL][1], xs_e, xs_o, SAP_N, SAP_M,
+                                         SAP_BLOCK, zero_init=False), ksap, 1,
+                       lambda i: (xs_e.copy_(pool_x[i % NPOOL]), xs_o.copy_(pool_x[(i + 1) % NPOOL]))) / ksap
+            ms5, n5 = ctx.kernel_time_ms(5, reset=False)
+            ms6, n6 = ctx.kernel_time_ms(6, reset=True)
+            ctx.kernel_timing(False)
+            t6 = ms6 / max(n6, 1) * 1e-3
+            # block kernel: per block site pair 2m+2 in-block hopping sums and 2m+2 6x6x2 products
+            flop_blk = (2 * SAP_M + 2) * (SAP_HOP_FLOP + 504) * Ve / 2
+            rows["sap_3x4_block4"] = {
+                "ms_per_call": ms, "site_iterations_per_s": V * SAP_N / (ms * 1e-3),
+                "block_kernel_ms": t6 * 1e3, "block_kernel_launches": n6,
+                "residual_kernel_ms": ms5 / max(n5, 1), "residual_kernel_launches": n5,
+                "block_kernel_GFLOPps": flop_blk / t6 / 1e9,
+                "block_kernel_bound": "latency (8 warps/SM; fp32 FMA pipe ~20 % busy, profiles/r1c_ncu_full_sap.md)",
+                "note": "SAP(n=3, m=4), 4^4 blocks, non-zero x0: per iteration and colour one streaming residual "
+                        "(2 launches) + one block-solve launch"}
+            del xs_e, xs_o
+        except Exception as e:
+            rows["sap_3x4_block4"] = {"error": str(e)}
 
     if args.rows in ("all", "multi_rhs"):
         # ---- multi-rhs batched Richardson (NEXT-2): links + clover fetched once for nrhs rhs
