@@ -263,6 +263,18 @@ int ddamg_get_clover(ddamg_ctx* ctx, void* A_nat, void* Ainv_nat);
  *   "sap_block_x", "sap_block_y", "sap_block_z", "sap_block_t"
  *                     block extents SAP uses as the FGMRES smoother (even integers >= 2,
  *                     default 4; checked against the lattice when the smoother runs).
+ *   "gauge_recon"     18 (default) or 12.  12 = two-row link storage: the
+ *                     fused hopping kernels (Schur apply, Richardson, GMRES, GCR, eq.-2
+ *                     factors, full operator, multi-rhs) read rows 0 and 1 of each SU(3) link
+ *                     (48 B instead of 72 B in fp32) from a second, context-owned copy and
+ *                     rebuild row 2 = conj(row0 x row1) in registers (sign of the antiperiodic
+ *                     boundary restored).  May be set before or after ddamg_load_gauge; every
+ *                     later ddamg_load_gauge re-compresses.  The links must be SU(3): if any
+ *                     stored third row differs from the rebuilt one by more than 2e-6 (fp32
+ *                     context) / 1e-12 (fp64) the call returns EINVAL and the context stays
+ *                     on 18-real links.  Results change by rounding only (third rows are
+ *                     rebuilt from rounded rows).  Clover build and SAP block solves always
+ *                     use the full links.
  * EINVAL for an unknown name or a bad value.
  */
 int ddamg_set_option(ddamg_ctx* ctx, const char* name, double value);

@@ -7,7 +7,7 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libddamg.so")
-SOURCES = ["ddamg_api.cu", "ddamg_dslash.cu", "ddamg_setup.cu", "ddamg_blas.cu", "ddamg_sap.cu"]
+SOURCES = ["ddamg_api.cu", "ddamg_dslash.cu", "ddamg_dslash12.cu", "ddamg_setup.cu", "ddamg_blas.cu", "ddamg_sap.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
     "-Xcompiler", "-fPIC", "--use_fast_math=false",

@@ -23,6 +23,10 @@ struct ddamg_ctx {
     size_t half_bytes;          // one native half spinor
     size_t nreal;               // reals per half spinor = 24 * Vh
     void* gauge;                // [parity][mu] link blocks
+    void* gauge12;              // two-row copy of the links (option "gauge_recon" = 12), else NULL
+    int recon;                  // 18 or 12: link format read by the fused hopping kernels
+    unsigned int* recon_dev;    // device: largest |stored row 2 - rebuilt row 2| of the last compression
+    double recon_deviation;     // host copy of it
     void* clov[2];              // [0] = A_ee blocks, [1] = A_oo^-1 blocks
     void* tmp_o;                // t_o of eq. 3
     void* tmp_e;                // scratch half spinor (power iteration, final residual)
@@ -94,6 +98,48 @@ static void* gauge_block(ddamg_ctx* c, int parity)
     return (char*)c->gauge + (size_t)parity * 4 * 18 * c->g.Vh * c->real_bytes;
 }
 
+// link blocks read by the fused hopping kernels: the two-row copy when gauge_recon = 12
+static void* hop_gauge_block(ddamg_ctx* c, int parity)
+{
+    if (c->recon == 12) return (char*)c->gauge12 + (size_t)parity * 4 * 12 * c->g.Vh * c->real_bytes;
+    return gauge_block(c, parity);
+}
+
+// (Re)build the two-row copy from the packed links; refuses links that are not SU(3).
+static int compress_gauge(ddamg_ctx* ctx)
+{
+    if (!ctx->gauge12) {
+        cudaError_t e = cudaMalloc(&ctx->gauge12, (size_t)2 * 4 * 12 * ctx->g.Vh * ctx->real_bytes);
+        if (e == cudaSuccess && !ctx->recon_dev) e = cudaMalloc((void**)&ctx->recon_dev, sizeof(unsigned int));
+        if (e != cudaSuccess) {
+            cudaGetLastError();
+            cudaFree(ctx->gauge12); ctx->gauge12 = nullptr;
+            ctx->recon = 18;
+            return fail(ctx, DDAMG_ENOMEM, "gauge_recon: cannot allocate the two-row link copy");
+        }
+    }
+    int s = check_cuda(ctx, cudaMemsetAsync(ctx->recon_dev, 0, sizeof(unsigned int), ctx->stream), "gauge_recon memset");
+    if (s != DDAMG_OK) return s;
+    if (ctx->prec == DDAMG_F32) launch_compress_gauge<float>(ctx->g, ctx->bc, ctx->gauge, ctx->gauge12, ctx->recon_dev, ctx->stream);
+    else launch_compress_gauge<double>(ctx->g, ctx->bc, ctx->gauge, ctx->gauge12, ctx->recon_dev, ctx->stream);
+    ctx->launches += 1;
+    s = check_cuda(ctx, cudaGetLastError(), "kernel launch");
+    if (s != DDAMG_OK) return s;
+    float dev = 0.f;
+    s = check_cuda(ctx, cudaMemcpyAsync(&dev, ctx->recon_dev, sizeof(float), cudaMemcpyDeviceToHost, ctx->stream), "gauge_recon D2H");
+    if (s == DDAMG_OK) s = check_cuda(ctx, cudaStreamSynchronize(ctx->stream), "gauge_recon sync");
+    if (s != DDAMG_OK) return s;
+    ctx->recon_deviation = dev;
+    const double tol = ctx->prec == DDAMG_F32 ? 2e-6 : 1e-12;
+    if (!(dev <= tol)) {
+        ctx->recon = 18;
+        char msg[200];
+        snprintf(msg, sizeof msg, "gauge_recon = 12 refused: links are not SU(3) (third row differs from conj(row0 x row1) by %.3g > %.1g); using 18-real links", (double)dev, tol);
+        return fail(ctx, DDAMG_EINVAL, msg);
+    }
+    return DDAMG_OK;
+}
+
 extern "C" const char* ddamg_version(void) { return "ddamg-b200 0.1 (sm_100a)"; }
 
 extern "C" const char* ddamg_last_error(ddamg_ctx* ctx) { return ctx ? ctx->err.c_str() : g_err_noctx.c_str(); }
@@ -126,6 +172,7 @@ extern "C" int ddamg_create(ddamg_ctx** out, int L, int T, double csw, double m0
     ctx->real_bytes = prec == DDAMG_F32 ? 4 : 8;
     ctx->nreal = (size_t)24 * ctx->g.Vh;
     ctx->half_bytes = ctx->nreal * ctx->real_bytes;
+    ctx->gauge12 = nullptr; ctx->recon = 18; ctx->recon_dev = nullptr; ctx->recon_deviation = 0.0;
     ctx->gauge = ctx->clov[0] = ctx->clov[1] = ctx->tmp_o = ctx->tmp_e = ctx->krylov = nullptr;
     ctx->kcap = 0;
     ctx->clov_oo = nullptr; ctx->sc2 = nullptr; ctx->fgm_basis = nullptr; ctx->fgm_cap = 0;
@@ -167,6 +214,7 @@ extern "C" int ddamg_destroy(ddamg_ctx* ctx)
     if (!ctx) return DDAMG_OK;
     cudaStreamSynchronize(ctx->stream);
     for (auto& ev : ctx->events) { cudaEventDestroy(ev.a); cudaEventDestroy(ev.b); }
+    cudaFree(ctx->gauge12); cudaFree(ctx->recon_dev);
     cudaFree(ctx->gauge); cudaFree(ctx->clov[0]); cudaFree(ctx->clov[1]);
     cudaFree(ctx->tmp_o); cudaFree(ctx->tmp_e); cudaFree(ctx->krylov);
     cudaFree(ctx->tmp_batch); cudaFree(ctx->partials_batch);
@@ -211,6 +259,7 @@ extern "C" int ddamg_load_gauge(ddamg_ctx* ctx, const void* U, int u_prec, int o
     ctx->have_gauge = true;
     ctx->have_clover = false;
     ctx->have_clov_oo = false;
+    if (ctx->recon == 12) return compress_gauge(ctx);      // option set before the links arrived
     return DDAMG_OK;
 }
 
@@ -277,11 +326,11 @@ static int dslash(ddamg_ctx* ctx, int epi, bool norm, int parity, const void* in
         cudaEventRecord(ev.a, ctx->stream);
     }
     if (ctx->prec == DDAMG_F32)
-        launch_dslash<float>(ctx->g, epi, norm, parity, in, gauge_block(ctx, parity), gauge_block(ctx, 1 - parity),
-                             clov, own, rhs, out, omega, partials, nrhs, ctx->batch_l2_bytes, ctx->stream);
+        launch_dslash<float>(ctx->g, epi, norm, parity, in, hop_gauge_block(ctx, parity), hop_gauge_block(ctx, 1 - parity),
+                             clov, own, rhs, out, omega, partials, nrhs, ctx->batch_l2_bytes, ctx->recon, ctx->bc == 1, ctx->stream);
     else
-        launch_dslash<double>(ctx->g, epi, norm, parity, in, gauge_block(ctx, parity), gauge_block(ctx, 1 - parity),
-                              clov, own, rhs, out, omega, partials, nrhs, ctx->batch_l2_bytes, ctx->stream);
+        launch_dslash<double>(ctx->g, epi, norm, parity, in, hop_gauge_block(ctx, parity), hop_gauge_block(ctx, 1 - parity),
+                              clov, own, rhs, out, omega, partials, nrhs, ctx->batch_l2_bytes, ctx->recon, ctx->bc == 1, ctx->stream);
     if (ctx->timing) {
         cudaEventRecord(ev.b, ctx->stream);
         ctx->events.push_back(ev);
@@ -1103,6 +1152,12 @@ extern "C" int ddamg_set_option(ddamg_ctx* ctx, const char* name, double value)
     if (strcmp(name, "batch_l2_bytes") == 0) {
         if (!(value >= 0.0)) return fail(ctx, DDAMG_EINVAL, "ddamg_set_option: batch_l2_bytes must be >= 0");
         ctx->batch_l2_bytes = value;
+        return DDAMG_OK;
+    }
+    if (strcmp(name, "gauge_recon") == 0) {
+        if (value != 12.0 && value != 18.0) return fail(ctx, DDAMG_EINVAL, "ddamg_set_option: gauge_recon must be 18 or 12");
+        ctx->recon = (int)value;
+        if (ctx->recon == 12 && ctx->have_gauge) return compress_gauge(ctx);
         return DDAMG_OK;
     }
     static const char* const sap_names[4] = { "sap_block_x", "sap_block_y", "sap_block_z", "sap_block_t" };

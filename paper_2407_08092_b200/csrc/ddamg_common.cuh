@@ -95,6 +95,57 @@ __device__ __forceinline__ void store_link(double* __restrict__ blk, int Vh, int
     for (int k = 0; k < 9; ++k) p[(size_t)k * Vh] = pack(&u[2 * k]);
 }
 
+// Two-row (12-real) link storage (option "gauge_recon" = 12; SURVEY.md 8(d) "two-row link
+// storage"): per (parity, mu) a block of 12*Vh reals holding rows 0 and 1 of U_mu(x)
+// (fp32: 3 planes of float4, fp64: 6 planes of double2).  For U in SU(3) the third row is
+// conj(row0 x row1); the antiperiodic sign folded into the stored rows of U_t(T-1) does not
+// survive the cross product, so the caller passes sgn = -1 for those links.
+template <typename T>
+__device__ __forceinline__ void reconstruct_row2(T sgn, T (&u)[18])
+{
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const int a = (c + 1) % 3, b = (c + 2) % 3;
+        // row0[a] * row1[b] - row0[b] * row1[a], conjugated
+        T re = u[2 * a] * u[6 + 2 * b];
+        re = fma(-u[2 * a + 1], u[6 + 2 * b + 1], re);
+        re = fma(-u[2 * b], u[6 + 2 * a], re);
+        re = fma(u[2 * b + 1], u[6 + 2 * a + 1], re);
+        T im = u[2 * a] * u[6 + 2 * b + 1];
+        im = fma(u[2 * a + 1], u[6 + 2 * b], im);
+        im = fma(-u[2 * b], u[6 + 2 * a + 1], im);
+        im = fma(-u[2 * b + 1], u[6 + 2 * a], im);
+        u[12 + 2 * c] = sgn * re;
+        u[12 + 2 * c + 1] = -sgn * im;
+    }
+}
+__device__ __forceinline__ void load_link12(const float* __restrict__ blk, int Vh, int cb, float sgn, float (&u)[18])
+{
+    const float4* p4 = reinterpret_cast<const float4*>(blk) + cb;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) unpack(ld_stream(p4 + (size_t)k * Vh), &u[4 * k]);
+    reconstruct_row2<float>(sgn, u);
+}
+__device__ __forceinline__ void load_link12(const double* __restrict__ blk, int Vh, int cb, double sgn, double (&u)[18])
+{
+    const double2* p = reinterpret_cast<const double2*>(blk) + cb;
+#pragma unroll
+    for (int k = 0; k < 6; ++k) unpack(ld_stream(p + (size_t)k * Vh), &u[2 * k]);
+    reconstruct_row2<double>(sgn, u);
+}
+__device__ __forceinline__ void store_link12(float* __restrict__ blk, int Vh, int cb, const float (&u)[18])
+{
+    float4* p4 = reinterpret_cast<float4*>(blk) + cb;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) p4[(size_t)k * Vh] = pack(&u[4 * k]);
+}
+__device__ __forceinline__ void store_link12(double* __restrict__ blk, int Vh, int cb, const double (&u)[18])
+{
+    double2* p = reinterpret_cast<double2*>(blk) + cb;
+#pragma unroll
+    for (int k = 0; k < 6; ++k) p[(size_t)k * Vh] = pack(&u[2 * k]);
+}
+
 // 36 reals of clover block b (0/1) of one site.  STREAM: read once per kernel (evict-first);
 // !STREAM: re-read by the same CTA (SAP block solves), keep it cacheable.
 template <typename T, bool STREAM = true>

@@ -1,0 +1,210 @@
+// ddamg_dslash_kernel.cuh -- the fused hopping + clover kernel template, instantiated once per
+// link storage format: RECON = 18 in ddamg_dslash.cu, RECON = 12 (two-row links) in
+// ddamg_dslash12.cu.
+#pragma once
+#include "ddamg_internal.h"
+#include "ddamg_hop.cuh"
+
+namespace ddamg {
+
+template <typename T>
+struct DslashArgs {
+    Geom g;
+    int parity;              // parity of the output sites
+    const T* in;             // opposite-parity spinor (the 8 neighbours)
+    const T* gauge_own;      // 4 link blocks of the output parity
+    const T* gauge_opp;      // 4 link blocks of the opposite parity
+    const T* clov;           // clover blocks stored for the output parity
+    const T* own;            // own-site spinor (EPI_SCHUR / RICHARDSON / RESIDUAL)
+    const T* rhs;            // b (EPI_RICHARDSON / RESIDUAL / *_RHS_*)
+    T* out;
+    T omega;
+    double* partials;        // per-block sum of |r|^2 (NORM) or nullptr; batch: [block][nrhs]
+    int nrhs;                // BATCH kernels: right-hand sides interleaved per site (else 1)
+    int zc;                  // BATCH: z-chunk of the CTA traversal (0 = plain lexicographic order)
+    int cpp;                 // BATCH: CTAs per (z,t) plane = Lh * L * nrhs / DSLASH_THREADS (when zc > 0)
+    int apbc;                // RECON = 12: antiperiodic time boundary (sign of the rebuilt third row of U_t(T-1))
+};
+
+__device__ __forceinline__ double block_sum(double v)
+{
+    __shared__ double warp_part[32];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    if (lane == 0) warp_part[w] = v;
+    __syncthreads();
+    const int nw = (blockDim.x + 31) >> 5;
+    v = (threadIdx.x < nw) ? warp_part[threadIdx.x] : 0.0;
+    if (w == 0) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    }
+    return v;     // valid in thread 0
+}
+
+// Register budget per thread (ptxas trades registers for loads in flight; measured on B200,
+// 128 registers = 4 CTAs of 128 threads per SM is the optimum for both
+// the kernel-A class (EPI <= EPI_RHS_MINUS_HOP) and the kernel-B class).
+#ifndef DDAMG_MAXREG_A
+#define DDAMG_MAXREG_A 128
+#endif
+#ifndef DDAMG_MAXREG_B
+#define DDAMG_MAXREG_B 128
+#endif
+
+// BATCH (multi-rhs): one thread per (site, rhs), rhs fastest, so that the
+// nrhs threads of a site share every link / clover vector they load while all spinor planes
+// stay contiguous per warp (vector index cb * nrhs + r).
+template <typename T, int EPI, bool NORM, bool BATCH, int RECON>
+__global__ void __launch_bounds__(DSLASH_THREADS)
+__maxnreg__(sizeof(T) == 4 ? (EPI <= EPI_RHS_MINUS_HOP ? DDAMG_MAXREG_A : DDAMG_MAXREG_B) : 255)
+dslash_kernel(const DslashArgs<T> a)
+{
+    // BATCH: with nrhs spinors per site one time slice of neighbour spinors no longer fits L2
+    // (64^3: nrhs * 12.6 MB), so the t-1 neighbours would be re-fetched from HBM.  CTAs therefore
+    // walk the lattice in z-chunks: for each chunk of zc z-planes, t runs over the whole time
+    // extent before the next chunk starts, which keeps three t-slabs of the chunk L2-resident.
+    int blk = blockIdx.x;
+    if (BATCH && a.zc > 0) {
+        const int plane = blk / a.cpp, within = blk - plane * a.cpp;     // plane in chunked order
+        const int per_chunk = a.zc * a.g.T;
+        const int chunk = plane / per_chunk, rem = plane - chunk * per_chunk;
+        const int t = rem / a.zc, z = chunk * a.zc + (rem - t * a.zc);
+        blk = (t * a.g.L + z) * a.cpp + within;
+    }
+    const int tid = blk * DSLASH_THREADS + threadIdx.x;
+    const int nrhs = BATCH ? a.nrhs : 1;
+    const int cb = BATCH ? tid / nrhs : tid;
+    const int rr = BATCH ? tid - cb * nrhs : 0;
+    const int Vs = a.g.Vh * nrhs;          // vectors per spinor plane
+    const int sv = cb * nrhs + rr;         // this thread's vector index in a spinor plane (== tid)
+    double nrm = 0.0;
+    if (cb < a.g.Vh) {
+        const Site s = site_of_cb(a.g, cb, a.parity);
+        T acc[24];
+        hop_site<T, RECON>(a.g, cb, s, a.in, nrhs, rr, a.gauge_own, a.gauge_opp, acc, a.apbc);
+        T res[24];
+        if (EPI == EPI_CLOV_HOP) {
+#pragma unroll
+            for (int i = 0; i < 24; ++i) acc[i] *= (T)(-0.5);
+            clover_site_mul<T>(a.clov, a.g.Vh, cb, acc, res);
+        } else if (EPI == EPI_CLOV_RHS_MINUS_HOP) {
+            T b[24];
+            load_spinor<T, true>(a.rhs, Vs, sv, b);
+#pragma unroll
+            for (int i = 0; i < 24; ++i) acc[i] = b[i] + (T)0.5 * acc[i];
+            clover_site_mul<T>(a.clov, a.g.Vh, cb, acc, res);
+        } else if (EPI == EPI_RHS_MINUS_HOP) {
+            T b[24];
+            load_spinor<T, true>(a.rhs, Vs, sv, b);
+#pragma unroll
+            for (int i = 0; i < 24; ++i) res[i] = b[i] + (T)0.5 * acc[i];
+        } else {
+            T x[24], ax[24];
+            load_spinor<T, true>(a.own, Vs, sv, x);
+            clover_site_mul<T>(a.clov, a.g.Vh, cb, x, ax);
+            // H = -1/2 acc:  Schur forms subtract H t (+1/2 acc), the full operator adds H x (-1/2 acc)
+            constexpr bool FULL = (EPI == EPI_FULL || EPI == EPI_FULL_RESIDUAL);
+            const T hs = FULL ? (T)(-0.5) : (T)0.5;
+            if (EPI == EPI_SCHUR || EPI == EPI_FULL) {
+#pragma unroll
+                for (int i = 0; i < 24; ++i) res[i] = ax[i] + hs * acc[i];     // A x - H t   or   A x + H x'
+            } else {
+                T b[24];
+                load_spinor<T, true>(a.rhs, Vs, sv, b);
+#pragma unroll
+                for (int i = 0; i < 24; ++i) {
+                    const T r = b[i] - (ax[i] + hs * acc[i]);
+                    if (NORM) nrm += (double)r * (double)r;
+                    res[i] = (EPI == EPI_RICHARDSON) ? x[i] + a.omega * r : r;
+                }
+            }
+        }
+        store_spinor<T>(a.out, Vs, sv, res);
+    }
+    if (NORM) {
+        if (BATCH) {
+            // per-rhs partial sums of this block: thread q < nrhs adds the entries of rhs q
+            __shared__ double per_thread[DSLASH_THREADS];
+            per_thread[threadIdx.x] = nrm;
+            __syncthreads();
+            if ((int)threadIdx.x < nrhs) {
+                const int first = (int)(((long long)blk * DSLASH_THREADS) % nrhs);          // rhs of thread 0
+                int i = (int)threadIdx.x - first;
+                if (i < 0) i += nrhs;
+                double tot = 0.0;
+                for (; i < DSLASH_THREADS; i += nrhs) tot += per_thread[i];
+                a.partials[(size_t)blk * nrhs + threadIdx.x] = tot;
+            }
+        } else {
+            const double tot = block_sum(nrm);
+            if (threadIdx.x == 0) a.partials[blockIdx.x] = tot;
+        }
+    }
+}
+
+template <typename T, int EPI, bool NORM, int RECON>
+static void launch(const DslashArgs<T>& a, cudaStream_t st)
+{
+    const int grid = dslash_grid(a.g, a.nrhs);
+    if (a.nrhs > 1) dslash_kernel<T, EPI, NORM, true, RECON><<<grid, DSLASH_THREADS, 0, st>>>(a);
+    else dslash_kernel<T, EPI, NORM, false, RECON><<<grid, DSLASH_THREADS, 0, st>>>(a);
+}
+
+template <typename T, int RECON>
+void launch_dslash_recon(const Geom& g, int epi, bool norm, int parity, const void* in, const void* gauge_own,
+                         const void* gauge_opp, const void* clov, const void* own, const void* rhs, void* out,
+                         double omega, double* partials, int nrhs, double batch_l2_bytes, int apbc, cudaStream_t st)
+{
+    DslashArgs<T> a;
+    a.apbc = apbc;
+    a.nrhs = nrhs;
+    a.zc = 0;
+    a.cpp = 0;
+    const long long plane_threads = (long long)g.Lh * g.L * nrhs;
+    if (nrhs > 1 && plane_threads % DSLASH_THREADS == 0) {
+        // largest divisor zc of L whose three t-slabs of spinors (zc planes each) fit the L2 budget
+        const double plane_bytes = (double)g.Lh * g.L * nrhs * 24 * sizeof(T);
+        int zc = 0;
+        for (int d = 1; d <= g.L; ++d)
+            if (g.L % d == 0 && 3.0 * d * plane_bytes <= batch_l2_bytes) zc = d;
+        if (zc == 0) zc = 1;
+        if (zc < g.L) {
+            a.zc = zc;
+            a.cpp = (int)(plane_threads / DSLASH_THREADS);
+        }
+    }
+    a.g = g;
+    a.parity = parity;
+    a.in = (const T*)in;
+    a.gauge_own = (const T*)gauge_own;
+    a.gauge_opp = (const T*)gauge_opp;
+    a.clov = (const T*)clov;
+    a.own = (const T*)own;
+    a.rhs = (const T*)rhs;
+    a.out = (T*)out;
+    a.omega = (T)omega;
+    a.partials = partials;
+    switch (epi) {
+    case EPI_CLOV_HOP: launch<T, EPI_CLOV_HOP, false, RECON>(a, st); break;
+    case EPI_CLOV_RHS_MINUS_HOP: launch<T, EPI_CLOV_RHS_MINUS_HOP, false, RECON>(a, st); break;
+    case EPI_RHS_MINUS_HOP: launch<T, EPI_RHS_MINUS_HOP, false, RECON>(a, st); break;
+    case EPI_SCHUR: launch<T, EPI_SCHUR, false, RECON>(a, st); break;
+    case EPI_RICHARDSON:
+        if (norm) launch<T, EPI_RICHARDSON, true, RECON>(a, st);
+        else launch<T, EPI_RICHARDSON, false, RECON>(a, st);
+        break;
+    case EPI_RESIDUAL:
+        if (norm) launch<T, EPI_RESIDUAL, true, RECON>(a, st);
+        else launch<T, EPI_RESIDUAL, false, RECON>(a, st);
+        break;
+    case EPI_FULL: launch<T, EPI_FULL, false, RECON>(a, st); break;
+    case EPI_FULL_RESIDUAL:
+        if (norm) launch<T, EPI_FULL_RESIDUAL, true, RECON>(a, st);
+        else launch<T, EPI_FULL_RESIDUAL, false, RECON>(a, st);
+        break;
+    }
+}
+
+}  // namespace ddamg

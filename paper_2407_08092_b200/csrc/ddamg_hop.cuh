@@ -125,14 +125,19 @@ __device__ __forceinline__ void hop_dir(const T (&psi)[24], const T (&u)[18], T 
 // Multi-rhs: `in` holds nrhs spinors interleaved per site (vector index
 // cb * nrhs + r, plane stride Vh * nrhs); links are indexed by site only, so the nrhs
 // adjacent threads of one site read the same link vectors (one DRAM fetch, L1 broadcast).
-template <typename T>
+// RECON = 18: full links.  RECON = 12: two-row storage, third row rebuilt in registers
+// (load_link12); apbc != 0 then restores the antiperiodic sign of the links U_t(t = T-1).
+template <typename T, int RECON = 18>
 __device__ __forceinline__ void hop_site(const Geom& g, int cb, const Site& s,
                                          const T* __restrict__ in, const int nrhs, const int r,
                                          const T* __restrict__ gauge_own,
-                                         const T* __restrict__ gauge_opp, T (&acc)[24])
+                                         const T* __restrict__ gauge_opp, T (&acc)[24], const int apbc = 0)
 {
     const int Vs = g.Vh * nrhs;                 // vectors per spinor plane
-    const size_t lblk = (size_t)18 * g.Vh;      // reals per (parity, mu) link block
+    const size_t lblk = (size_t)RECON * g.Vh;   // reals per (parity, mu) link block
+    // sign of the third row of the forward / backward link in direction MU (RECON = 12 only)
+    const T sgn_f3 = (apbc && s.t == g.T - 1) ? (T)-1 : (T)1;
+    const T sgn_b3 = (apbc && s.t == 0) ? (T)-1 : (T)1;
 #pragma unroll
     for (int i = 0; i < 24; ++i) acc[i] = 0;
     T psi[24], u[18];
@@ -143,10 +148,12 @@ __device__ __forceinline__ void hop_site(const Geom& g, int cb, const Site& s,
     nbs[6] = neighbour_cb<3, +1>(g, cb, s); nbs[7] = neighbour_cb<3, -1>(g, cb, s);
 #define DDAMG_HOP(MU)                                                        \
     load_spinor<T>(in, Vs, nbs[2 * MU] * nrhs + r, psi);                     \
-    load_link(gauge_own + MU * lblk, g.Vh, cb, u);                           \
+    if (RECON == 12) load_link12(gauge_own + MU * lblk, g.Vh, cb, MU == 3 ? sgn_f3 : (T)1, u); \
+    else load_link(gauge_own + MU * lblk, g.Vh, cb, u);                      \
     hop_dir<MU, true>(psi, u, acc);                                          \
     load_spinor<T>(in, Vs, nbs[2 * MU + 1] * nrhs + r, psi);                 \
-    load_link(gauge_opp + MU * lblk, g.Vh, nbs[2 * MU + 1], u);              \
+    if (RECON == 12) load_link12(gauge_opp + MU * lblk, g.Vh, nbs[2 * MU + 1], MU == 3 ? sgn_b3 : (T)1, u); \
+    else load_link(gauge_opp + MU * lblk, g.Vh, nbs[2 * MU + 1], u);         \
     hop_dir<MU, false>(psi, u, acc);
     DDAMG_HOP(0)
     DDAMG_HOP(1)

@@ -32,7 +32,14 @@ enum {
 template <typename T>
 void launch_dslash(const Geom& g, int epi, bool norm, int parity, const void* in, const void* gauge_own,
                    const void* gauge_opp, const void* clov, const void* own, const void* rhs, void* out,
-                   double omega, double* partials, int nrhs, double batch_l2_bytes, cudaStream_t st);
+                   double omega, double* partials, int nrhs, double batch_l2_bytes, int recon, int apbc,
+                   cudaStream_t st);
+// two-row copy of the packed gauge field (option "gauge_recon" = 12) + max deviation of the
+// stored third rows from conj(row0 x row1): *dev_max_bits = bit pattern of the largest
+// absolute deviation as a non-negative float (atomicMax on the bits; zero it first)
+template <typename T>
+void launch_compress_gauge(const Geom& g, int bc, const void* gauge, void* gauge12, unsigned int* dev_max_bits,
+                           cudaStream_t st);
 template <typename T>
 void launch_clover_apply(const Geom& g, const void* clov, const void* in, void* out, int nrhs, cudaStream_t st);
 int dslash_grid(const Geom& g, int nrhs = 1);

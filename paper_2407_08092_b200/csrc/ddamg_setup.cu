@@ -69,6 +69,47 @@ template void launch_pack_gauge<double, float>(const Geom&, int, const void*, vo
 template void launch_pack_gauge<float, double>(const Geom&, int, const void*, void*, cudaStream_t);
 template void launch_pack_gauge<double, double>(const Geom&, int, const void*, void*, cudaStream_t);
 
+// ------------------------------------------------------------------ two-row link copy
+// gauge12 = rows 0, 1 of every packed link (sign of the antiperiodic boundary included, as in
+// `gauge`).  Also measures how far the stored third rows are from sgn * conj(row0 x row1): the
+// caller refuses two-row storage for links that are not SU(3) to working precision.
+template <typename T>
+__global__ void compress_gauge_kernel(Geom g, int bc, const T* __restrict__ gauge, T* __restrict__ gauge12,
+                                      unsigned int* __restrict__ dev_max_bits)
+{
+    const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    float dev = 0.f;
+    if (idx < 2 * g.Vh) {
+        const int parity = idx / g.Vh, cb = idx % g.Vh;
+        const Site s = site_of_cb(g, cb, parity);
+#pragma unroll
+        for (int mu = 0; mu < 4; ++mu) {
+            T u[18], v[18];
+            load_link(gauge + ((size_t)parity * 4 + mu) * (size_t)18 * g.Vh, g.Vh, cb, u);
+#pragma unroll
+            for (int k = 0; k < 12; ++k) v[k] = u[k];
+            const T sgn = (bc == 1 && mu == 3 && s.t == g.T - 1) ? (T)-1 : (T)1;
+            reconstruct_row2<T>(sgn, v);
+#pragma unroll
+            for (int k = 12; k < 18; ++k) dev = fmaxf(dev, fabsf((float)(v[k] - u[k])));
+            store_link12(gauge12 + ((size_t)parity * 4 + mu) * (size_t)12 * g.Vh, g.Vh, cb, u);
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) dev = fmaxf(dev, __shfl_xor_sync(0xffffffffu, dev, o));
+    if ((threadIdx.x & 31) == 0 && dev > 0.f) atomicMax(dev_max_bits, __float_as_uint(dev));
+}
+
+template <typename T>
+void launch_compress_gauge(const Geom& g, int bc, const void* gauge, void* gauge12, unsigned int* dev_max_bits,
+                           cudaStream_t st)
+{
+    const int n = 2 * g.Vh;
+    compress_gauge_kernel<T><<<(n + 255) / 256, 256, 0, st>>>(g, bc, (const T*)gauge, (T*)gauge12, dev_max_bits);
+}
+template void launch_compress_gauge<float>(const Geom&, int, const void*, void*, unsigned int*, cudaStream_t);
+template void launch_compress_gauge<double>(const Geom&, int, const void*, void*, unsigned int*, cudaStream_t);
+
 // ------------------------------------------------------------------ spinor layout converters
 template <typename T>
 __global__ void pack_spinor_kernel(Geom g, const T* __restrict__ nat, T* __restrict__ xe, T* __restrict__ xo)
