@@ -191,7 +191,12 @@ def main():
     ap.add_argument("--rows", default="all", help="'all', 'main' (skip the side measurements) or 'multi_rhs' (main + multi-rhs rows)")
     ap.add_argument("--nrhs", default="2,4,8", help="batch sizes of the multi-rhs rows")
     ap.add_argument("--batch-l2-bytes", type=float, default=None, help="override ddamg option batch_l2_bytes")
+    ap.add_argument("--gauge-recon", type=int, default=18, choices=[18, 12],
+                    help="link storage read by the fused hopping kernels: 18 reals, or two-row 12 reals (ddamg option gauge_recon)")
     args = ap.parse_args()
+    global BYTES_A, BYTES_B, BYTES_BR
+    if args.gauge_recon == 12:          # 8 links x (72 - 48) B less per output site and kernel
+        BYTES_A, BYTES_B, BYTES_BR = BYTES_A - 192, BYTES_B - 192, BYTES_BR - 192
     if args.impl == "reference":
         run_reference(args)
         return
@@ -237,6 +242,8 @@ def main():
     e1.record()
     ctx.build_clover()
     e2.record()
+    if args.gauge_recon == 12:
+        ctx.set_option("gauge_recon", 12)
     torch.cuda.synchronize()
     t_a0, t_a1 = e0.elapsed_time(e1), e1.elapsed_time(e2)
     del U
@@ -319,7 +326,7 @@ def main():
     ach_A = BYTES_A * Ve / tA / 1e9
     roofline = {"bound": "hbm", "kernel": "dslash_kernel<float, EPI_RICHARDSON> (kernel B')",
                 "achieved": ach_B, "peak": peak, "unit": "GB/s", "frac": ach_B / peak,
-                "traffic": NCU_TRAFFIC_BYTES.get(cfg), "peak_source": peak_src,
+                "traffic": NCU_TRAFFIC_BYTES.get(cfg) if args.gauge_recon == 18 else None, "peak_source": peak_src,
                 "bytes_per_launch": BYTES_BR * Ve, "avg_launch_ms": tB * 1e3, "launches_timed": nB,
                 "other_kernels": [{"kernel": "dslash_kernel<float, EPI_CLOV_HOP> (kernel A)", "achieved": ach_A,
                                    "frac": ach_A / peak, "bytes_per_launch": BYTES_A * Ve, "avg_launch_ms": tA * 1e3,
@@ -442,6 +449,8 @@ def main():
                                f"omega={c['omega']}) on Gaussian b_e and non-zero Gaussian x0",
                    "l2_policy": "working set per sweep (gauge+clover+spinors = %.1f GB) is far larger than the 126 MB L2; no flush needed"
                                 % ((BYTES_A + BYTES_BR) * Ve / 1e9),
+                   "gauge_recon": args.gauge_recon,
+                   "bytes_per_even_site": {"kernel_A": BYTES_A, "kernel_B": BYTES_B, "kernel_Bprime": BYTES_BR},
                    "multi_gpu": "replicas only (no sharding, no collective on the data path)",
                    "timing": "sum of per-step CUDA-event times on the launching stream; x0 refresh copy outside the events",
                    "wall_s_timed_region": wall},
