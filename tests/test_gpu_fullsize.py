@@ -38,7 +38,7 @@ def _cut(field: torch.Tensor, origin, B, L, T) -> torch.Tensor:
 
 
 class FullSize:
-    def __init__(self):
+    def __init__(self, recon=18):
         import oracle
         import paper_2407_08092_b200 as dd
         self.oracle, self.dd = oracle, dd
@@ -51,6 +51,8 @@ class FullSize:
         self.ctx = dd.Ddamg(self.L, self.T, c["csw"], c["m0"], c["bc"], dd.F32)
         self.ctx.load_gauge(self.U)
         self.ctx.build_clover()
+        if recon == 12:                        # bench.py --gauge-recon 12: two-row links in the hopping kernels
+            self.ctx.set_option("gauge_recon", 12)
         self.x_nat = gen.spinor_field(self.L, self.T, 3000 + CFG, device=dev, dtype=torch.complex64)
         self.b_nat = gen.spinor_field(self.L, self.T, 2000 + CFG, device=dev, dtype=torch.complex64)
         self.x_e, _ = self.ctx.pack(self.x_nat, want_odd=False)
@@ -70,9 +72,9 @@ class FullSize:
         return ora, np.where(ora.even, xb, 0.0), np.where(ora.even, bb, 0.0)
 
 
-@pytest.fixture(scope="module")
-def fs():
-    f = FullSize()
+@pytest.fixture(scope="module", params=[18, 12], ids=["links18", "links12"])
+def fs(request):
+    f = FullSize(request.param)
     yield f
     f.ctx.close()
 
