@@ -40,6 +40,9 @@ struct ddamg_ctx {
     double* partials_batch;     // multi-rhs reduction scratch
     int batch_cap;
     double batch_l2_bytes;      // L2 budget of the z-chunked multi-rhs traversal (option "batch_l2_bytes")
+    void* sap_links;            // SAP: block-ordered copy of the links (launch_sap_reorder), or NULL
+    void* sap_clov;             // SAP: block-ordered copy of A_ee / A_oo^-1
+    int sap_built[4];           // block extents the two copies were built for ({0,..} = stale)
     int sap_block[4];           // SAP block extents used when SAP is the FGMRES smoother (options "sap_block_x".."_t")
     double* partials;           // reduction scratch
     size_t partials_len;
@@ -178,6 +181,8 @@ extern "C" int ddamg_create(ddamg_ctx** out, int L, int T, double csw, double m0
     ctx->clov_oo = nullptr; ctx->sc2 = nullptr; ctx->fgm_basis = nullptr; ctx->fgm_cap = 0;
     ctx->tmp_batch = nullptr; ctx->partials_batch = nullptr; ctx->batch_cap = 0; ctx->batch_l2_bytes = 40e6;
     for (int mu = 0; mu < 4; ++mu) ctx->sap_block[mu] = 4;
+    ctx->sap_links = ctx->sap_clov = nullptr;
+    for (int mu = 0; mu < 4; ++mu) ctx->sap_built[mu] = 0;
     ctx->partials = nullptr; ctx->sc = nullptr; ctx->host_hist = nullptr; ctx->singular = nullptr;
     ctx->have_gauge = ctx->have_clover = ctx->have_clov_oo = false;
     ctx->sticky = DDAMG_OK; ctx->launches = 0; ctx->timing = false;
@@ -215,6 +220,7 @@ extern "C" int ddamg_destroy(ddamg_ctx* ctx)
     cudaStreamSynchronize(ctx->stream);
     for (auto& ev : ctx->events) { cudaEventDestroy(ev.a); cudaEventDestroy(ev.b); }
     cudaFree(ctx->gauge12); cudaFree(ctx->recon_dev);
+    cudaFree(ctx->sap_links); cudaFree(ctx->sap_clov);
     cudaFree(ctx->gauge); cudaFree(ctx->clov[0]); cudaFree(ctx->clov[1]);
     cudaFree(ctx->tmp_o); cudaFree(ctx->tmp_e); cudaFree(ctx->krylov);
     cudaFree(ctx->tmp_batch); cudaFree(ctx->partials_batch);
@@ -259,6 +265,7 @@ extern "C" int ddamg_load_gauge(ddamg_ctx* ctx, const void* U, int u_prec, int o
     ctx->have_gauge = true;
     ctx->have_clover = false;
     ctx->have_clov_oo = false;
+    ctx->sap_built[0] = 0;
     if (ctx->recon == 12) return compress_gauge(ctx);      // option set before the links arrived
     return DDAMG_OK;
 }
@@ -279,6 +286,7 @@ extern "C" int ddamg_build_clover(ddamg_ctx* ctx)
     CK(cudaStreamSynchronize(ctx->stream));
     if (flag) return fail(ctx, DDAMG_ESINGULAR, "ddamg_build_clover: a 6x6 odd-site block is numerically singular");
     ctx->have_clover = true;
+    ctx->sap_built[0] = 0;                                  // SAP operand copies are stale
     return DDAMG_OK;
 }
 
@@ -1067,6 +1075,24 @@ extern "C" int ddamg_sap(ddamg_ctx* ctx, const void* b_e, const void* b_o, void*
     const bool hist = res_hist != nullptr;
     const bool f32 = ctx->prec == DDAMG_F32;
     const int dgrid = dslash_grid(ctx->g);
+    // block-ordered links and clover blocks for this geometry (built once, kept until the
+    // gauge field, the clover term or the block extents change)
+    if (m > 0 && memcmp(ctx->sap_built, sg.B, sizeof(int) * 4) != 0) {
+        if (!ctx->sap_links) {
+            cudaError_t e = cudaMalloc(&ctx->sap_links, (size_t)2 * 4 * 18 * ctx->g.Vh * ctx->real_bytes);
+            if (e == cudaSuccess) e = cudaMalloc(&ctx->sap_clov, (size_t)2 * 72 * ctx->g.Vh * ctx->real_bytes);
+            if (e != cudaSuccess) {
+                cudaGetLastError();
+                cudaFree(ctx->sap_links); ctx->sap_links = nullptr;
+                return fail(ctx, DDAMG_ENOMEM, "ddamg_sap: cannot allocate the block-ordered operand copies");
+            }
+        }
+        if (f32) launch_sap_reorder<float>(ctx->g, sg, ctx->gauge, ctx->clov[0], ctx->clov[1], ctx->sap_links, ctx->sap_clov, st);
+        else launch_sap_reorder<double>(ctx->g, sg, ctx->gauge, ctx->clov[0], ctx->clov[1], ctx->sap_links, ctx->sap_clov, st);
+        s = after_launch(ctx);
+        if (s != DDAMG_OK) return s;
+        memcpy(ctx->sap_built, sg.B, sizeof(int) * 4);
+    }
     if (hist) { s = reset_hist(ctx); if (s != DDAMG_OK) return s; }
     if (zero_init) {
         CK(cudaMemsetAsync(x_e, 0, ctx->half_bytes, st));
@@ -1091,8 +1117,8 @@ extern "C" int ddamg_sap(ddamg_ctx* ctx, const void* b_e, const void* b_o, void*
             cudaEventRecord(ev.a, st);
         }
         cudaError_t e = f32
-            ? launch_sap_blocks<float>(ctx->g, sg, colour, m, ctx->gauge, ctx->clov[0], ctx->clov[1], ctx->tmp_e, ctx->tmp_o, x_e, x_o, st)
-            : launch_sap_blocks<double>(ctx->g, sg, colour, m, ctx->gauge, ctx->clov[0], ctx->clov[1], ctx->tmp_e, ctx->tmp_o, x_e, x_o, st);
+            ? launch_sap_blocks<float>(ctx->g, sg, colour, m, ctx->sap_links, ctx->sap_clov, ctx->tmp_e, ctx->tmp_o, x_e, x_o, st)
+            : launch_sap_blocks<double>(ctx->g, sg, colour, m, ctx->sap_links, ctx->sap_clov, ctx->tmp_e, ctx->tmp_o, x_e, x_o, st);
         if (e != cudaSuccess) return check_cuda(ctx, e, "sap_block_kernel attributes");
         if (ctx->timing) { cudaEventRecord(ev.b, st); ctx->events.push_back(ev); }
         return after_launch(ctx);

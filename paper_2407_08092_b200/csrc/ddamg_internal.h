@@ -53,9 +53,14 @@ struct SapGeom {
     int nbxh;            // nb[0] / 2
 };
 size_t sap_smem_bytes(const SapGeom& sg, size_t real_bytes);
+// block-ordered copies of the links (2 * 4 * 18 reals per site pair) and of A_ee / A_oo^-1
+// (2 * 72 reals per site pair), V/2 site pairs each, for one block geometry
 template <typename T>
-cudaError_t launch_sap_blocks(const Geom& g, const SapGeom& sg, int colour, int m, const void* gauge,
-                              const void* clov_e, const void* clov_oinv, const void* r_e, const void* r_o,
+void launch_sap_reorder(const Geom& g, const SapGeom& sg, const void* gauge, const void* clov_e, const void* clov_oinv,
+                        void* blk_links, void* blk_clov, cudaStream_t st);
+template <typename T>
+cudaError_t launch_sap_blocks(const Geom& g, const SapGeom& sg, int colour, int m, const void* blk_links,
+                              const void* blk_clov, const void* r_e, const void* r_o,
                               void* x_e, void* x_o, cudaStream_t st);
 
 // ---- setup (ddamg_setup.cu)

@@ -31,9 +31,8 @@ struct SapArgs {
     SapGeom sg;
     int colour;              // colour of the blocks this launch solves (0 = red)
     int m;                   // Minimal Residual iterations (>= 1)
-    const T* gauge;          // [parity][mu] link blocks
-    const T* clov_e;         // A_ee
-    const T* clov_oinv;      // A_oo^-1
+    const T* blk_links;      // block-ordered links:  [block][parity][mu][18 * n]   (sap_reorder_kernel)
+    const T* blk_clov;       // block-ordered A_ee / A_oo^-1 blocks:  [block][parity][72 * n]
     const T* r_e;            // global residual r = b - D x
     const T* r_o;
     T* x_e;                  // iterate, updated in place on the blocks of this colour
@@ -159,6 +158,9 @@ __global__ void __launch_bounds__(SAP_MAX_THREADS, 1) sap_block_kernel(const Sap
     const int ct = r / sg.nb[2];
     const int cx = 2 * cxh + ((cy + cz + ct + a.colour) & 1);
     const int ox = cx * sg.B[0], oy = cy * sg.B[1], oz = cz * sg.B[2], ot = ct * sg.B[3];
+    const size_t bid = (size_t)cx + (size_t)sg.nb[0] * (cy + (size_t)sg.nb[1] * (cz + (size_t)sg.nb[2] * ct));
+    const T* clov_e = a.blk_clov + bid * 2 * 72 * n;          // this block's A_ee, in-block SoA (n sites)
+    const T* clov_oinv = clov_e + 72 * n;                      // and A_oo^-1
 
     LSite ls[2];                                               // this thread's even / odd site in the block
     int cbg[2] = { 0, 0 };                                     // and their global checkerboard indices
@@ -171,19 +173,20 @@ __global__ void __launch_bounds__(SAP_MAX_THREADS, 1) sap_block_kernel(const Sap
         }
     }
     const int sblk = 4 * 18 * n;                               // one parity's four link blocks in shared memory
+    {
+        // ---- stage the block's links (read once from HBM per launch): the block-ordered copy has
+        // the shared-memory layout, so this is one contiguous, fully coalesced 16-byte-vector copy
+        using V = typename VecOf<T>::type;
+        const V* src = reinterpret_cast<const V*>(a.blk_links + bid * 2 * sblk);
+        V* dst = reinterpret_cast<V*>(links);
+        const int nv = 2 * sblk / VecOf<T>::N;
+        for (int i = tid; i < nv; i += blockDim.x) dst[i] = ld_stream(src + i);
+    }
     if (active) {
-        // ---- stage the block's links (each is read once from HBM per launch)
-        const size_t gblk = (size_t)18 * a.g.Vh;
-        T u[18];
-#pragma unroll 1
-        for (int pm = 0; pm < 8; ++pm) {                       // (parity, mu)
-            load_link(a.gauge + (size_t)pm * gblk, a.g.Vh, cbg[pm >> 2], u);
-            sts_link(links + pm * 18 * n, n, tid, u);
-        }
         // ---- eq. 2 right factor, odd half: t_o = A_oo^-1 r_o;  rho starts as r_e
         T v[24], t[24];
         load_spinor<T, false>(a.r_o, a.g.Vh, cbg[1], v);
-        clover_site_mul<T, false>(a.clov_oinv, a.g.Vh, cbg[1], v, t);
+        clover_site_mul<T, false>(clov_oinv, n, tid, v, t);
         sts_spinor<T>(S_o, n, tid, t);
         load_spinor<T, true>(a.r_e, a.g.Vh, cbg[0], rho);
     }
@@ -212,7 +215,7 @@ __global__ void __launch_bounds__(SAP_MAX_THREADS, 1) sap_block_kernel(const Sap
 #pragma unroll
                     for (int i = 0; i < 24; ++i) v[i] = (T)(-0.5) * acc[i];              // H rho
                 }
-                clover_site_mul<T, false>(a.clov_oinv, a.g.Vh, cbg[1], v, t);
+                clover_site_mul<T, false>(clov_oinv, n, tid, v, t);
                 if (hs == last) {
                     load_spinor<T, true>(a.x_o, a.g.Vh, cbg[1], v);
 #pragma unroll
@@ -239,7 +242,7 @@ __global__ void __launch_bounds__(SAP_MAX_THREADS, 1) sap_block_kernel(const Sap
             T q[24];
             double nr = 0.0, ni = 0.0, dd = 0.0;
             if (active) {
-                clover_site_mul<T, false>(a.clov_e, a.g.Vh, cbg[0], rho, q);
+                clover_site_mul<T, false>(clov_e, n, tid, rho, q);
 #pragma unroll
                 for (int i = 0; i < 24; ++i) q[i] = q[i] + (T)0.5 * acc[i];
                 // <q, rho> = q^H rho and <q, q>, this site's share
@@ -279,19 +282,72 @@ __global__ void __launch_bounds__(SAP_MAX_THREADS, 1) sap_block_kernel(const Sap
     }
 }
 
+// ---- block-ordered operand copies (built once per block geometry, ddamg_api.cu caches them)
+// In the checkerboard layout a 4^4 block owns x-runs of two sites per parity: 32-byte runs, so
+// half of every 64-byte DRAM access and three quarters of every 128-byte L2 line were wasted
+// on the links and on the 6x6 blocks that all 2m+2 half steps re-read (profiles/
+// r1c_ncu_full_sap.md).  Here every block's links and clover blocks are stored contiguously in
+// the block's own SoA order (plane-major, n = V_b/2 sites per plane), block id = cx + nbx (cy +
+// nby (cz + nbz ct)) over the blocks of BOTH colours.
+template <typename T>
+__global__ void sap_reorder_kernel(Geom g, SapGeom sg, const T* __restrict__ gauge, const T* __restrict__ clov_e,
+                                   const T* __restrict__ clov_oinv, T* __restrict__ blk_links, T* __restrict__ blk_clov)
+{
+    const int n = sg.Vbh, i = threadIdx.x;
+    if (i >= n) return;
+    int r = blockIdx.x;
+    const int cx = r % sg.nb[0]; r /= sg.nb[0];
+    const int cy = r % sg.nb[1]; r /= sg.nb[1];
+    const int cz = r % sg.nb[2];
+    const int ct = r / sg.nb[2];
+    const size_t bid = blockIdx.x;
+    const size_t gblk = (size_t)18 * g.Vh;
+#pragma unroll 1
+    for (int p = 0; p < 2; ++p) {
+        const LSite ls = lsite_of(sg, i, p);
+        const int cbg = ((cx * sg.B[0] + ls.lx) >> 1) +
+                        g.Lh * ((cy * sg.B[1] + ls.ly) + g.L * ((cz * sg.B[2] + ls.lz) + g.L * (ct * sg.B[3] + ls.lt)));
+#pragma unroll 1
+        for (int mu = 0; mu < 4; ++mu) {
+            T u[18];
+            load_link(gauge + (size_t)(p * 4 + mu) * gblk, g.Vh, cbg, u);
+            store_link(blk_links + (bid * 8 + p * 4 + mu) * 18 * n, n, i, u);
+        }
+        const T* src = p ? clov_oinv : clov_e;
+#pragma unroll 1
+        for (int b = 0; b < 2; ++b) {
+            T c[36];
+            load_clover_block<T, true>(src, g.Vh, cbg, b, c);
+            store_clover_block<T>(blk_clov + (bid * 2 + p) * 72 * n, n, i, b, c);
+        }
+    }
+}
+
+template <typename T>
+void launch_sap_reorder(const Geom& g, const SapGeom& sg, const void* gauge, const void* clov_e, const void* clov_oinv,
+                        void* blk_links, void* blk_clov, cudaStream_t st)
+{
+    const int threads = (sg.Vbh + 31) / 32 * 32;
+    const int grid = sg.nb[0] * sg.nb[1] * sg.nb[2] * sg.nb[3];
+    sap_reorder_kernel<T><<<grid, threads, 0, st>>>(g, sg, (const T*)gauge, (const T*)clov_e, (const T*)clov_oinv,
+                                                    (T*)blk_links, (T*)blk_clov);
+}
+template void launch_sap_reorder<float>(const Geom&, const SapGeom&, const void*, const void*, const void*, void*, void*, cudaStream_t);
+template void launch_sap_reorder<double>(const Geom&, const SapGeom&, const void*, const void*, const void*, void*, void*, cudaStream_t);
+
 size_t sap_smem_bytes(const SapGeom& sg, size_t real_bytes)
 {
     return (size_t)(2 * 4 * 18 + 48) * sg.Vbh * real_bytes + (size_t)32 * 3 * sizeof(double);
 }
 
 template <typename T>
-cudaError_t launch_sap_blocks(const Geom& g, const SapGeom& sg, int colour, int m, const void* gauge,
-                              const void* clov_e, const void* clov_oinv, const void* r_e, const void* r_o,
+cudaError_t launch_sap_blocks(const Geom& g, const SapGeom& sg, int colour, int m, const void* blk_links,
+                              const void* blk_clov, const void* r_e, const void* r_o,
                               void* x_e, void* x_o, cudaStream_t st)
 {
     SapArgs<T> a;
     a.g = g; a.sg = sg; a.colour = colour; a.m = m;
-    a.gauge = (const T*)gauge; a.clov_e = (const T*)clov_e; a.clov_oinv = (const T*)clov_oinv;
+    a.blk_links = (const T*)blk_links; a.blk_clov = (const T*)blk_clov;
     a.r_e = (const T*)r_e; a.r_o = (const T*)r_o; a.x_e = (T*)x_e; a.x_o = (T*)x_o;
     const size_t smem = sap_smem_bytes(sg, sizeof(T));
     cudaError_t e = cudaFuncSetAttribute(sap_block_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -302,8 +358,8 @@ cudaError_t launch_sap_blocks(const Geom& g, const SapGeom& sg, int colour, int 
     return cudaSuccess;
 }
 template cudaError_t launch_sap_blocks<float>(const Geom&, const SapGeom&, int, int, const void*, const void*,
-                                              const void*, const void*, const void*, void*, void*, cudaStream_t);
+                                              const void*, const void*, void*, void*, cudaStream_t);
 template cudaError_t launch_sap_blocks<double>(const Geom&, const SapGeom&, int, int, const void*, const void*,
-                                               const void*, const void*, const void*, void*, void*, cudaStream_t);
+                                               const void*, const void*, void*, void*, cudaStream_t);
 
 }  // namespace ddamg
