@@ -50,7 +50,7 @@ BYTES_BR = 1248         # kernel B': kernel B + b_e 96
 FLOP_PER_SITE = 1824    # 1320 (hop) + 504 (2 x 6x6 Hermitian mat-vec), per lattice site
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of kernel B' at config 5, from the
 # ncu --set full capture summarised in profiles/ (None until a capture exists)
-NCU_TRAFFIC_BYTES = {5: 21.274e9, 3: None}     # profiles/r1b_ncu_full_dslash.md
+NCU_TRAFFIC_BYTES = {18: {5: 21.274e9}, 12: {5: 18.073e9}}     # profiles/r1b_ncu_full_dslash.md, profiles/r1d_ncu_full_dslash12.md
 CPU_SAMPLE = dict(L=16, T=32)
 # SAP(n, m) row: the paper's smoother parameters (Tables 1, 2, 6) on 4^4 blocks
 SAP_N, SAP_M, SAP_BLOCK = 3, 4, (4, 4, 4, 4)
@@ -191,7 +191,7 @@ def main():
     ap.add_argument("--rows", default="all", help="'all', 'main' (skip the side measurements) or 'multi_rhs' (main + multi-rhs rows)")
     ap.add_argument("--nrhs", default="2,4,8", help="batch sizes of the multi-rhs rows")
     ap.add_argument("--batch-l2-bytes", type=float, default=None, help="override ddamg option batch_l2_bytes")
-    ap.add_argument("--gauge-recon", type=int, default=18, choices=[18, 12],
+    ap.add_argument("--gauge-recon", type=int, default=12, choices=[18, 12],
                     help="link storage read by the fused hopping kernels: 18 reals, or two-row 12 reals (ddamg option gauge_recon)")
     args = ap.parse_args()
     global BYTES_A, BYTES_B, BYTES_BR
@@ -326,7 +326,7 @@ def main():
     ach_A = BYTES_A * Ve / tA / 1e9
     roofline = {"bound": "hbm", "kernel": "dslash_kernel<float, EPI_RICHARDSON> (kernel B')",
                 "achieved": ach_B, "peak": peak, "unit": "GB/s", "frac": ach_B / peak,
-                "traffic": NCU_TRAFFIC_BYTES.get(cfg) if args.gauge_recon == 18 else None, "peak_source": peak_src,
+                "traffic": NCU_TRAFFIC_BYTES[args.gauge_recon].get(cfg), "peak_source": peak_src,
                 "bytes_per_launch": BYTES_BR * Ve, "avg_launch_ms": tB * 1e3, "launches_timed": nB,
                 "other_kernels": [{"kernel": "dslash_kernel<float, EPI_CLOV_HOP> (kernel A)", "achieved": ach_A,
                                    "frac": ach_A / peak, "bytes_per_launch": BYTES_A * Ve, "avg_launch_ms": tA * 1e3,
@@ -335,6 +335,17 @@ def main():
                                    "frac": (BYTES_A + BYTES_BR) * Ve * NU / (ms_per_step * 1e-3) / 1e9 / peak}}
 
     rows = {"a0_load_gauge_ms": t_a0, "a1_build_clover_ms": t_a1, "input_generation_s": t_gen}
+    if args.rows == "all" and args.gauge_recon == 12:
+        # ---- the same step on full 18-real links (two-pass model 1056 + 1248 B per even site)
+        ctx.set_option("gauge_recon", 18)
+        ks = max(3, min(K, 10))
+        ms18 = timed(step, ks, 3, prep_x) / ks
+        ctx.set_option("gauge_recon", 12)
+        b18 = (BYTES_A + BYTES_BR + 2 * 192) * Ve * NU
+        rows["richardson_links18"] = {"ms_per_step": ms18, "site_sweeps_per_s": job_value(V, NU, world, ms18),
+                                      "GBps_two_pass_model": b18 / (ms18 * 1e-3) / 1e9,
+                                      "frac_of_peak": b18 / (ms18 * 1e-3) / 1e9 / peak,
+                                      "bytes_per_even_site_sweep": BYTES_A + BYTES_BR + 2 * 192}
     if args.rows == "all":
         # ---- Schur apply (BASELINE.json metric: GB/s and GFLOP/s, fp32)
         ks = max(3, min(K, 20))
@@ -383,7 +394,7 @@ def main():
                 "block_kernel_ms": t6 * 1e3, "block_kernel_launches": n6,
                 "residual_kernel_ms": ms5 / max(n5, 1), "residual_kernel_launches": n5,
                 "block_kernel_GFLOPps": flop_blk / t6 / 1e9,
-                "block_kernel_bound": "latency (8 warps/SM; fp32 FMA pipe ~20 % busy, profiles/r1c_ncu_full_sap.md)",
+                "block_kernel_bound": "latency (8 warps/SM; fp32 FMA pipe ~28 % busy, profiles/r1d_ncu_full_sap.md)",
                 "note": "SAP(n=3, m=4), 4^4 blocks, non-zero x0: per iteration and colour one streaming residual "
                         "(2 launches) + one block-solve launch"}
             del xs_e, xs_o
@@ -408,8 +419,9 @@ def main():
                 ms3, n3 = ctx.kernel_time_ms(3, reset=False)
                 ms4, n4 = ctx.kernel_time_ms(4, reset=True)
                 ctx.kernel_timing(False)
-                bA = 192 + 864 / nrhs            # per (site, rhs): x_e neighbours 96 + write 96 + (links 576 + clover 288) / nrhs
-                bB = 384 + 864 / nrhs            # t_o 96 + x_e 96 + b_e 96 + write 96 + (576 + 288) / nrhs
+                lk = 384 if args.gauge_recon == 12 else 576          # 8 links per output site
+                bA = 192 + (lk + 288) / nrhs     # per (site, rhs): x_e neighbours 96 + write 96 + (links + clover 288) / nrhs
+                bB = 384 + (lk + 288) / nrhs     # t_o 96 + x_e 96 + b_e 96 + write 96 + (links + 288) / nrhs
                 tA3, tB4 = ms3 / max(n3, 1) * 1e-3, ms4 / max(n4, 1) * 1e-3
                 rows["multi_rhs_richardson"][str(nrhs)] = {
                     "ms_per_call": ms, "rhs_site_sweeps_per_s": V * NU * nrhs / (ms * 1e-3),
@@ -429,15 +441,48 @@ def main():
     hb.copy_(pool_b[0][0]); hx.copy_(pool_x[0])
     d_b = ctx.half_spinor()
 
-    def e2e_step(i):
-        d_b.copy_(hb, non_blocking=True)
-        x_e.copy_(hx, non_blocking=True)
-        ctx.richardson(d_b, x_e, NU, c["omega"])
-        hout.copy_(x_e, non_blocking=True)
+    # Steps are independent, so the copies of neighbouring steps are pipelined: H2D of step i+1 and
+    # D2H of step i-1 run on two copy streams while step i computes (double-buffered device inputs);
+    # every step still moves its own inputs host->device and its own result device->host.
+    d_b2, d_x2 = [d_b, ctx.half_spinor()], [x_e, ctx.half_spinor()]
+    s_in, s_out = torch.cuda.Stream(device=dev), torch.cuda.Stream(device=dev)
+    main = torch.cuda.current_stream()
+
+    def e2e_run(nsteps):
+        t0, t1 = ev(), ev()
+        t0.record(main)
+        s_in.wait_event(t0)
+        freed = [None, None]
+        last_out = None
+        for i in range(nsteps):
+            k = i & 1
+            with torch.cuda.stream(s_in):
+                if freed[k] is not None:
+                    s_in.wait_event(freed[k])                 # buffer k was read back by step i-2
+                d_b2[k].copy_(hb, non_blocking=True)
+                d_x2[k].copy_(hx, non_blocking=True)
+                e_in = ev(); e_in.record(s_in)
+            main.wait_event(e_in)
+            ctx.richardson(d_b2[k], d_x2[k], NU, c["omega"])
+            e_done = ev(); e_done.record(main)
+            with torch.cuda.stream(s_out):
+                s_out.wait_event(e_done)
+                hout.copy_(d_x2[k], non_blocking=True)
+                freed[k] = ev(); freed[k].record(s_out)
+                last_out = freed[k]
+        main.wait_event(last_out)
+        t1.record(main)
+        return t0, t1
     ke = max(3, min(K, 10))
-    ms_e2e = timed(e2e_step, ke, 2) / ke
+    e2e_run(2)
+    barrier()
+    t0, t1 = e2e_run(ke)
+    barrier()
+    ms_e2e = max_over_ranks(t0.elapsed_time(t1), world, dev) / ke
     e2e = {"value": job_value(V, NU, world, ms_e2e), "unit": "site-sweeps/s", "ms_per_step": ms_e2e,
-           "h2d_bytes_per_step": 2 * ctx.half_bytes, "d2h_bytes_per_step": ctx.half_bytes}
+           "h2d_bytes_per_step": 2 * ctx.half_bytes, "d2h_bytes_per_step": ctx.half_bytes,
+           "note": "through Ddamg.richardson with pinned HOST buffers; per step H2D of b_e and x0, the call, D2H of x^(nu); "
+                   "copies of neighbouring steps overlap the compute (two copy streams, double-buffered inputs)"}
 
     line = {
         "metric": "Richardson sites/s (odd-even Schur Wilson-clover, nu=4)",
