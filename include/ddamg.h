@@ -275,6 +275,14 @@ int ddamg_get_clover(ddamg_ctx* ctx, void* A_nat, void* Ainv_nat);
  *                     on 18-real links.  Results change by rounding only (third rows are
  *                     rebuilt from rounded rows).  Clover build and SAP block solves always
  *                     use the full links.
+ *   "fused_sweep"     0 (default) or 1.  1 = ddamg_apply_schur and every sweep of
+ *                     ddamg_richardson run kernel A and kernel B / B' as ONE launch, pipelined
+ *                     time slice by time slice (SURVEY.md 8(d) "A->B slab pipelining in L2").
+ *                     Bit-identical results.  Used only when a time slice (L^3/2 sites) is a
+ *                     multiple of 128 sites, else the two-launch path runs.  Measured slower
+ *                     than two launches on B200 at 32^3x64 .. 64^3x128.
+ *   "sweep_lag"       1..64 (default 2): time slices kernel A runs ahead of kernel B in the
+ *                     fused sweep.
  * EINVAL for an unknown name or a bad value.
  */
 int ddamg_set_option(ddamg_ctx* ctx, const char* name, double value);

@@ -40,6 +40,9 @@ struct ddamg_ctx {
     double* partials_batch;     // multi-rhs reduction scratch
     int batch_cap;
     double batch_l2_bytes;      // L2 budget of the z-chunked multi-rhs traversal (option "batch_l2_bytes")
+    unsigned int* sweep_sync;   // fused sweep: ticket + per-slice counters (T + 1 words)
+    int fused_sweep;            // option "fused_sweep": Schur apply / Richardson sweep as one pipelined launch
+    int sweep_lag;              // option "sweep_lag": slices kernel A runs ahead of kernel B
     void* sap_links;            // SAP: block-ordered copy of the links (launch_sap_reorder), or NULL
     void* sap_clov;             // SAP: block-ordered copy of A_ee / A_oo^-1
     int sap_built[4];           // block extents the two copies were built for ({0,..} = stale)
@@ -182,6 +185,7 @@ extern "C" int ddamg_create(ddamg_ctx** out, int L, int T, double csw, double m0
     ctx->tmp_batch = nullptr; ctx->partials_batch = nullptr; ctx->batch_cap = 0; ctx->batch_l2_bytes = 40e6;
     for (int mu = 0; mu < 4; ++mu) ctx->sap_block[mu] = 4;
     ctx->sap_links = ctx->sap_clov = nullptr;
+    ctx->sweep_sync = nullptr; ctx->fused_sweep = 0; ctx->sweep_lag = 2;
     for (int mu = 0; mu < 4; ++mu) ctx->sap_built[mu] = 0;
     ctx->partials = nullptr; ctx->sc = nullptr; ctx->host_hist = nullptr; ctx->singular = nullptr;
     ctx->have_gauge = ctx->have_clover = ctx->have_clov_oo = false;
@@ -201,6 +205,7 @@ extern "C" int ddamg_create(ddamg_ctx** out, int L, int T, double csw, double m0
     if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->partials, ctx->partials_len * sizeof(double));
     if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->sc, sizeof(Scalars));
     if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->singular, sizeof(int));
+    if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->sweep_sync, sizeof(unsigned int) * (size_t)(T + 1));
     if (e == cudaSuccess) e = cudaMallocHost((void**)&ctx->host_hist, sizeof(double) * (HIST_MAX + 8));
     if (e == cudaSuccess) e = cudaMemsetAsync(ctx->sc, 0, sizeof(Scalars), ctx->stream);
     if (e != cudaSuccess) {
@@ -220,7 +225,7 @@ extern "C" int ddamg_destroy(ddamg_ctx* ctx)
     cudaStreamSynchronize(ctx->stream);
     for (auto& ev : ctx->events) { cudaEventDestroy(ev.a); cudaEventDestroy(ev.b); }
     cudaFree(ctx->gauge12); cudaFree(ctx->recon_dev);
-    cudaFree(ctx->sap_links); cudaFree(ctx->sap_clov);
+    cudaFree(ctx->sap_links); cudaFree(ctx->sap_clov); cudaFree(ctx->sweep_sync);
     cudaFree(ctx->gauge); cudaFree(ctx->clov[0]); cudaFree(ctx->clov[1]);
     cudaFree(ctx->tmp_o); cudaFree(ctx->tmp_e); cudaFree(ctx->krylov);
     cudaFree(ctx->tmp_batch); cudaFree(ctx->partials_batch);
@@ -353,9 +358,34 @@ static int need_ready(ddamg_ctx* ctx, const char* who)
     return DDAMG_OK;
 }
 
+// Kernel A and kernel B / B' / residual as ONE pipelined launch (option "fused_sweep").
+static bool use_fused(ddamg_ctx* ctx) { return ctx->fused_sweep && sweep_eligible(ctx->g); }
+
+static int fused(ddamg_ctx* ctx, int epi_b, bool norm, const void* x_e, const void* rhs, void* out, double omega)
+{
+    ddamg_ctx::Ev ev;
+    if (ctx->timing) {
+        if (cudaEventCreate(&ev.a) != cudaSuccess || cudaEventCreate(&ev.b) != cudaSuccess)
+            return check_cuda(ctx, cudaGetLastError(), "cudaEventCreate");
+        ev.which = 7;
+        cudaEventRecord(ev.a, ctx->stream);
+    }
+    cudaError_t e = ctx->prec == DDAMG_F32
+        ? launch_sweep<float>(ctx->g, epi_b, norm, x_e, ctx->tmp_o, hop_gauge_block(ctx, 0), hop_gauge_block(ctx, 1),
+                              ctx->clov[0], ctx->clov[1], rhs, out, omega, ctx->partials, ctx->sweep_sync,
+                              ctx->sweep_lag, ctx->recon, ctx->bc == 1, ctx->stream)
+        : launch_sweep<double>(ctx->g, epi_b, norm, x_e, ctx->tmp_o, hop_gauge_block(ctx, 0), hop_gauge_block(ctx, 1),
+                               ctx->clov[0], ctx->clov[1], rhs, out, omega, ctx->partials, ctx->sweep_sync,
+                               ctx->sweep_lag, ctx->recon, ctx->bc == 1, ctx->stream);
+    if (e != cudaSuccess) return check_cuda(ctx, e, "fused sweep memset");
+    if (ctx->timing) { cudaEventRecord(ev.b, ctx->stream); ctx->events.push_back(ev); }
+    return after_launch(ctx);
+}
+
 // y_e = D_S x_e  (kernel A then kernel B)
 static int schur(ddamg_ctx* ctx, const void* x_e, void* y_e)
 {
+    if (use_fused(ctx)) return fused(ctx, EPI_SCHUR, false, x_e, nullptr, y_e, 0.0);
     int s = dslash(ctx, EPI_CLOV_HOP, false, 1, x_e, nullptr, nullptr, ctx->tmp_o, 0.0, 0);
     if (s != DDAMG_OK) return s;
     return dslash(ctx, EPI_SCHUR, false, 0, ctx->tmp_o, x_e, nullptr, y_e, 0.0, 1);
@@ -416,11 +446,17 @@ extern "C" int ddamg_richardson(ddamg_ctx* ctx, const void* b_e, void* x_e, int 
     } else if (zero_init) {
         CK(cudaMemsetAsync(x_e, 0, ctx->half_bytes, ctx->stream));
     }
+    const bool one_launch = use_fused(ctx);
     for (int i = done; i < nu; ++i) {
-        s = dslash(ctx, EPI_CLOV_HOP, false, 1, x_e, nullptr, nullptr, ctx->tmp_o, 0.0, 0);        // kernel A
-        if (s != DDAMG_OK) return s;
-        s = dslash(ctx, EPI_RICHARDSON, hist, 0, ctx->tmp_o, x_e, b_e, x_e, omega, 1);              // kernel B'
-        if (s != DDAMG_OK) return s;
+        if (one_launch) {
+            s = fused(ctx, EPI_RICHARDSON, hist, x_e, b_e, x_e, omega);                                // A and B' pipelined
+            if (s != DDAMG_OK) return s;
+        } else {
+            s = dslash(ctx, EPI_CLOV_HOP, false, 1, x_e, nullptr, nullptr, ctx->tmp_o, 0.0, 0);        // kernel A
+            if (s != DDAMG_OK) return s;
+            s = dslash(ctx, EPI_RICHARDSON, hist, 0, ctx->tmp_o, x_e, b_e, x_e, omega, 1);              // kernel B'
+            if (s != DDAMG_OK) return s;
+        }
         if (hist) {
             launch_finalize_norm(ctx->partials, dslash_grid(ctx->g), ctx->sc, 1, ctx->stream);
             s = after_launch(ctx);
@@ -1178,6 +1214,17 @@ extern "C" int ddamg_set_option(ddamg_ctx* ctx, const char* name, double value)
     if (strcmp(name, "batch_l2_bytes") == 0) {
         if (!(value >= 0.0)) return fail(ctx, DDAMG_EINVAL, "ddamg_set_option: batch_l2_bytes must be >= 0");
         ctx->batch_l2_bytes = value;
+        return DDAMG_OK;
+    }
+    if (strcmp(name, "fused_sweep") == 0) {
+        if (value != 0.0 && value != 1.0) return fail(ctx, DDAMG_EINVAL, "ddamg_set_option: fused_sweep must be 0 or 1");
+        ctx->fused_sweep = (int)value;
+        return DDAMG_OK;
+    }
+    if (strcmp(name, "sweep_lag") == 0) {
+        const int lag = (int)value;
+        if ((double)lag != value || lag < 1 || lag > 64) return fail(ctx, DDAMG_EINVAL, "ddamg_set_option: sweep_lag must be an integer in 1..64");
+        ctx->sweep_lag = lag;
         return DDAMG_OK;
     }
     if (strcmp(name, "gauge_recon") == 0) {
