@@ -29,8 +29,11 @@ _lib = None
 def lib() -> ctypes.CDLL:
     global _lib
     if _lib is None:
-        _build()
-        _lib = ctypes.CDLL(_LIB)
+        path = os.environ.get("ORACLE_LIB")          # a sanitizer build (tests/test_oracle_sanitizers.py)
+        if not path:
+            _build()
+            path = _LIB
+        _lib = ctypes.CDLL(path)
         _lib.oracle_invert_sites.restype = ctypes.c_long
     return _lib
 

@@ -24,5 +24,18 @@ def build(force: bool = False) -> str:
     return LIB
 
 
+def build_sanitized() -> str:
+    """The same source under AddressSanitizer + UndefinedBehaviorSanitizer (no OpenMP, -O1): used by
+    tests/test_oracle_sanitizers.py in a subprocess with libasan preloaded (ORACLE_LIB selects it)."""
+    out = os.path.join(HERE, "liboracle_asan.so")
+    if os.path.exists(out) and os.path.getmtime(out) >= os.path.getmtime(SRC):
+        return out
+    cmd = ["gcc", "-O1", "-g", "-std=c11", "-fPIC", "-shared", "-Wall", "-Wextra", "-fno-omit-frame-pointer",
+           "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined", "-Wno-unknown-pragmas",
+           "-o", out, SRC, "-lm"]
+    subprocess.run(cmd, check=True)
+    return out
+
+
 if __name__ == "__main__":
     print(build(force=True))
