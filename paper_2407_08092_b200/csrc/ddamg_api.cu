@@ -9,6 +9,8 @@
 #include <string>
 #include <vector>
 
+#include <nvtx3/nvToolsExt.h>
+
 #include "../../include/ddamg.h"
 #include "ddamg_internal.h"
 
@@ -87,7 +89,15 @@ static int check_cuda(ddamg_ctx* c, cudaError_t e, const char* what)
         if (_s != DDAMG_OK) return _s;                               \
     } while (0)
 
+// NVTX range per API call (tracing): visible to ncu --nvtx / any NVTX-aware
+// profiler, a no-op costing a few ns without one.
+struct NvtxRange {
+    explicit NvtxRange(const char* name) { nvtxRangePushA(name); }
+    ~NvtxRange() { nvtxRangePop(); }
+};
+
 #define ENTER(ctx)                                                           \
+    NvtxRange nvtx_range_(__func__);                                         \
     do {                                                                     \
         if (!(ctx)) return DDAMG_EINVAL;                                     \
         if ((ctx)->sticky != DDAMG_OK) return (ctx)->sticky;                 \
