@@ -52,13 +52,16 @@ __device__ __forceinline__ double block_sum(double v)
 #ifndef DDAMG_MAXREG_B
 #define DDAMG_MAXREG_B 128
 #endif
+#ifndef DDAMG_MAXREG_BATCH
+#define DDAMG_MAXREG_BATCH 128     // multi-rhs kernels
+#endif
 
 // BATCH (multi-rhs): one thread per (site, rhs), rhs fastest, so that the
 // nrhs threads of a site share every link / clover vector they load while all spinor planes
 // stay contiguous per warp (vector index cb * nrhs + r).
 template <typename T, int EPI, bool NORM, bool BATCH, int RECON>
 __global__ void __launch_bounds__(DSLASH_THREADS)
-__maxnreg__(sizeof(T) == 4 ? (EPI <= EPI_RHS_MINUS_HOP ? DDAMG_MAXREG_A : DDAMG_MAXREG_B) : 255)
+__maxnreg__(sizeof(T) == 4 ? (BATCH ? DDAMG_MAXREG_BATCH : EPI <= EPI_RHS_MINUS_HOP ? DDAMG_MAXREG_A : DDAMG_MAXREG_B) : 255)
 dslash_kernel(const DslashArgs<T> a)
 {
     // BATCH: with nrhs spinors per site one time slice of neighbour spinors no longer fits L2
