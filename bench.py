@@ -180,6 +180,61 @@ def run_reference(args):
 
 
 # --------------------------------------------------------------------------- our arm
+def paper_context_row(torch, gen, Ddamg, F32, dev, recon):
+    """One smoother call each of odd-even Richardson(12, 1.5), odd-even GMRES(3, 4) and SAP(3, 4) at 48^3 x 96."""
+    c = CONFIGS[4]
+    L, T = c["L"], c["T"]
+    ctx = Ddamg(L, T, c["csw"], c["m0"], c["bc"], F32, stream=None, device=dev)
+    U = gen.gauge_field(L, T, 1004, c["eps"], c["reunit"], device=dev, dtype=torch.complex64)
+    ctx.load_gauge(U)
+    ctx.build_clover()
+    del U
+    if recon == 12:
+        ctx.set_option("gauge_recon", 12)
+    b_e, b_o = ctx.pack(gen.spinor_field(L, T, 2004, device=dev, dtype=torch.complex64))
+    v = b_e.clone()
+    lam = ctx.power_iteration(v, 10)              # Alg. 4 line 1: omega = delta / |lambda_max|, delta = 1.5
+    omega = 1.5 / lam
+    bhat, x_e, x_o = ctx.half_spinor(), ctx.half_spinor(), ctx.half_spinor()
+
+    def timed_call(fn, n=5):
+        for _ in range(2):
+            fn()
+        torch.cuda.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        for _ in range(n):
+            fn()
+        b.record()
+        torch.cuda.synchronize()
+        return a.elapsed_time(b) / n
+
+    def rich():
+        ctx.prepare_rhs(b_e, b_o, bhat)
+        ctx.richardson(bhat, x_e, 12, omega, zero_init=True)
+        ctx.reconstruct_odd(b_o, x_e, x_o)
+
+    def gm():
+        ctx.prepare_rhs(b_e, b_o, bhat)
+        ctx.gmres_oe(bhat, x_e, 4, 3, zero_init=True)
+        ctx.reconstruct_odd(b_o, x_e, x_o)
+
+    def sap():
+        ctx.sap(b_e, b_o, x_e, x_o, 3, 4, block=(4, 4, 4, 4), zero_init=True)
+
+    out = {"lattice": "48^3x96 (the paper's 96x48^3 shape), synthetic links, fp32, one B200",
+           "omega_power_iteration": omega,
+           "odd_even_richardson_12_ms": timed_call(rich), "odd_even_gmres_3x4_ms": timed_call(gm),
+           "sap_3x4_ms": timed_call(sap),
+           "paper_gpu_ms": {"odd_even_richardson": 360.0, "odd_even_gmres_3x4": 450.0, "sap_3x4": 330.0},
+           "paper_cpu_ms": {"odd_even_richardson": 4800.0, "odd_even_gmres_3x4": 5660.0, "sap_3x4": 4390.0},
+           "paper_hardware": "Table 2, PAPER.md:258-262: 4 ORISE nodes, 16 GPUs (64 SMs, 16 GB HBM2, HIP, host-staged halos) "
+                             "/ 16 MPI ranks x 4 OpenMP threads on 32-core x86; CLQCD configuration at m_s; precision not stated; "
+                             "another machine and a thermalised configuration: context, not a target"}
+    ctx.close()
+    return out
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -433,6 +488,15 @@ def main():
                 torch.cuda.empty_cache()
             except Exception as e:
                 rows["multi_rhs_richardson"][str(nrhs)] = {"error": str(e)}
+
+    if args.rows == "all" and rank == 0 and world == 1:
+        # ---- context row: the paper's three smoother configurations (Table 2) on the
+        # paper's lattice SHAPE 48^3 x 96 (synthetic links, fp32; the paper: CLQCD configuration, 16 GPUs
+        # of 64 SMs / 16 GB HBM2 on 4 ORISE nodes, 32-core x86 hosts, precision not stated).  Context only.
+        try:
+            rows["paper_smoother_calls_48x96"] = paper_context_row(torch, gen, Ddamg, F32, dev, args.gauge_recon)
+        except Exception as exc:                  # noqa: BLE001 - a side row must not lose the headline
+            rows["paper_smoother_calls_48x96"] = {"error": str(exc)[:200]}
 
     # ---- e2e: HOST buffers, copies inside the timed region, through the public API
     hb = torch.empty_like(pool_b[0][0], device="cpu").pin_memory()
