@@ -622,9 +622,13 @@ static int gmres_impl(ddamg_ctx* ctx, const void* b_e, void* x_e, int k, int cyc
     const int dgrid = dslash_grid(ctx->g);
     char* V = (char*)ctx->krylov;
     auto Vj = [&](int j) { return (void*)(V + (size_t)j * ctx->half_bytes); };
-    double* coef_y = (double*)((char*)ctx->sc + offsetof(Scalars, y));
+    // The basis is kept lazily normalised: slot i holds an un-normalised vector and the device
+    // scalar vs[i] its factor, v_i = vs[i] * stored_i.  The normalisation pass v_{j+1} = w / h_{j+1,j}
+    // (one read and one write of a half spinor per Arnoldi step) disappears: its factor goes into the
+    // dot products, the axpy coefficients and the final x += V y instead (scalar work only).
+    double* coef_ys = (double*)((char*)ctx->sc + offsetof(Scalars, ys));
     double* coef_negh = (double*)((char*)ctx->sc + offsetof(Scalars, negh));
-    double* scale = (double*)((char*)ctx->sc + offsetof(Scalars, scale));
+    double* vs = (double*)((char*)ctx->sc + offsetof(Scalars, vs));
     int s = reset_hist(ctx);
     if (s != DDAMG_OK) return s;
     double bnorm = 0.0;
@@ -650,9 +654,8 @@ static int gmres_impl(ddamg_ctx* ctx, const void* b_e, void* x_e, int k, int cyc
             if (s != DDAMG_OK) return s;
             launch_finalize_norm(ctx->partials, dgrid, ctx->sc, 1, st);
         }
-        launch_gmres_begin_cycle(ctx->sc, st);
-        launch_scale_by_dev<T>(nreal, Vj(0), scale, st);                 // v_1 = r / beta
-        s = after_launch(ctx, 3); if (s != DDAMG_OK) return s;
+        launch_gmres_begin_cycle(ctx->sc, st);                           // v_1 = r / beta as (vs[0] = 1 / beta, r)
+        s = after_launch(ctx, 2); if (s != DDAMG_OK) return s;
         if (tol > 0.0) {
             double beta = 0.0;
             CK(cudaMemcpyAsync(&beta, (char*)ctx->sc + offsetof(Scalars, value), sizeof(double), cudaMemcpyDeviceToHost, st));
@@ -661,27 +664,27 @@ static int gmres_impl(ddamg_ctx* ctx, const void* b_e, void* x_e, int k, int cyc
         }
         int m = 0;
         for (int j = 0; j < k; ++j) {
-            // line 5: w = D_S v_j  -> V[j+1]
+            // line 5: w = D_S v_j = vs[j] * D_S stored_j;  D_S stored_j -> V[j+1]
             s = schur(ctx, Vj(j), Vj(j + 1));
             if (s != DDAMG_OK) return s;
             // lines 6-7 (fused classical Gram-Schmidt): h_ij = <v_i, w>, i = 0..j
             for (int i0 = 0; i0 <= j; i0 += MDOT_NB) {
                 const int nb = (j + 1 - i0) < MDOT_NB ? (j + 1 - i0) : MDOT_NB;
                 launch_multi_dot<T>(nreal, nb, Vj(i0), nreal, Vj(j + 1), ctx->partials, st);
-                launch_finalize_dots(ctx->partials, bgrid, nb, ctx->sc, i0, st);
+                launch_finalize_dots_lazy(ctx->partials, bgrid, nb, ctx->sc, i0, j, st);
                 s = after_launch(ctx, 2); if (s != DDAMG_OK) return s;
             }
-            // w -= sum_i h_ij v_i ; line 8: h_{j+1,j} = ||w||
+            // w = vs[j] V[j+1] - sum_i h_ij vs[i] stored_i ; line 8: h_{j+1,j} = ||w||
             for (int i0 = 0; i0 <= j; i0 += MDOT_NB) {
                 const int nb = (j + 1 - i0) < MDOT_NB ? (j + 1 - i0) : MDOT_NB;
                 const bool last = i0 + MDOT_NB > j;
-                launch_multi_axpy<T>(nreal, nb, Vj(i0), nreal, coef_negh + 2 * i0, Vj(j + 1), last ? ctx->partials : nullptr, st);
+                launch_multi_axpy<T>(nreal, nb, Vj(i0), nreal, coef_negh + 2 * i0, Vj(j + 1), last ? ctx->partials : nullptr, st,
+                                     i0 == 0 ? vs + j : nullptr);
                 s = after_launch(ctx); if (s != DDAMG_OK) return s;
             }
             launch_finalize_norm(ctx->partials, bgrid, ctx->sc, 0, st);
-            launch_gmres_givens(ctx->sc, j, st);
-            launch_scale_by_dev<T>(nreal, Vj(j + 1), scale, st);         // v_{j+1} = w / h_{j+1,j}
-            s = after_launch(ctx, 3); if (s != DDAMG_OK) return s;
+            launch_gmres_givens(ctx->sc, j, st);                         // also vs[j+1] = 1 / h_{j+1,j}
+            s = after_launch(ctx, 2); if (s != DDAMG_OK) return s;
             m = j + 1;
             if (tol > 0.0) {
                 int nh = 0;
@@ -698,7 +701,7 @@ static int gmres_impl(ddamg_ctx* ctx, const void* b_e, void* x_e, int k, int cyc
         s = after_launch(ctx); if (s != DDAMG_OK) return s;
         for (int i0 = 0; i0 < m; i0 += MDOT_NB) {
             const int nb = (m - i0) < MDOT_NB ? (m - i0) : MDOT_NB;
-            launch_multi_axpy<T>(nreal, nb, Vj(i0), nreal, coef_y + 2 * i0, x_e, nullptr, st);
+            launch_multi_axpy<T>(nreal, nb, Vj(i0), nreal, coef_ys + 2 * i0, x_e, nullptr, st);
             s = after_launch(ctx); if (s != DDAMG_OK) return s;
         }
     }

@@ -208,21 +208,50 @@ void launch_finalize_dots(const double* partials, int nblocks, int nb, Scalars* 
     finalize_dots_kernel<<<1, 32 * 2 * MDOT_NB, 0, st>>>(partials, nblocks, nb, sc, first);
 }
 
+// GMRES with a lazily normalised basis (v_i = vs[i] * stored_i, DESIGN.md section 7 "GMRES"):
+// the raw sums are <stored_i, D_S stored_j>, so  h_ij = vs[i] vs[j] sum  and the coefficient of
+// stored_i in  w~ = vs[j] D_S stored_j - sum_i h_ij vs[i] stored_i  is  negh_i = -h_ij vs[i].
+__global__ void finalize_dots_lazy_kernel(const double* __restrict__ partials, int nblocks, int nb, Scalars* sc,
+                                          int first, int j)
+{
+    const int c = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (c < 2 * nb) {
+        double s = 0;
+        for (int b = lane; b < nblocks; b += 32) s += partials[(size_t)b * 2 * nb + c];
+        s = warp_sum(s);
+        if (lane == 0) {
+            const double si = sc->vs[first + (c >> 1)];
+            const double h = s * si * sc->vs[j];
+            sc->hcol[2 * first + c] = h;
+            sc->negh[2 * first + c] = -h * si;
+        }
+    }
+}
+void launch_finalize_dots_lazy(const double* partials, int nblocks, int nb, Scalars* sc, int first, int j, cudaStream_t st)
+{
+    finalize_dots_lazy_kernel<<<1, 32 * 2 * MDOT_NB, 0, st>>>(partials, nblocks, nb, sc, first, j);
+}
+
 // ------------------------------------------------------------------ w += sum_i coef_i v_i  (+ |w|^2)
 template <typename T, int NB>
 __global__ void __launch_bounds__(BLAS_THREADS)
 multi_axpy_kernel(size_t nvec, const typename VecOf<T>::type* __restrict__ V0, size_t vstride,
                   const double* __restrict__ coef, typename VecOf<T>::type* __restrict__ w,
-                  double* __restrict__ partials)
+                  double* __restrict__ partials, const double* __restrict__ wscale)
 {
     constexpr int N = VecOf<T>::N;
     double cr[NB], ci[NB];
 #pragma unroll
     for (int b = 0; b < NB; ++b) { cr[b] = coef[2 * b]; ci[b] = coef[2 * b + 1]; }
+    const double ws = wscale ? *wscale : 1.0;        // w <- ws * w + sum_i coef_i v_i
     double acc[1] = { 0.0 };
     for (size_t i = (size_t)blockIdx.x * BLAS_THREADS + threadIdx.x; i < nvec; i += (size_t)gridDim.x * BLAS_THREADS) {
         double wr[N];
         cvt(w[i], wr);
+        if (wscale) {
+#pragma unroll
+            for (int c = 0; c < N; ++c) wr[c] *= ws;
+        }
 #pragma unroll
         for (int b = 0; b < NB; ++b) {
             double vr[N];
@@ -242,17 +271,17 @@ multi_axpy_kernel(size_t nvec, const typename VecOf<T>::type* __restrict__ V0, s
 }
 template <typename T>
 void launch_multi_axpy(size_t nreal, int nb, const void* V, size_t vstride_real, const double* coef, void* w,
-                       double* partials, cudaStream_t st)
+                       double* partials, cudaStream_t st, const double* wscale)
 {
     using VT = typename VecOf<T>::type;
     const size_t nvec = nreal / VecOf<T>::N, vs = vstride_real / VecOf<T>::N;
     const int grid = blas_grid(nvec);
-#define MA(NB) case NB: multi_axpy_kernel<T, NB><<<grid, BLAS_THREADS, 0, st>>>(nvec, (const VT*)V, vs, coef, (VT*)w, partials); break;
+#define MA(NB) case NB: multi_axpy_kernel<T, NB><<<grid, BLAS_THREADS, 0, st>>>(nvec, (const VT*)V, vs, coef, (VT*)w, partials, wscale); break;
     switch (nb) { MA(1) MA(2) MA(3) MA(4) MA(5) MA(6) MA(7) MA(8) MA(9) MA(10) MA(11) MA(12) }
 #undef MA
 }
-template void launch_multi_axpy<float>(size_t, int, const void*, size_t, const double*, void*, double*, cudaStream_t);
-template void launch_multi_axpy<double>(size_t, int, const void*, size_t, const double*, void*, double*, cudaStream_t);
+template void launch_multi_axpy<float>(size_t, int, const void*, size_t, const double*, void*, double*, cudaStream_t, const double*);
+template void launch_multi_axpy<double>(size_t, int, const void*, size_t, const double*, void*, double*, cudaStream_t, const double*);
 
 // ------------------------------------------------------------------ GCR (Alg. 3)
 // lines 11-14 in one pass:  z = w + sum_j beta_j z_j  (in place on w),  p = r + sum_j beta_j p_j,
@@ -403,6 +432,7 @@ __global__ void gmres_begin_cycle_kernel(Scalars* sc)
 {
     for (int i = 0; i < 2 * (GMRES_KMAX + 1); ++i) sc->gvec[i] = 0.0;
     sc->gvec[0] = sc->value;          // beta e_1
+    sc->vs[0] = sc->scale;            // v_1 = r / beta, kept as (1 / beta, r)
 }
 void launch_gmres_begin_cycle(Scalars* sc, cudaStream_t st) { gmres_begin_cycle_kernel<<<1, 1, 0, st>>>(sc); }
 
@@ -415,6 +445,7 @@ __global__ void gmres_givens_kernel(Scalars* sc, int j)
     for (int i = 0; i <= j; ++i) { H[2 * i] = sc->hcol[2 * i]; H[2 * i + 1] = sc->hcol[2 * i + 1]; }
     H[2 * (j + 1)] = sc->value;
     H[2 * (j + 1) + 1] = 0.0;
+    sc->vs[j + 1] = sc->scale;        // v_{j+1} = w / h_{j+1,j}, kept as (1 / h_{j+1,j}, w)
     for (int i = 0; i < j; ++i) {
         const double cr = sc->cs[2 * i], ci = sc->cs[2 * i + 1], sr = sc->sn[2 * i], si = sc->sn[2 * i + 1];
         const double ar = H[2 * i], ai = H[2 * i + 1], br = H[2 * i + 2], bi = H[2 * i + 3];
@@ -457,6 +488,8 @@ __global__ void gmres_solve_kernel(Scalars* sc, int m)
         const double den = d[0] * d[0] + d[1] * d[1];
         sc->y[2 * i] = den > 0 ? (sr * d[0] + si * d[1]) / den : 0.0;
         sc->y[2 * i + 1] = den > 0 ? (si * d[0] - sr * d[1]) / den : 0.0;
+        sc->ys[2 * i] = sc->y[2 * i] * sc->vs[i];            // x += sum_i y_i vs[i] stored_i
+        sc->ys[2 * i + 1] = sc->y[2 * i + 1] * sc->vs[i];
     }
 }
 void launch_gmres_solve(Scalars* sc, int m, cudaStream_t st) { gmres_solve_kernel<<<1, 1, 0, st>>>(sc, m); }

@@ -96,6 +96,8 @@ struct Scalars {
     double cs[GMRES_KMAX * 2], sn[GMRES_KMAX * 2];      // Givens rotations
     double gvec[(GMRES_KMAX + 1) * 2];                  // rotated beta e_1
     double y[GMRES_KMAX * 2];                           // least-squares solution
+    double ys[GMRES_KMAX * 2];                          // y_i * vs[i]: coefficients of the stored basis vectors
+    double vs[GMRES_KMAX + 1];                          // GMRES: v_i = vs[i] * stored_i (lazy normalisation)
     double hcol[(GMRES_KMAX + 1) * 2];                  // current column h_{1..j,j}
     double negh[(GMRES_KMAX + 1) * 2];                  // -hcol (axpy coefficients)
     double delta[GMRES_KMAX];                           // GCR: delta_j = (z_j, z_j)
@@ -120,10 +122,12 @@ template <typename T>
 void launch_multi_dot(size_t nreal, int nb, const void* V, size_t vstride_real, const void* w, double* partials,
                       cudaStream_t st);
 void launch_finalize_dots(const double* partials, int nblocks, int nb, Scalars* sc, int first, cudaStream_t st);
-// w += sum_i coef[i] v_i (complex coef on device, nb <= MDOT_NB); optional |w|^2 partials
+void launch_finalize_dots_lazy(const double* partials, int nblocks, int nb, Scalars* sc, int first, int j, cudaStream_t st);
+// w <- (*wscale) w + sum_i coef[i] v_i (complex coef and real wscale on device, nb <= MDOT_NB;
+// wscale NULL = 1); optional |w|^2 partials
 template <typename T>
 void launch_multi_axpy(size_t nreal, int nb, const void* V, size_t vstride_real, const double* coef, void* w,
-                       double* partials, cudaStream_t st);
+                       double* partials, cudaStream_t st, const double* wscale = nullptr);
 // GCR (Alg. 3)
 template <typename T>
 void launch_gcr_form(size_t nreal, int nb, const void* Z0, const void* P0, size_t vstride_real, const double* coef,
