@@ -189,11 +189,14 @@ int ddamg_fgmres(ddamg_ctx* ctx, const void* b_e, const void* b_o, void* x_e, vo
  *   block      HOST array of 4 ints; each even, dividing L (L, L, T) with an EVEN quotient, at
  *              most 512 sites per block, links of one block must fit in shared memory
  *              (fp32: up to 512 sites, fp64: up to 256 sites) -- else EINVAL
- *   x_e, x_o   in: x^(0) (ignored if zero_init != 0); out: x^(n).  In place.
+ *   x_e, x_o   in: x^(0) (ignored if zero_init != 0); out: x^(n).  In place.  With zero_init and
+ *              res_hist == NULL the first residual is b itself (b - D 0) and is not computed.
  *   res_hist   HOST array of n+1 doubles or NULL: ||b - D x^(i)||_2 for i = 0..n (the first n
  *              are the residuals of line 2; the last costs one extra residual).  NULL skips
  *              the reductions and the stream synchronisation.
- * m = 0 leaves x unchanged.  Builds and keeps A_oo on first use (as ddamg_apply_full).
+ * m = 0 leaves x unchanged.  Builds and keeps A_oo on first use (as ddamg_apply_full), and
+ * block-ordered copies of the links and of A_ee / A_oo^-1 for the block geometry last used
+ * (2 x the size of the gauge field; rebuilt when the geometry, the links or the clover change).
  */
 int ddamg_sap(ddamg_ctx* ctx, const void* b_e, const void* b_o, void* x_e, void* x_o, int n, int m,
               const int* block, int zero_init, double* res_hist);

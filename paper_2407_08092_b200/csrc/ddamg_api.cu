@@ -1156,7 +1156,7 @@ extern "C" int ddamg_sap(ddamg_ctx* ctx, const void* b_e, const void* b_o, void*
         if (norm) { launch_finalize_norm(ctx->partials, 2 * dgrid, ctx->sc, 1, st); q = after_launch(ctx); }
         return q;
     };
-    auto blocks = [&](int colour) -> int {
+    auto blocks = [&](int colour, const void* r_e, const void* r_o) -> int {
         if (m == 0) return DDAMG_OK;                       // zero Minimal Residual iterations: e_k = 0
         ddamg_ctx::Ev ev;
         if (ctx->timing) {
@@ -1166,17 +1166,23 @@ extern "C" int ddamg_sap(ddamg_ctx* ctx, const void* b_e, const void* b_o, void*
             cudaEventRecord(ev.a, st);
         }
         cudaError_t e = f32
-            ? launch_sap_blocks<float>(ctx->g, sg, colour, m, ctx->sap_links, ctx->sap_clov, ctx->tmp_e, ctx->tmp_o, x_e, x_o, st)
-            : launch_sap_blocks<double>(ctx->g, sg, colour, m, ctx->sap_links, ctx->sap_clov, ctx->tmp_e, ctx->tmp_o, x_e, x_o, st);
+            ? launch_sap_blocks<float>(ctx->g, sg, colour, m, ctx->sap_links, ctx->sap_clov, r_e, r_o, x_e, x_o, st)
+            : launch_sap_blocks<double>(ctx->g, sg, colour, m, ctx->sap_links, ctx->sap_clov, r_e, r_o, x_e, x_o, st);
         if (e != cudaSuccess) return check_cuda(ctx, e, "sap_block_kernel attributes");
         if (ctx->timing) { cudaEventRecord(ev.b, st); ctx->events.push_back(ev); }
         return after_launch(ctx);
     };
     for (int i = 0; i < n; ++i) {
-        s = residual(hist); if (s != DDAMG_OK) return s;             // line 2
-        s = blocks(0); if (s != DDAMG_OK) return s;                  // lines 4-6: red blocks
+        if (i == 0 && zero_init && !hist) {
+            // line 2 with x = 0: r = b - D 0 = b exactly, so the red blocks read b itself (the smoother
+            // use: one residual evaluation of 2n saved)
+            s = blocks(0, b_e, b_o); if (s != DDAMG_OK) return s;
+        } else {
+            s = residual(hist); if (s != DDAMG_OK) return s;         // line 2
+            s = blocks(0, ctx->tmp_e, ctx->tmp_o); if (s != DDAMG_OK) return s;   // lines 4-6: red blocks
+        }
         s = residual(false); if (s != DDAMG_OK) return s;            // line 7
-        s = blocks(1); if (s != DDAMG_OK) return s;                  // lines 8-10: black blocks
+        s = blocks(1, ctx->tmp_e, ctx->tmp_o); if (s != DDAMG_OK) return s;       // lines 8-10: black blocks
     }
     if (hist) {
         s = residual(true); if (s != DDAMG_OK) return s;             // final true residual
