@@ -180,6 +180,39 @@ def run_reference(args):
 
 
 # --------------------------------------------------------------------------- our arm
+def f64_apply_row(torch, gen, Ddamg, dev):
+    """fp64 Schur apply at 48^3 x 96 (config 4 recipe, 18-real links): the precision of BASELINE.json's
+    fp64 parity bar, timed against the two-pass byte model at 8 bytes per real (4416 B per even site)."""
+    from paper_2407_08092_b200 import F64
+    c = CONFIGS[4]
+    L, T = c["L"], c["T"]
+    ctx = Ddamg(L, T, c["csw"], c["m0"], c["bc"], F64, stream=None, device=dev)
+    U = gen.gauge_field(L, T, 1004, c["eps"], c["reunit"], device=dev, dtype=torch.complex128)
+    ctx.load_gauge(U)
+    ctx.build_clover()
+    del U
+    x, _ = ctx.pack(gen.spinor_field(L, T, 2004, device=dev, dtype=torch.complex128))
+    y = ctx.half_spinor()
+    for _ in range(3):
+        ctx.apply_schur(x, y)
+    torch.cuda.synchronize()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    n = 10
+    a.record()
+    for _ in range(n):
+        ctx.apply_schur(x, y)
+    b.record()
+    torch.cuda.synchronize()
+    ms = a.elapsed_time(b) / n
+    V = L * L * L * T
+    peak, _ = _peaks()
+    gbs = 2 * 2208 * (V // 2) / (ms * 1e-3) / 1e9
+    ctx.close()
+    return {"lattice": "48^3x96, fp64, 18-real links", "ms": ms, "sites_per_s": V / (ms * 1e-3),
+            "GBps_two_pass_model": gbs, "frac_of_peak": gbs / peak,
+            "GFLOPps": (FLOP_PER_SITE * V + 24 * (V // 2)) / (ms * 1e-3) / 1e9}
+
+
 def paper_context_row(torch, gen, Ddamg, F32, dev, recon):
     """One smoother call each of odd-even Richardson(12, 1.5), odd-even GMRES(3, 4) and SAP(3, 4) at 48^3 x 96."""
     c = CONFIGS[4]
@@ -497,6 +530,10 @@ def main():
             rows["paper_smoother_calls_48x96"] = paper_context_row(torch, gen, Ddamg, F32, dev, args.gauge_recon)
         except Exception as exc:                  # noqa: BLE001 - a side row must not lose the headline
             rows["paper_smoother_calls_48x96"] = {"error": str(exc)[:200]}
+        try:
+            rows["schur_apply_f64_48x96"] = f64_apply_row(torch, gen, Ddamg, dev)
+        except Exception as exc:                  # noqa: BLE001
+            rows["schur_apply_f64_48x96"] = {"error": str(exc)[:200]}
 
     # ---- e2e: HOST buffers, copies inside the timed region, through the public API
     hb = torch.empty_like(pool_b[0][0], device="cpu").pin_memory()
