@@ -1,5 +1,6 @@
 """Full-size parity (BASELINE.json configs[4]: 64^3 x 128, fp32) in the launch configuration
-bench.py times, on sampled outputs the oracle can compute one by one.
+bench.py times, on sampled outputs the oracle can compute one by one; the same at the other
+full-size shapes of BASELINE.json (configs[2]: 32^3 x 64, configs[3]: 48^3 x 96).
 
 The oracle cannot run on 33.5 M sites in seconds, but one Schur apply depends only on spinors
 within 2 sites and links within 3 sites of the output site, and nu Richardson sweeps on 2 nu
@@ -22,7 +23,6 @@ from helpers import CONFIGS, rel_l2
 
 pytestmark = pytest.mark.gpu
 
-CFG = 5
 NU = 4
 
 
@@ -38,23 +38,23 @@ def _cut(field: torch.Tensor, origin, B, L, T) -> torch.Tensor:
 
 
 class FullSize:
-    def __init__(self, recon=18):
+    def __init__(self, cfg=5, recon=18):
         import oracle
         import paper_2407_08092_b200 as dd
         self.oracle, self.dd = oracle, dd
-        c = CONFIGS[CFG]
+        c = CONFIGS[cfg]
         self.c = c
         self.L, self.T = c["L"], c["T"]
         dev = "cuda"
-        self.U = gen.gauge_field(self.L, self.T, 1000 + CFG, c["eps"], c["reunit"], device=dev,
+        self.U = gen.gauge_field(self.L, self.T, 1000 + cfg, c["eps"], c["reunit"], device=dev,
                                  dtype=torch.complex64)
         self.ctx = dd.Ddamg(self.L, self.T, c["csw"], c["m0"], c["bc"], dd.F32)
         self.ctx.load_gauge(self.U)
         self.ctx.build_clover()
         if recon == 12:                        # bench.py --gauge-recon 12: two-row links in the hopping kernels
             self.ctx.set_option("gauge_recon", 12)
-        self.x_nat = gen.spinor_field(self.L, self.T, 3000 + CFG, device=dev, dtype=torch.complex64)
-        self.b_nat = gen.spinor_field(self.L, self.T, 2000 + CFG, device=dev, dtype=torch.complex64)
+        self.x_nat = gen.spinor_field(self.L, self.T, 3000 + cfg, device=dev, dtype=torch.complex64)
+        self.b_nat = gen.spinor_field(self.L, self.T, 2000 + cfg, device=dev, dtype=torch.complex64)
         self.x_e, _ = self.ctx.pack(self.x_nat, want_odd=False)
         self.b_e, _ = self.ctx.pack(self.b_nat, want_odd=False)
 
@@ -72,9 +72,12 @@ class FullSize:
         return ora, np.where(ora.even, xb, 0.0), np.where(ora.even, bb, 0.0)
 
 
-@pytest.fixture(scope="module", params=[18, 12], ids=["links18", "links12"])
+# config 5 = the bench workload (both link formats); configs 3 and 4 = the other full-size shapes
+# of BASELINE.json (32^3 x 64, 48^3 x 96) in the bench's default link format
+@pytest.fixture(scope="module", params=[(5, 18), (5, 12), (3, 12), (4, 12)],
+                ids=["cfg5-links18", "cfg5-links12", "cfg3-links12", "cfg4-links12"])
 def fs(request):
-    f = FullSize(request.param)
+    f = FullSize(*request.param)
     yield f
     f.ctx.close()
 
@@ -83,11 +86,21 @@ def _core(a, m):
     return a[m:-m, m:-m, m:-m, m:-m]
 
 
-BOXES = [((20, 30, 40, 50), "interior"), ((58, 60, 56, 122), "wrap corner + antiperiodic seam")]
+def _origin(fs, name):
+    """Even-parity box origins: one interior, one whose box crosses the periodic seam of all four
+    axes and the antiperiodic time boundary (for config 5: (20,30,40,50) and (58,60,56,122))."""
+    L, T = fs.L, fs.T
+    if name == "interior":
+        return (5 * L // 16, 15 * L // 32, 5 * L // 8, 25 * T // 64)
+    return (L - 6, L - 4, L - 8, T - 6)
 
 
-@pytest.mark.parametrize("origin,name", BOXES)
-def test_schur_apply_full_size_sampled(fs, origin, name):
+BOXES = ["interior", "wrap corner + antiperiodic seam"]
+
+
+@pytest.mark.parametrize("name", BOXES)
+def test_schur_apply_full_size_sampled(fs, name):
+    origin = _origin(fs, name)
     B, m = 12, 4                                        # dependence radius 3 < margin 4; core 4^4
     y = fs.ctx.apply_schur(fs.x_e)
     y_nat = fs.ctx.unpack(y, None)
@@ -100,8 +113,9 @@ def test_schur_apply_full_size_sampled(fs, origin, name):
     assert rel_l2(got, ref) > 1e-3
 
 
-@pytest.mark.parametrize("origin,name", BOXES)
-def test_richardson_full_size_sampled(fs, origin, name):
+@pytest.mark.parametrize("name", BOXES)
+def test_richardson_full_size_sampled(fs, name):
+    origin = _origin(fs, name)
     omega = fs.c["omega"]
     m = 2 * NU + 2                                      # dependence radius 2 nu + 1
     B = 4 + 2 * m
