@@ -81,7 +81,7 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(
-                ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100",
+                ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "50",
                  "-i", str(self.idx)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.th = threading.Thread(target=self._read, daemon=True)
             self.th.start()
@@ -91,6 +91,14 @@ class ClockSampler:
     def _read(self):
         for line in self.proc.stdout:
             self.rows.append([c.strip() for c in line.split(",")])
+
+    def wait_ready(self, timeout_s: float = 5.0):
+        """Block until nvidia-smi has delivered its first sample (its start-up takes longer than a short
+        timed region), then forget the idle samples: everything kept is from the warm-up on."""
+        t0 = time.perf_counter()
+        while self.proc and not self.rows and time.perf_counter() - t0 < timeout_s:
+            time.sleep(0.02)
+        self.rows.clear()
 
     def stop(self):
         if not self.proc:
@@ -390,6 +398,7 @@ def main():
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()                      # sampled from the warm-up on, so short runs still see load
+        sampler.wait_ready()
     ctx.kernel_timing(True)
     for i in range(W):
         prep_x(i); step(i)
