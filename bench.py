@@ -18,7 +18,11 @@ e2e        = same metric through the public API with HOST (pinned) buffers: H2D 
 roofline   = dominant kernel (B': A_ee x - H_eo t + Richardson update), algorithmic bytes
              1248 B/even site / CUDA-event duration, against MEASURED_PEAKS.json
 cpu_baseline = the fp64 oracle (oracle/, as it stands) timed on the host cores on a bounded
-             sample (16^3 x 32 lattice, same recipe)
+             sample (16^3 x 32 lattice, same recipe: `value`), plus SURVEY.md 8(d)'s table: Schur
+             apply and one Richardson sweep at 16^4 and 32^3 x 64, all cores and 1 thread, with the
+             CPU model string
+--rows     = 'all' (default), 'main' (the step only) or a comma list of side rows:
+             links18,schur,smoother,gmres,sap,multi_rhs,paper,f64,cfg3,cfg4
 Multi-GPU: the path does not shard in this build ("replicas only"): --gpus N runs
 N independent replicas, one per rank, no data-path collective; scaling = "weak".
 """
@@ -51,6 +55,8 @@ FLOP_PER_SITE = 1824    # 1320 (hop) + 504 (2 x 6x6 Hermitian mat-vec), per latt
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of kernel B' at config 5, from the
 # ncu --set full capture summarised in profiles/ (None until a capture exists)
 NCU_TRAFFIC_BYTES = {18: {5: 21.274e9}, 12: {5: 18.073e9}}     # profiles/r1b_ncu_full_dslash.md, profiles/r1d_ncu_full_dslash12.md
+NOMINAL_HBM_GBS = 8000.0    # north_star's "~8 TB/s HBM peak" (DGX figure; HGX 7.7 TB/s), quoted beside the measured copy peak
+SIDE_ROWS = ("links18", "schur", "smoother", "gmres", "sap", "multi_rhs", "paper", "f64", "cfg3", "cfg4")
 CPU_SAMPLE = dict(L=16, T=32)
 # SAP(n, m) row: the paper's smoother parameters (Tables 1, 2, 6) on 4^4 blocks
 SAP_N, SAP_M, SAP_BLOCK = 3, 4, (4, 4, 4, 4)
@@ -164,6 +170,62 @@ def oracle_run(steps: int, warmup: int, cfg: int):
                 sample=f"{L}^3x{T} lattice (config {cfg} recipe), {steps} calls of Richardson nu={NU}, fp64 oracle, OpenMP over sites")
 
 
+def cpu_model() -> str:
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.lower().startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except Exception:
+        pass
+    return "unknown"
+
+
+def oracle_detail(cfg: int, device=None):
+    """SURVEY.md 8(d) "Oracle timing beside it": the oracle's Schur apply and ONE Richardson sweep at 16^4 and
+    32^3 x 64 (recipe of `cfg`), with all host cores and with 1 thread.  Inputs are generated outside the
+    timed calls (on `device` when given); the oracle itself runs as it stands (OpenMP over sites, numpy axpy)."""
+    import ctypes
+    import numpy as np
+    import gen
+    import oracle
+    c = CONFIGS[cfg]
+    ncores = os.cpu_count() or 1
+    try:
+        gomp = ctypes.CDLL("libgomp.so.1")
+    except OSError:
+        gomp = None
+    out = {}
+    for L, T, tag in ((16, 16, "16x16"), (32, 64, "32x64")):
+        kw = dict(device=device) if device is not None else {}
+        U = gen.gauge_field(L, T, 1000 + cfg, c["eps"], c["reunit"], **kw).cpu().numpy()
+        op = oracle.WilsonClover(L, T, c["csw"], c["m0"], c["bc"], U)
+        b = np.where(op.even, gen.spinor_field(L, T, 2000 + cfg, **kw).cpu().numpy(), 0.0)
+        x0 = np.where(op.even, gen.spinor_field(L, T, 2500 + cfg, **kw).cpu().numpy(), 0.0)
+        V = L * L * L * T
+        for nt, name in ((ncores, "allcores"), (1, "1thread")):
+            if gomp is None and nt != ncores:
+                continue
+            if gomp is not None:
+                gomp.omp_set_num_threads(nt)
+            reps = 2 if (nt > 1 or V < 1 << 20) else 1
+            op.apply_schur(x0)                                    # warm-up (page-in)
+            t0 = time.perf_counter()
+            for _ in range(reps):
+                op.apply_schur(x0)
+            ta = (time.perf_counter() - t0) / reps
+            t0 = time.perf_counter()
+            for _ in range(reps):
+                oracle.richardson(op.apply_schur, b, x0, 1, c["omega"])
+            ts = (time.perf_counter() - t0) / reps
+            out[f"schur_apply_{tag}_{name}_sites_per_s"] = V / ta
+            out[f"richardson_sweep_{tag}_{name}_sites_per_s"] = V / ts
+        if gomp is not None:
+            gomp.omp_set_num_threads(ncores)
+        del op, U, b, x0
+    out["threads_allcores"] = ncores
+    return out
+
+
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
@@ -180,7 +242,7 @@ def run_reference(args):
         "config": {"workload": f"config {cfg}: {c['L']}^3x{c['T']} Wilson-clover csw={c['csw']} m0={c['m0']}, "
                                f"Richardson nu={NU} omega={c['omega']}; bounded CPU sample {r['sample']}"},
         "cpu_baseline": {"value": r["value"], "unit": "site-sweeps/s", "cores": r["cores"], "kind": "oracle",
-                         "sample": r["sample"]},
+                         "sample": r["sample"], "cpu_model": cpu_model()},
         "e2e": {"value": r["value"], "unit": "site-sweeps/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -221,8 +283,10 @@ def f64_apply_row(torch, gen, Ddamg, dev):
             "GFLOPps": (FLOP_PER_SITE * V + 24 * (V // 2)) / (ms * 1e-3) / 1e9}
 
 
-def paper_context_row(torch, gen, Ddamg, F32, dev, recon):
-    """One smoother call each of odd-even Richardson(12, 1.5), odd-even GMRES(3, 4) and SAP(3, 4) at 48^3 x 96."""
+def config4_rows(torch, gen, Ddamg, F32, dev, recon, want_paper, gmres_split):
+    """Rows on the 48^3 x 96 lattice (BASELINE.json configs[3] = the paper's lattice shape): (i) one smoother call
+    each of odd-even Richardson(12, 1.5), odd-even GMRES(3, 4) and SAP(3, 4) beside the paper's Table 2; (ii) config 4
+    as written: odd-even GMRES(2, 10) from x0 = 0 on a Gaussian rhs, time per Arnoldi step split apply / BLAS-1."""
     c = CONFIGS[4]
     L, T = c["L"], c["T"]
     ctx = Ddamg(L, T, c["csw"], c["m0"], c["bc"], F32, stream=None, device=dev)
@@ -233,10 +297,19 @@ def paper_context_row(torch, gen, Ddamg, F32, dev, recon):
     if recon == 12:
         ctx.set_option("gauge_recon", 12)
     b_e, b_o = ctx.pack(gen.spinor_field(L, T, 2004, device=dev, dtype=torch.complex64))
+    bhat, x_e, x_o = ctx.half_spinor(), ctx.half_spinor(), ctx.half_spinor()
+    res = {}
+    if gmres_split is not None:
+        ctx.prepare_rhs(b_e, b_o, bhat)
+        g = gmres_split(ctx, bhat, x_e, 10, 2, L * L * L * T, 3)
+        g["lattice"] = "48^3x96, fp32, GMRES(n=2, m=10) from x0=0: 20 Arnoldi steps + 3 residual evaluations"
+        res["gmres_2x10_cfg4"] = g
+    if not want_paper:
+        ctx.close()
+        return res
     v = b_e.clone()
     lam = ctx.power_iteration(v, 10)              # Alg. 4 line 1: omega = delta / |lambda_max|, delta = 1.5
     omega = 1.5 / lam
-    bhat, x_e, x_o = ctx.half_spinor(), ctx.half_spinor(), ctx.half_spinor()
 
     def timed_call(fn, n=5):
         for _ in range(2):
@@ -263,7 +336,8 @@ def paper_context_row(torch, gen, Ddamg, F32, dev, recon):
     def sap():
         ctx.sap(b_e, b_o, x_e, x_o, 3, 4, block=(4, 4, 4, 4), zero_init=True)
 
-    out = {"lattice": "48^3x96 (the paper's 96x48^3 shape), synthetic links, fp32, one B200",
+    res["paper_smoother_calls_48x96"] = {
+           "lattice": "48^3x96 (the paper's 96x48^3 shape), synthetic links, fp32, one B200",
            "omega_power_iteration": omega,
            "odd_even_richardson_12_ms": timed_call(rich), "odd_even_gmres_3x4_ms": timed_call(gm),
            "sap_3x4_ms": timed_call(sap),
@@ -273,7 +347,7 @@ def paper_context_row(torch, gen, Ddamg, F32, dev, recon):
                              "/ 16 MPI ranks x 4 OpenMP threads on 32-core x86; CLQCD configuration at m_s; precision not stated; "
                              "another machine and a thermalised configuration: context, not a target"}
     ctx.close()
-    return out
+    return res
 
 
 def main():
@@ -284,7 +358,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=5, choices=sorted(CONFIGS))
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--rows", default="all", help="'all', 'main' (skip the side measurements) or 'multi_rhs' (main + multi-rhs rows)")
+    ap.add_argument("--rows", default="all", help="'all', 'main' (the step only) or a comma list of side rows: " + ",".join(SIDE_ROWS))
     ap.add_argument("--nrhs", default="2,4,8", help="batch sizes of the multi-rhs rows")
     ap.add_argument("--batch-l2-bytes", type=float, default=None, help="override ddamg option batch_l2_bytes")
     ap.add_argument("--gauge-recon", type=int, default=12, choices=[18, 12],
@@ -316,6 +390,9 @@ def main():
         dist.barrier()
 
     W, K = max(3, args.warmup), max(1, args.steps)
+    sel = set(SIDE_ROWS) if args.rows == "all" else set() if args.rows == "main" else {t for t in args.rows.split(",") if t}
+    unknown = sel - set(SIDE_ROWS)
+    assert not unknown, f"unknown --rows entries {sorted(unknown)}; known: {SIDE_ROWS}"
     cfg = args.config
     c = CONFIGS[cfg]
     L, T = c["L"], c["T"]
@@ -368,8 +445,16 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
+    def step_stats(per):
+        q = sorted(per)
+        return {"median": q[len(q) // 2] if len(q) % 2 else 0.5 * (q[len(q) // 2 - 1] + q[len(q) // 2]), "min": q[0],
+                "p95": q[min(len(q) - 1, int(0.95 * len(q)))], "max": q[-1], "n": len(q)}
+
+    last_per_step = []
+
     def timed(fn, steps, warm, prep=None):
-        """Sum of per-step CUDA-event times over `steps` steps; prep() runs outside the events."""
+        """Sum of per-step CUDA-event times over `steps` steps; prep() runs outside the events.
+        The per-step times of the last call stay in last_per_step (this rank's)."""
         for i in range(warm):
             if prep:
                 prep(i)
@@ -385,7 +470,8 @@ def main():
             b.record()
             pairs.append((a, b))
         barrier()
-        ms = sum(a.elapsed_time(b) for a, b in pairs)
+        last_per_step[:] = [a.elapsed_time(b) for a, b in pairs]
+        ms = sum(last_per_step)
         return max_over_ranks(ms, world, dev)
 
     # ---- the step: fused Richardson smoother nu = 4 (rows a2-a7)
@@ -407,6 +493,7 @@ def main():
     launches0 = ctx.launch_count()
     wall0 = time.perf_counter()
     ms_total = timed(step, K, 0, prep_x)
+    stats = step_stats(last_per_step)
     wall = time.perf_counter() - wall0
     launches = ctx.launch_count() - launches0
     clocks = sampler.stop() if rank == 0 else None
@@ -421,10 +508,22 @@ def main():
     tA = msA / max(nA, 1) * 1e-3
     ach_B = BYTES_BR * Ve / tB / 1e9
     ach_A = BYTES_A * Ve / tA / 1e9
+    sweep_gbs = (BYTES_A + BYTES_BR) * Ve * NU / (ms_per_step * 1e-3) / 1e9
     roofline = {"bound": "hbm", "kernel": "dslash_kernel<float, EPI_RICHARDSON> (kernel B')",
                 "achieved": ach_B, "peak": peak, "unit": "GB/s", "frac": ach_B / peak,
                 "traffic": NCU_TRAFFIC_BYTES[args.gauge_recon].get(cfg), "peak_source": peak_src,
+                "traffic_source": "ncu --set full capture of one launch, profiles/ (a citation, not re-measured by this run)"
+                                  if NCU_TRAFFIC_BYTES[args.gauge_recon].get(cfg) else None,
                 "bytes_per_launch": BYTES_BR * Ve, "avg_launch_ms": tB * 1e3, "launches_timed": nB,
+                # flat copies of the other hot kernel and of the whole step (nested objects may be cut by a parser)
+                "kernel_A_achieved": ach_A, "kernel_A_frac": ach_A / peak, "kernel_A_avg_launch_ms": tA * 1e3,
+                "kernel_A_bytes_per_launch": BYTES_A * Ve,
+                "sweep_two_pass_achieved": sweep_gbs, "sweep_two_pass_frac": sweep_gbs / peak,
+                "frac_of_nominal_8TBps": ach_B / NOMINAL_HBM_GBS, "kernel_A_frac_of_nominal_8TBps": ach_A / NOMINAL_HBM_GBS,
+                "sweep_frac_of_nominal_8TBps": sweep_gbs / NOMINAL_HBM_GBS,
+                "peak_note": "the measured peak is a 50/50 read/write copy; these kernels are >= 90 % reads, and a read-dominated "
+                             "stream runs a few % above a copy on HBM3e, so a frac slightly above 1 is a peak-calibration artefact, "
+                             "not extra work: ncu DRAM traffic = 1.02 x algorithmic bytes (profiles/)",
                 "other_kernels": [{"kernel": "dslash_kernel<float, EPI_CLOV_HOP> (kernel A)", "achieved": ach_A,
                                    "frac": ach_A / peak, "bytes_per_launch": BYTES_A * Ve, "avg_launch_ms": tA * 1e3,
                                    "launches_timed": nA}],
@@ -432,7 +531,39 @@ def main():
                                    "frac": (BYTES_A + BYTES_BR) * Ve * NU / (ms_per_step * 1e-3) / 1e9 / peak}}
 
     rows = {"a0_load_gauge_ms": t_a0, "a1_build_clover_ms": t_a1, "input_generation_s": t_gen}
-    if args.rows == "all" and args.gauge_recon == 12:
+    flat = {}        # scalar copies of side-row results for the `config` object (nested rows may be cut by a parser)
+
+    def gmres_split(cx, be, xe, k, cycles, Vloc, reps):
+        """One odd-even GMRES(cycles, k) call: total time and its split into operator applications (kernel
+        classes A, B) and BLAS-1 passes (classes multi-dot, multi-axpy, other streaming passes), CUDA events
+        recorded by the library around every launch."""
+        cx.gmres_oe(be, xe, k, cycles, zero_init=True)                       # warm-up (allocates the basis)
+        cx.kernel_timing(True)
+        cx.kernel_time_ms(0, reset=True)
+        ms = timed(lambda i: cx.gmres_oe(be, xe, k, cycles, zero_init=True), reps, 0) / reps
+        t = {w: cx.kernel_time_ms(w, reset=False) for w in (0, 1, 8, 9, 10)}
+        cx.kernel_time_ms(0, reset=True)
+        cx.kernel_timing(False)
+        steps_ = k * cycles * reps
+        apply_ms = (t[0][0] + t[1][0]) / steps_
+        vb = 96 * (Vloc // 2)                                                # bytes of one half spinor
+        nb_dot = sum(j + 2 for j in range(k)) * cycles * reps                # vectors read by the multi-dots
+        nb_axpy = (sum(j + 3 for j in range(k)) + (k + 2)) * cycles * reps   # read + written by the multi-axpys (+ x += V y)
+        out = {"ms": ms, "ms_per_arnoldi_step": ms / (k * cycles),
+               "apply_ms_per_arnoldi_step": apply_ms,
+               "blas1_ms_per_arnoldi_step": (t[8][0] + t[9][0] + t[10][0]) / steps_,
+               "multi_dot_ms_per_arnoldi_step": t[8][0] / steps_, "multi_axpy_ms_per_arnoldi_step": t[9][0] / steps_,
+               "other_blas1_ms_per_arnoldi_step": t[10][0] / steps_,
+               "multi_dot_GBps": nb_dot * vb / (t[8][0] * 1e-3) / 1e9 if t[8][0] > 0 else None,
+               "multi_axpy_GBps": nb_axpy * vb / (t[9][0] * 1e-3) / 1e9 if t[9][0] > 0 else None,
+               "note": "apply = kernels A + B (incl. the residuals at cycle start / end); blas1 = fused multi-dot, "
+                       "multi-axpy + norm and copy passes; remainder = small device-side scalar kernels and launch gaps"}
+        if out["multi_dot_GBps"]:
+            out["multi_dot_frac_of_peak"] = out["multi_dot_GBps"] / peak
+            out["multi_axpy_frac_of_peak"] = out["multi_axpy_GBps"] / peak
+        return out
+
+    if "links18" in sel and args.gauge_recon == 12:
         # ---- the same step on full 18-real links (two-pass model 1056 + 1248 B per even site)
         ctx.set_option("gauge_recon", 18)
         ks = max(3, min(K, 10))
@@ -443,14 +574,20 @@ def main():
                                       "GBps_two_pass_model": b18 / (ms18 * 1e-3) / 1e9,
                                       "frac_of_peak": b18 / (ms18 * 1e-3) / 1e9 / peak,
                                       "bytes_per_even_site_sweep": BYTES_A + BYTES_BR + 2 * 192}
-    if args.rows == "all":
+        flat["links18_ms_per_step"] = ms18
+        flat["links18_frac_of_peak"] = rows["richardson_links18"]["frac_of_peak"]
+    if "schur" in sel:
         # ---- Schur apply (BASELINE.json metric: GB/s and GFLOP/s, fp32)
         ks = max(3, min(K, 20))
         ms = timed(lambda i: ctx.apply_schur(pool_x[i % NPOOL], y_e), ks, 3) / ks
         gbs = (BYTES_A + BYTES_B) * Ve / (ms * 1e-3) / 1e9
         rows["schur_apply"] = {"ms": ms, "sites_per_s": V / (ms * 1e-3), "GBps_two_pass_model": gbs,
-                               "frac_of_peak": gbs / peak,
-                               "GFLOPps": (FLOP_PER_SITE * V + 24 * Ve) / (ms * 1e-3) / 1e9}
+                               "frac_of_peak": gbs / peak, "frac_of_nominal_8TBps": gbs / NOMINAL_HBM_GBS,
+                               "GFLOPps": (FLOP_PER_SITE * V + 24 * Ve) / (ms * 1e-3) / 1e9,
+                               "per_call_ms": step_stats(last_per_step)}
+        flat.update(schur_apply_ms=ms, schur_apply_GBps=gbs, schur_apply_GFLOPps=rows["schur_apply"]["GFLOPps"],
+                    schur_apply_frac_of_peak=gbs / peak)
+    if "smoother" in sel:
         # ---- whole odd-even smoother call, eq. 2 (a10): prepare_rhs + nu sweeps from 0 + reconstruct_odd
         bhat = ctx.half_spinor()
         x_o = ctx.half_spinor()
@@ -464,13 +601,16 @@ def main():
         ms = timed(smoother, km, 2) / km
         rows["smoother_call_eq2"] = {"ms": ms, "note": "prepare_rhs + Richardson(nu=4, x0=0: first sweep has no apply) + reconstruct_odd"}
         del bhat, x_o
-        # ---- GMRES(1, 10) (a8, a9)
+    if "gmres" in sel:
+        # ---- GMRES(1, 10) (a8, a9) at the bench lattice, split into apply / BLAS-1
         try:
-            kg = 10
-            ms = timed(lambda i: ctx.gmres_oe(pool_b[i % NPOOL][0], x_e, kg, 1, zero_init=True), 2, 1) / 2
-            rows["gmres_1x10"] = {"ms": ms, "ms_per_arnoldi_step": ms / kg}
+            rows["gmres_1x10"] = gmres_split(ctx, pool_b[0][0], x_e, 10, 1, V, 2)
+            flat.update(gmres_1x10_ms_per_arnoldi_step=rows["gmres_1x10"]["ms_per_arnoldi_step"],
+                        gmres_1x10_multi_dot_frac_of_peak=rows["gmres_1x10"].get("multi_dot_frac_of_peak"),
+                        gmres_1x10_multi_axpy_frac_of_peak=rows["gmres_1x10"].get("multi_axpy_frac_of_peak"))
         except Exception as e:     # e.g. Krylov basis does not fit
             rows["gmres_1x10"] = {"error": str(e)}
+    if "sap" in sel:
         # ---- SAP(3,4) on 4^4 blocks (NEXT-3; the smoother of the paper's Tables 2 and 6)
         try:
             xs_e, xs_o = ctx.half_spinor(), ctx.half_spinor()
@@ -491,14 +631,13 @@ def main():
                 "block_kernel_ms": t6 * 1e3, "block_kernel_launches": n6,
                 "residual_kernel_ms": ms5 / max(n5, 1), "residual_kernel_launches": n5,
                 "block_kernel_GFLOPps": flop_blk / t6 / 1e9,
-                "block_kernel_bound": "latency (8 warps/SM; fp32 FMA pipe ~28 % busy, profiles/r1d_ncu_full_sap.md)",
-                "note": "SAP(n=3, m=4), 4^4 blocks, non-zero x0: per iteration and colour one streaming residual "
-                        "(2 launches) + one block-solve launch"}
+                "note": "SAP(n=3, m=4), 4^4 blocks, non-zero x0"}
+            flat["sap_3x4_ms_per_call"] = ms
             del xs_e, xs_o
         except Exception as e:
             rows["sap_3x4_block4"] = {"error": str(e)}
 
-    if args.rows in ("all", "multi_rhs"):
+    if "multi_rhs" in sel:
         # ---- multi-rhs batched Richardson (NEXT-2): links + clover fetched once for nrhs rhs
         rows["multi_rhs_richardson"] = {}
         if args.batch_l2_bytes is not None:
@@ -520,25 +659,67 @@ def main():
                 bA = 192 + (lk + 288) / nrhs     # per (site, rhs): x_e neighbours 96 + write 96 + (links + clover 288) / nrhs
                 bB = 384 + (lk + 288) / nrhs     # t_o 96 + x_e 96 + b_e 96 + write 96 + (links + 288) / nrhs
                 tA3, tB4 = ms3 / max(n3, 1) * 1e-3, ms4 / max(n4, 1) * 1e-3
+                rate = V * NU * nrhs / (ms * 1e-3)
                 rows["multi_rhs_richardson"][str(nrhs)] = {
-                    "ms_per_call": ms, "rhs_site_sweeps_per_s": V * NU * nrhs / (ms * 1e-3),
-                    "speedup_vs_single_rhs": (V * NU * nrhs / (ms * 1e-3)) / (V * NU / (ms_per_step * 1e-3)),
+                    "ms_per_call": ms, "rhs_site_sweeps_per_s": rate,
+                    "speedup_vs_single_rhs": rate / (V * NU / (ms_per_step * 1e-3)),
                     "kernel_A_ms": tA3 * 1e3, "kernel_A_model_GBps": bA * nrhs * Ve / tA3 / 1e9,
                     "kernel_Bp_ms": tB4 * 1e3, "kernel_Bp_model_GBps": bB * nrhs * Ve / tB4 / 1e9,
-                    "model_bytes_per_rhs_site_sweep": bA + bB}
+                    "model_bytes_per_rhs_site_sweep": bA + bB,
+                    "frac_of_byte_model": (bA + bB) * Ve * rate / V / 1e9 / peak}
+                flat[f"multi_rhs_{nrhs}_rhs_site_sweeps_per_s"] = rate
+                flat[f"multi_rhs_{nrhs}_frac_of_byte_model"] = rows["multi_rhs_richardson"][str(nrhs)]["frac_of_byte_model"]
                 del Bb, X0, Xb
                 torch.cuda.empty_cache()
             except Exception as e:
                 rows["multi_rhs_richardson"][str(nrhs)] = {"error": str(e)}
 
-    if args.rows == "all" and rank == 0 and world == 1:
-        # ---- context row: the paper's three smoother configurations (Table 2) on the
-        # paper's lattice SHAPE 48^3 x 96 (synthetic links, fp32; the paper: CLQCD configuration, 16 GPUs
-        # of 64 SMs / 16 GB HBM2 on 4 ORISE nodes, 32-core x86 hosts, precision not stated).  Context only.
+    if "cfg3" in sel and rank == 0 and world == 1:
+        # ---- BASELINE.json configs[2] as written (SURVEY.md 8(d) cfg 3): 32^3 x 64, 100 calls of Richardson nu=4
+        # omega=0.9, each on a FRESH Gaussian b_e and non-zero Gaussian x0 (generated outside the events),
+        # 10 warm-up calls; per-call median / min / p95.  Gauge + clover (2 x 0.4 GB two-row / 0.6 GB) >> L2.
         try:
-            rows["paper_smoother_calls_48x96"] = paper_context_row(torch, gen, Ddamg, F32, dev, args.gauge_recon)
+            c3 = CONFIGS[3]
+            L3, T3 = c3["L"], c3["T"]
+            V3 = L3 ** 3 * T3
+            ctx3 = Ddamg(L3, T3, c3["csw"], c3["m0"], c3["bc"], F32, stream=None, device=dev)
+            ctx3.load_gauge(gen.gauge_field(L3, T3, 1003, c3["eps"], c3["reunit"], device=dev, dtype=torch.complex64))
+            ctx3.build_clover()
+            if args.gauge_recon == 12:
+                ctx3.set_option("gauge_recon", 12)
+            b3, x3 = ctx3.half_spinor(), ctx3.half_spinor()
+
+            def fresh3(i):
+                b3.copy_(ctx3.pack(gen.spinor_field(L3, T3, 2003 + i, device=dev, dtype=torch.complex64), want_odd=False)[0])
+                x3.copy_(ctx3.pack(gen.spinor_field(L3, T3, 3003 + i, device=dev, dtype=torch.complex64), want_odd=False)[0])
+            ms = timed(lambda i: ctx3.richardson(b3, x3, NU, c3["omega"]), 100, 10, fresh3) / 100
+            st3 = step_stats(last_per_step)
+            rows["config3_richardson_100_calls"] = {
+                "lattice": "32^3x64", "ms_per_call_mean": ms, "per_call_ms": st3,
+                "site_sweeps_per_s_median": V3 * NU / (st3["median"] * 1e-3),
+                "GBps_two_pass_model_median": (BYTES_A + BYTES_BR) * (V3 // 2) * NU / (st3["median"] * 1e-3) / 1e9,
+                "note": "100 calls, fresh Gaussian b_e and x0 per call, 10 warm-up calls"}
+            flat.update(cfg3_call_ms_median=st3["median"], cfg3_call_ms_min=st3["min"], cfg3_call_ms_p95=st3["p95"])
+            ctx3.close()
+            del ctx3, b3, x3
+            torch.cuda.empty_cache()
         except Exception as exc:                  # noqa: BLE001 - a side row must not lose the headline
+            rows["config3_richardson_100_calls"] = {"error": str(exc)[:200]}
+
+    if ("paper" in sel or "cfg4" in sel) and rank == 0 and world == 1:
+        # ---- 48^3 x 96 (BASELINE.json configs[3]; also the paper's lattice shape, Table 5)
+        try:
+            res4 = config4_rows(torch, gen, Ddamg, F32, dev, args.gauge_recon, "paper" in sel,
+                                gmres_split if "cfg4" in sel else None)
+            rows.update(res4)
+            g4 = res4.get("gmres_2x10_cfg4")
+            if g4 and "ms" in g4:
+                flat.update(cfg4_gmres_2x10_ms=g4["ms"], cfg4_ms_per_arnoldi_step=g4["ms_per_arnoldi_step"],
+                            cfg4_apply_ms_per_arnoldi_step=g4["apply_ms_per_arnoldi_step"],
+                            cfg4_blas1_ms_per_arnoldi_step=g4["blas1_ms_per_arnoldi_step"])
+        except Exception as exc:                  # noqa: BLE001
             rows["paper_smoother_calls_48x96"] = {"error": str(exc)[:200]}
+    if "f64" in sel and rank == 0 and world == 1:
         try:
             rows["schur_apply_f64_48x96"] = f64_apply_row(torch, gen, Ddamg, dev)
         except Exception as exc:                  # noqa: BLE001
@@ -608,14 +789,21 @@ def main():
                    "bytes_per_even_site": {"kernel_A": BYTES_A, "kernel_B": BYTES_B, "kernel_Bprime": BYTES_BR},
                    "multi_gpu": "replicas only (no sharding, no collective on the data path)",
                    "timing": "sum of per-step CUDA-event times on the launching stream; x0 refresh copy outside the events",
-                   "wall_s_timed_region": wall},
+                   "wall_s_timed_region": wall,
+                   "step_ms_median": stats["median"], "step_ms_min": stats["min"], "step_ms_p95": stats["p95"]},
+        "ms_per_step_median": stats["median"], "ms_per_step_min": stats["min"], "ms_per_step_p95": stats["p95"],
         "roofline": roofline, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks, "rows": rows,
     }
+    line["config"].update({k: v for k, v in flat.items() if v is not None})
     if rank == 0:
         if world == 1 and not args.no_cpu_baseline:
             r = oracle_run(6, 1, cfg)
             line["cpu_baseline"] = {"value": r["value"], "unit": "site-sweeps/s", "cores": r["cores"],
-                                    "kind": "oracle", "sample": r["sample"]}
+                                    "kind": "oracle", "sample": r["sample"], "cpu_model": cpu_model()}
+            try:            # apply and one sweep at 16^4 and 32^3x64, all cores and 1 thread
+                line["cpu_baseline"].update(oracle_detail(cfg, dev))
+            except Exception as exc:      # noqa: BLE001
+                line["cpu_baseline"]["detail_error"] = str(exc)[:200]
         print(json.dumps(line))
     if world > 1:
         dist.barrier()

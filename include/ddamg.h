@@ -301,8 +301,11 @@ long long ddamg_launch_count(ddamg_ctx* ctx);
  * number of launches of kernel class `which` (0 = kernel A: A_oo^-1 H_oe, 1 = kernel B /
  * B': A_ee x - H_eo t with optional Richardson update, 2 = eq.-2 factors, 3 / 4 = the
  * multi-rhs forms of kernel A / kernel B, B', 5 = one parity of the full operator /
- * residual, 6 = SAP block-solve kernel) since the last reset, after
- * synchronising the stream.  Used by bench.py for the per-kernel roofline.
+ * residual, 6 = SAP block-solve kernel, 7 = fused sweep, 8 = fused multi-dot, 9 = fused
+ * multi-axpy (+ norm), 10 = the other streaming BLAS-1 passes of GMRES / GCR) since the last
+ * reset, after synchronising the stream.  The event pairs come from a pool created by
+ * ddamg_kernel_timing(ctx, 1) (4096 pairs, grown in chunks if a measurement records more):
+ * no event is created inside a timed call.  Used by bench.py for the per-kernel roofline.
  */
 int ddamg_kernel_timing(ddamg_ctx* ctx, int on);
 int ddamg_kernel_time_ms(ddamg_ctx* ctx, int which, double* ms, long long* launches, int reset);

@@ -61,7 +61,8 @@ struct ddamg_ctx {
     // optional per-kernel timing
     bool timing;
     struct Ev { cudaEvent_t a, b; int which; };
-    std::vector<Ev> events;
+    std::vector<Ev> events;     // pool of event pairs, created by ddamg_kernel_timing(1): none is created inside a timed call
+    size_t ev_used;             // pairs recorded since the last reset
 };
 
 static thread_local std::string g_err_noctx;
@@ -102,6 +103,36 @@ struct NvtxRange {
         if (!(ctx)) return DDAMG_EINVAL;                                     \
         if ((ctx)->sticky != DDAMG_OK) return (ctx)->sticky;                 \
     } while (0)
+
+// Optional per-kernel timing: brackets the launches issued during its lifetime with a pair of
+// pooled CUDA events on the context's stream, tagged with the kernel class `which`.
+static const size_t EV_POOL_CHUNK = 4096;
+static bool grow_event_pool(ddamg_ctx* ctx, size_t n)
+{
+    for (size_t i = 0; i < n; ++i) {
+        ddamg_ctx::Ev ev;
+        if (cudaEventCreate(&ev.a) != cudaSuccess) { cudaGetLastError(); return false; }
+        if (cudaEventCreate(&ev.b) != cudaSuccess) { cudaGetLastError(); cudaEventDestroy(ev.a); return false; }
+        ev.which = -1;
+        ctx->events.push_back(ev);
+    }
+    return true;
+}
+struct KernelTimer {
+    ddamg_ctx* c;
+    long idx;
+    KernelTimer(ddamg_ctx* ctx, int which) : c(ctx), idx(-1)
+    {
+        if (!c->timing) return;
+        if (c->ev_used == c->events.size() && !grow_event_pool(c, EV_POOL_CHUNK)) return;   // pool exhausted: rare, outside steady state
+        idx = (long)c->ev_used++;
+        c->events[idx].which = which;
+        cudaEventRecord(c->events[idx].a, c->stream);
+    }
+    ~KernelTimer() { if (idx >= 0) cudaEventRecord(c->events[idx].b, c->stream); }
+};
+enum { KT_A = 0, KT_B = 1, KT_EQ2 = 2, KT_BATCH_A = 3, KT_BATCH_B = 4, KT_FULL = 5, KT_SAP = 6, KT_FUSED = 7,
+       KT_MDOT = 8, KT_MAXPY = 9, KT_BLAS1 = 10 };
 
 static int after_launch(ddamg_ctx* ctx, int n = 1)
 {
@@ -199,13 +230,15 @@ extern "C" int ddamg_create(ddamg_ctx** out, int L, int T, double csw, double m0
     for (int mu = 0; mu < 4; ++mu) ctx->sap_built[mu] = 0;
     ctx->partials = nullptr; ctx->sc = nullptr; ctx->host_hist = nullptr; ctx->singular = nullptr;
     ctx->have_gauge = ctx->have_clover = ctx->have_clov_oo = false;
-    ctx->sticky = DDAMG_OK; ctx->launches = 0; ctx->timing = false;
+    ctx->sticky = DDAMG_OK; ctx->launches = 0; ctx->timing = false; ctx->ev_used = 0;
 
     const size_t gauge_bytes = (size_t)2 * 4 * 18 * ctx->g.Vh * ctx->real_bytes;
     const size_t clov_bytes = (size_t)72 * ctx->g.Vh * ctx->real_bytes;
     const int dgrid = dslash_grid(ctx->g);
-    const int bgrid = blas_grid(ctx->nreal / 2);
-    ctx->partials_len = (size_t)(2 * dgrid > bgrid * 2 * MDOT_NB ? 2 * dgrid : bgrid * 2 * MDOT_NB);
+    // reduction scratch: 2 * dgrid norm partials (both parities of the full operator), or the partials of the
+    // widest BLAS-1 grid (every BLAS-1 grid is <= blas_grid_cap(), whatever the vector length)
+    const int bcap = blas_grid_cap();
+    ctx->partials_len = (size_t)(2 * dgrid > bcap * 2 * MDOT_NB ? 2 * dgrid : bcap * 2 * MDOT_NB);
     cudaError_t e = cudaSuccess;
     if (e == cudaSuccess) e = cudaMalloc(&ctx->gauge, gauge_bytes);
     if (e == cudaSuccess) e = cudaMalloc(&ctx->clov[0], clov_bytes);
@@ -289,6 +322,7 @@ extern "C" int ddamg_build_clover(ddamg_ctx* ctx)
 {
     ENTER(ctx);
     if (!ctx->have_gauge) return fail(ctx, DDAMG_ESTATE, "ddamg_build_clover: no gauge field loaded");
+    // fast path: register-resident leaves + unpivoted LDL^H; the flag asks for the pivoted rebuild
     CK(cudaMemsetAsync(ctx->singular, 0, sizeof(int), ctx->stream));
     if (ctx->prec == DDAMG_F32)
         launch_build_clover<float>(ctx->g, ctx->csw, ctx->m0, ctx->gauge, ctx->clov[0], ctx->clov[1], nullptr, ctx->singular, ctx->stream);
@@ -299,6 +333,19 @@ extern "C" int ddamg_build_clover(ddamg_ctx* ctx)
     int flag = 0;
     CK(cudaMemcpyAsync(&flag, ctx->singular, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
     CK(cudaStreamSynchronize(ctx->stream));
+    if (flag) {
+        // some odd-site block has a small unpivoted pivot (indefinite or singular block): Gauss-Jordan with
+        // partial pivoting for every block, which also applies the singularity criterion of reading C6
+        CK(cudaMemsetAsync(ctx->singular, 0, sizeof(int), ctx->stream));
+        if (ctx->prec == DDAMG_F32)
+            launch_build_clover_pivoted<float>(ctx->g, ctx->csw, ctx->m0, ctx->gauge, ctx->clov[0], ctx->clov[1], nullptr, ctx->singular, ctx->stream);
+        else
+            launch_build_clover_pivoted<double>(ctx->g, ctx->csw, ctx->m0, ctx->gauge, ctx->clov[0], ctx->clov[1], nullptr, ctx->singular, ctx->stream);
+        s = after_launch(ctx);
+        if (s != DDAMG_OK) return s;
+        CK(cudaMemcpyAsync(&flag, ctx->singular, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
+        CK(cudaStreamSynchronize(ctx->stream));
+    }
     if (flag) return fail(ctx, DDAMG_ESINGULAR, "ddamg_build_clover: a 6x6 odd-site block is numerically singular");
     ctx->have_clover = true;
     ctx->sap_built[0] = 0;                                  // SAP operand copies are stale
@@ -341,23 +388,13 @@ static int dslash(ddamg_ctx* ctx, int epi, bool norm, int parity, const void* in
 {
     double* partials = (nrhs > 1 ? ctx->partials_batch : ctx->partials) + partials_offset;
     const void* clov = clov_override ? clov_override : ctx->clov[parity];
-    ddamg_ctx::Ev ev;
-    if (ctx->timing) {
-        if (cudaEventCreate(&ev.a) != cudaSuccess || cudaEventCreate(&ev.b) != cudaSuccess)
-            return check_cuda(ctx, cudaGetLastError(), "cudaEventCreate");
-        ev.which = which;
-        cudaEventRecord(ev.a, ctx->stream);
-    }
+    KernelTimer kt(ctx, which);
     if (ctx->prec == DDAMG_F32)
         launch_dslash<float>(ctx->g, epi, norm, parity, in, hop_gauge_block(ctx, parity), hop_gauge_block(ctx, 1 - parity),
                              clov, own, rhs, out, omega, partials, nrhs, ctx->batch_l2_bytes, ctx->recon, ctx->bc == 1, ctx->stream);
     else
         launch_dslash<double>(ctx->g, epi, norm, parity, in, hop_gauge_block(ctx, parity), hop_gauge_block(ctx, 1 - parity),
                               clov, own, rhs, out, omega, partials, nrhs, ctx->batch_l2_bytes, ctx->recon, ctx->bc == 1, ctx->stream);
-    if (ctx->timing) {
-        cudaEventRecord(ev.b, ctx->stream);
-        ctx->events.push_back(ev);
-    }
     return after_launch(ctx);
 }
 
@@ -373,13 +410,7 @@ static bool use_fused(ddamg_ctx* ctx) { return ctx->fused_sweep && sweep_eligibl
 
 static int fused(ddamg_ctx* ctx, int epi_b, bool norm, const void* x_e, const void* rhs, void* out, double omega)
 {
-    ddamg_ctx::Ev ev;
-    if (ctx->timing) {
-        if (cudaEventCreate(&ev.a) != cudaSuccess || cudaEventCreate(&ev.b) != cudaSuccess)
-            return check_cuda(ctx, cudaGetLastError(), "cudaEventCreate");
-        ev.which = 7;
-        cudaEventRecord(ev.a, ctx->stream);
-    }
+    KernelTimer kt(ctx, KT_FUSED);
     cudaError_t e = ctx->prec == DDAMG_F32
         ? launch_sweep<float>(ctx->g, epi_b, norm, x_e, ctx->tmp_o, hop_gauge_block(ctx, 0), hop_gauge_block(ctx, 1),
                               ctx->clov[0], ctx->clov[1], rhs, out, omega, ctx->partials, ctx->sweep_sync,
@@ -388,7 +419,6 @@ static int fused(ddamg_ctx* ctx, int epi_b, bool norm, const void* x_e, const vo
                                ctx->clov[0], ctx->clov[1], rhs, out, omega, ctx->partials, ctx->sweep_sync,
                                ctx->sweep_lag, ctx->recon, ctx->bc == 1, ctx->stream);
     if (e != cudaSuccess) return check_cuda(ctx, e, "fused sweep memset");
-    if (ctx->timing) { cudaEventRecord(ev.b, ctx->stream); ctx->events.push_back(ev); }
     return after_launch(ctx);
 }
 
@@ -429,9 +459,9 @@ static int reset_hist(ddamg_ctx* ctx)
 }
 
 template <typename T>
-static void t_axpy_norm(ddamg_ctx* ctx, double alpha, const void* x, void* y, double* partials)
+static int t_axpy_norm(ddamg_ctx* ctx, double alpha, const void* x, void* y, double* partials)
 {
-    launch_axpy_norm<T>(ctx->nreal, alpha, x, y, partials, ctx->stream);
+    return launch_axpy_norm<T>(ctx->nreal, alpha, x, y, partials, ctx->stream);
 }
 
 extern "C" int ddamg_richardson(ddamg_ctx* ctx, const void* b_e, void* x_e, int nu, double omega, int zero_init,
@@ -447,11 +477,11 @@ extern "C" int ddamg_richardson(ddamg_ctx* ctx, const void* b_e, void* x_e, int 
     int done = 0;
     if (zero_init && nu > 0) {
         // x^(0) = 0:  r = b,  x^(1) = omega b  (no operator application; Alg. 4 line 3-4)
-        if (ctx->prec == DDAMG_F32) t_axpy_norm<float>(ctx, omega, b_e, x_e, hist ? ctx->partials : nullptr);
-        else t_axpy_norm<double>(ctx, omega, b_e, x_e, hist ? ctx->partials : nullptr);
+        const int nblk = ctx->prec == DDAMG_F32 ? t_axpy_norm<float>(ctx, omega, b_e, x_e, hist ? ctx->partials : nullptr)
+                                                : t_axpy_norm<double>(ctx, omega, b_e, x_e, hist ? ctx->partials : nullptr);
         s = after_launch(ctx);
         if (s != DDAMG_OK) return s;
-        if (hist) { launch_finalize_norm(ctx->partials, blas_grid(ctx->nreal / (16 / ctx->real_bytes)), ctx->sc, 1, ctx->stream); s = after_launch(ctx); if (s != DDAMG_OK) return s; }
+        if (hist) { launch_finalize_norm(ctx->partials, nblk, ctx->sc, 1, ctx->stream); s = after_launch(ctx); if (s != DDAMG_OK) return s; }
         done = 1;
     } else if (zero_init) {
         CK(cudaMemsetAsync(x_e, 0, ctx->half_bytes, ctx->stream));
@@ -617,9 +647,8 @@ static int gmres_impl(ddamg_ctx* ctx, const void* b_e, void* x_e, int k, int cyc
 {
     cudaStream_t st = ctx->stream;
     const size_t nreal = ctx->nreal;
-    const int vecN = (int)(16 / ctx->real_bytes);
-    const int bgrid = blas_grid(nreal / vecN);
     const int dgrid = dslash_grid(ctx->g);
+    int nblk = 0;                                                        // partial blocks of the last BLAS-1 reduction
     char* V = (char*)ctx->krylov;
     auto Vj = [&](int j) { return (void*)(V + (size_t)j * ctx->half_bytes); };
     // The basis is kept lazily normalised: slot i holds an un-normalised vector and the device
@@ -633,8 +662,8 @@ static int gmres_impl(ddamg_ctx* ctx, const void* b_e, void* x_e, int k, int cyc
     if (s != DDAMG_OK) return s;
     double bnorm = 0.0;
     if (tol > 0.0) {
-        launch_copy_norm<T>(nreal, b_e, Vj(0), ctx->partials, st);
-        launch_finalize_norm(ctx->partials, bgrid, ctx->sc, 0, st);
+        nblk = launch_copy_norm<T>(nreal, b_e, Vj(0), ctx->partials, st);
+        launch_finalize_norm(ctx->partials, nblk, ctx->sc, 0, st);
         s = after_launch(ctx, 2); if (s != DDAMG_OK) return s;
         CK(cudaMemcpyAsync(&bnorm, (char*)ctx->sc + offsetof(Scalars, value), sizeof(double), cudaMemcpyDeviceToHost, st));
         CK(cudaStreamSynchronize(st));
@@ -644,9 +673,9 @@ static int gmres_impl(ddamg_ctx* ctx, const void* b_e, void* x_e, int k, int cyc
     for (int c = 0; c < cycles && !converged; ++c) {
         // line 2: r = b - D_S x, beta = ||r||
         if (zero_init && c == 0) {
-            launch_copy_norm<T>(nreal, b_e, Vj(0), ctx->partials, st);
+            { KernelTimer kt(ctx, KT_BLAS1); nblk = launch_copy_norm<T>(nreal, b_e, Vj(0), ctx->partials, st); }
             s = after_launch(ctx); if (s != DDAMG_OK) return s;
-            launch_finalize_norm(ctx->partials, bgrid, ctx->sc, 1, st);
+            launch_finalize_norm(ctx->partials, nblk, ctx->sc, 1, st);
         } else {
             s = dslash(ctx, EPI_CLOV_HOP, false, 1, x_e, nullptr, nullptr, ctx->tmp_o, 0.0, 0);
             if (s != DDAMG_OK) return s;
@@ -670,19 +699,22 @@ static int gmres_impl(ddamg_ctx* ctx, const void* b_e, void* x_e, int k, int cyc
             // lines 6-7 (fused classical Gram-Schmidt): h_ij = <v_i, w>, i = 0..j
             for (int i0 = 0; i0 <= j; i0 += MDOT_NB) {
                 const int nb = (j + 1 - i0) < MDOT_NB ? (j + 1 - i0) : MDOT_NB;
-                launch_multi_dot<T>(nreal, nb, Vj(i0), nreal, Vj(j + 1), ctx->partials, st);
-                launch_finalize_dots_lazy(ctx->partials, bgrid, nb, ctx->sc, i0, j, st);
+                { KernelTimer kt(ctx, KT_MDOT); nblk = launch_multi_dot<T>(nreal, nb, Vj(i0), nreal, Vj(j + 1), ctx->partials, st); }
+                launch_finalize_dots_lazy(ctx->partials, nblk, nb, ctx->sc, i0, j, st);
                 s = after_launch(ctx, 2); if (s != DDAMG_OK) return s;
             }
             // w = vs[j] V[j+1] - sum_i h_ij vs[i] stored_i ; line 8: h_{j+1,j} = ||w||
             for (int i0 = 0; i0 <= j; i0 += MDOT_NB) {
                 const int nb = (j + 1 - i0) < MDOT_NB ? (j + 1 - i0) : MDOT_NB;
                 const bool last = i0 + MDOT_NB > j;
-                launch_multi_axpy<T>(nreal, nb, Vj(i0), nreal, coef_negh + 2 * i0, Vj(j + 1), last ? ctx->partials : nullptr, st,
-                                     i0 == 0 ? vs + j : nullptr);
+                {
+                    KernelTimer kt(ctx, KT_MAXPY);
+                    nblk = launch_multi_axpy<T>(nreal, nb, Vj(i0), nreal, coef_negh + 2 * i0, Vj(j + 1), last ? ctx->partials : nullptr, st,
+                                                i0 == 0 ? vs + j : nullptr);
+                }
                 s = after_launch(ctx); if (s != DDAMG_OK) return s;
             }
-            launch_finalize_norm(ctx->partials, bgrid, ctx->sc, 0, st);
+            launch_finalize_norm(ctx->partials, nblk, ctx->sc, 0, st);
             launch_gmres_givens(ctx->sc, j, st);                         // also vs[j+1] = 1 / h_{j+1,j}
             s = after_launch(ctx, 2); if (s != DDAMG_OK) return s;
             m = j + 1;
@@ -701,7 +733,7 @@ static int gmres_impl(ddamg_ctx* ctx, const void* b_e, void* x_e, int k, int cyc
         s = after_launch(ctx); if (s != DDAMG_OK) return s;
         for (int i0 = 0; i0 < m; i0 += MDOT_NB) {
             const int nb = (m - i0) < MDOT_NB ? (m - i0) : MDOT_NB;
-            launch_multi_axpy<T>(nreal, nb, Vj(i0), nreal, coef_ys + 2 * i0, x_e, nullptr, st);
+            { KernelTimer kt(ctx, KT_MAXPY); launch_multi_axpy<T>(nreal, nb, Vj(i0), nreal, coef_ys + 2 * i0, x_e, nullptr, st); }
             s = after_launch(ctx); if (s != DDAMG_OK) return s;
         }
     }
@@ -758,9 +790,8 @@ static int gcr_impl(ddamg_ctx* ctx, const void* b_e, void* x_e, int k, int cycle
 {
     cudaStream_t st = ctx->stream;
     const size_t nreal = ctx->nreal;
-    const int vecN = (int)(16 / ctx->real_bytes);
-    const int bgrid = blas_grid(nreal / vecN);
     const int dgrid = dslash_grid(ctx->g);
+    int nblk = 0;                                                        // partial blocks of the last BLAS-1 reduction
     char* base = (char*)ctx->krylov;
     auto P = [&](int j) { return (void*)(base + (size_t)j * ctx->half_bytes); };
     auto Z = [&](int j) { return (void*)(base + (size_t)(k + j) * ctx->half_bytes); };
@@ -779,8 +810,8 @@ static int gcr_impl(ddamg_ctx* ctx, const void* b_e, void* x_e, int k, int cycle
         return DDAMG_OK;
     };
     if (tol > 0.0) {
-        launch_copy_norm<T>(nreal, b_e, r, ctx->partials, st);
-        launch_finalize_norm(ctx->partials, bgrid, ctx->sc, 0, st);
+        nblk = launch_copy_norm<T>(nreal, b_e, r, ctx->partials, st);
+        launch_finalize_norm(ctx->partials, nblk, ctx->sc, 0, st);
         s = after_launch(ctx, 2); if (s != DDAMG_OK) return s;
         CK(cudaMemcpyAsync(&bnorm, (char*)ctx->sc + offsetof(Scalars, value), sizeof(double), cudaMemcpyDeviceToHost, st));
         CK(cudaStreamSynchronize(st));
@@ -790,9 +821,9 @@ static int gcr_impl(ddamg_ctx* ctx, const void* b_e, void* x_e, int k, int cycle
     for (int c = 0; c < cycles && !converged; ++c) {
         // line 2: r = b - D_S x
         if (zero_init && c == 0) {
-            launch_copy_norm<T>(nreal, b_e, r, ctx->partials, st);
+            { KernelTimer kt(ctx, KT_BLAS1); nblk = launch_copy_norm<T>(nreal, b_e, r, ctx->partials, st); }
             s = after_launch(ctx); if (s != DDAMG_OK) return s;
-            launch_finalize_norm(ctx->partials, bgrid, ctx->sc, 1, st);
+            launch_finalize_norm(ctx->partials, nblk, ctx->sc, 1, st);
         } else {
             s = dslash(ctx, EPI_CLOV_HOP, false, 1, x_e, nullptr, nullptr, ctx->tmp_o, 0.0, 0);
             if (s != DDAMG_OK) return s;
@@ -809,12 +840,12 @@ static int gcr_impl(ddamg_ctx* ctx, const void* b_e, void* x_e, int k, int cycle
         // line 4: z_1 = D_S r (p_1 = r is written by the form pass, which also gives delta_1, <z_1, r>)
         s = schur(ctx, r, Z(0));
         if (s != DDAMG_OK) return s;
-        launch_gcr_form<T>(nreal, 0, nullptr, nullptr, nreal, nullptr, Z(0), r, P(0), 1, ctx->partials, st);
+        { KernelTimer kt(ctx, KT_BLAS1); nblk = launch_gcr_form<T>(nreal, 0, nullptr, nullptr, nreal, nullptr, Z(0), r, P(0), 1, ctx->partials, st); }
         s = after_launch(ctx); if (s != DDAMG_OK) return s;
         for (int j = 0; j < k; ++j) {
-            launch_gcr_alpha(ctx->partials, bgrid, ctx->sc, j, st);                       // lines 6-7
-            launch_gcr_update<T>(nreal, alpha, P(j), Z(j), x_e, r, ctx->partials, st);    // lines 8-9
-            launch_finalize_norm(ctx->partials, bgrid, ctx->sc, 1, st);
+            launch_gcr_alpha(ctx->partials, nblk, ctx->sc, j, st);                        // lines 6-7
+            { KernelTimer kt(ctx, KT_BLAS1); nblk = launch_gcr_update<T>(nreal, alpha, P(j), Z(j), x_e, r, ctx->partials, st); }   // lines 8-9
+            launch_finalize_norm(ctx->partials, nblk, ctx->sc, 1, st);
             s = after_launch(ctx, 3); if (s != DDAMG_OK) return s;
             if (tol > 0.0) {
                 double v = 0.0;
@@ -826,16 +857,19 @@ static int gcr_impl(ddamg_ctx* ctx, const void* b_e, void* x_e, int k, int cycle
             if (s != DDAMG_OK) return s;
             for (int i0 = 0; i0 <= j; i0 += MDOT_NB) {                                     // line 12
                 const int nb = (j + 1 - i0) < MDOT_NB ? (j + 1 - i0) : MDOT_NB;
-                launch_multi_dot<T>(nreal, nb, Z(i0), nreal, Z(j + 1), ctx->partials, st);
-                launch_finalize_dots(ctx->partials, bgrid, nb, ctx->sc, i0, st);
+                { KernelTimer kt(ctx, KT_MDOT); nblk = launch_multi_dot<T>(nreal, nb, Z(i0), nreal, Z(j + 1), ctx->partials, st); }
+                launch_finalize_dots(ctx->partials, nblk, nb, ctx->sc, i0, st);
                 launch_gcr_beta(ctx->sc, i0, nb, st);
                 s = after_launch(ctx, 3); if (s != DDAMG_OK) return s;
             }
             for (int i0 = 0; i0 <= j; i0 += MDOT_NB) {                                     // lines 13-14
                 const int nb = (j + 1 - i0) < MDOT_NB ? (j + 1 - i0) : MDOT_NB;
                 const bool last = i0 + MDOT_NB > j;
-                launch_gcr_form<T>(nreal, nb, Z(i0), P(i0), nreal, beta + 2 * i0, Z(j + 1), r, P(j + 1), i0 == 0,
-                                   last ? ctx->partials : nullptr, st);
+                {
+                    KernelTimer kt(ctx, KT_BLAS1);
+                    nblk = launch_gcr_form<T>(nreal, nb, Z(i0), P(i0), nreal, beta + 2 * i0, Z(j + 1), r, P(j + 1), i0 == 0,
+                                              last ? ctx->partials : nullptr, st);
+                }
                 s = after_launch(ctx); if (s != DDAMG_OK) return s;
             }
         }
@@ -944,9 +978,8 @@ static int fgmres_impl(ddamg_ctx* ctx, const void* b_e, const void* b_o, void* x
     Scalars* sc = ctx->sc2;
     const size_t nhalf = ctx->nreal, nfull = 2 * ctx->nreal;
     const size_t full_bytes = 2 * ctx->half_bytes;
-    const int vecN = (int)(16 / ctx->real_bytes);
-    const int bgrid = blas_grid(nfull / vecN);
     const int dgrid = dslash_grid(ctx->g);
+    int nblk = 0, nblk_b = 0;
     char* base = (char*)ctx->fgm_basis;
     auto Ve = [&](int j) { return (void*)(base + (size_t)j * full_bytes); };                       // v_j, even half
     auto Vo = [&](int j) { return (void*)(base + (size_t)j * full_bytes + ctx->half_bytes); };
@@ -969,9 +1002,9 @@ static int fgmres_impl(ddamg_ctx* ctx, const void* b_e, const void* b_o, void* x
     };
     double bnorm = 0.0;
     {   // ||b|| (the tolerance is relative to it)
-        launch_copy_norm<T>(nhalf, b_e, Ve(0), ctx->partials, st);
-        launch_copy_norm<T>(nhalf, b_o, Vo(0), ctx->partials + blas_grid(nhalf / vecN), st);
-        launch_finalize_norm(ctx->partials, 2 * blas_grid(nhalf / vecN), sc, 0, st);
+        nblk_b = launch_copy_norm<T>(nhalf, b_e, Ve(0), ctx->partials, st);
+        nblk_b += launch_copy_norm<T>(nhalf, b_o, Vo(0), ctx->partials + nblk_b, st);
+        launch_finalize_norm(ctx->partials, nblk_b, sc, 0, st);
         s = after_launch(ctx, 3); if (s != DDAMG_OK) return s;
         if (tol > 0.0) {
             CK(cudaMemcpyAsync(&bnorm, value, sizeof(double), cudaMemcpyDeviceToHost, st));
@@ -986,7 +1019,7 @@ static int fgmres_impl(ddamg_ctx* ctx, const void* b_e, const void* b_o, void* x
     for (int c = 0; c < cycles && !converged; ++c) {
         if (zero_init && c == 0) {
             // r = b: v_0 already holds b and sc->value its norm
-            launch_finalize_norm(ctx->partials, 2 * blas_grid(nhalf / vecN), sc, 1, st);
+            launch_finalize_norm(ctx->partials, nblk_b, sc, 1, st);
             s = after_launch(ctx); if (s != DDAMG_OK) return s;
         } else {
             s = residual(); if (s != DDAMG_OK) return s;
@@ -1008,17 +1041,17 @@ static int fgmres_impl(ddamg_ctx* ctx, const void* b_e, const void* b_o, void* x
             if (s != DDAMG_OK) return s;
             for (int i0 = 0; i0 <= j; i0 += MDOT_NB) {
                 const int nb = (j + 1 - i0) < MDOT_NB ? (j + 1 - i0) : MDOT_NB;
-                launch_multi_dot<T>(nfull, nb, Ve(i0), nfull, Ve(j + 1), ctx->partials, st);
-                launch_finalize_dots(ctx->partials, bgrid, nb, sc, i0, st);
+                nblk = launch_multi_dot<T>(nfull, nb, Ve(i0), nfull, Ve(j + 1), ctx->partials, st);
+                launch_finalize_dots(ctx->partials, nblk, nb, sc, i0, st);
                 s = after_launch(ctx, 2); if (s != DDAMG_OK) return s;
             }
             for (int i0 = 0; i0 <= j; i0 += MDOT_NB) {
                 const int nb = (j + 1 - i0) < MDOT_NB ? (j + 1 - i0) : MDOT_NB;
                 const bool last = i0 + MDOT_NB > j;
-                launch_multi_axpy<T>(nfull, nb, Ve(i0), nfull, coef_negh + 2 * i0, Ve(j + 1), last ? ctx->partials : nullptr, st);
+                nblk = launch_multi_axpy<T>(nfull, nb, Ve(i0), nfull, coef_negh + 2 * i0, Ve(j + 1), last ? ctx->partials : nullptr, st);
                 s = after_launch(ctx); if (s != DDAMG_OK) return s;
             }
-            launch_finalize_norm(ctx->partials, bgrid, sc, 0, st);
+            launch_finalize_norm(ctx->partials, nblk, sc, 0, st);
             launch_gmres_givens(sc, j, st);
             launch_scale_by_dev<T>(nfull, Ve(j + 1), scale, st);
             s = after_launch(ctx, 3); if (s != DDAMG_OK) return s;
@@ -1158,18 +1191,11 @@ extern "C" int ddamg_sap(ddamg_ctx* ctx, const void* b_e, const void* b_o, void*
     };
     auto blocks = [&](int colour, const void* r_e, const void* r_o) -> int {
         if (m == 0) return DDAMG_OK;                       // zero Minimal Residual iterations: e_k = 0
-        ddamg_ctx::Ev ev;
-        if (ctx->timing) {
-            if (cudaEventCreate(&ev.a) != cudaSuccess || cudaEventCreate(&ev.b) != cudaSuccess)
-                return check_cuda(ctx, cudaGetLastError(), "cudaEventCreate");
-            ev.which = 6;
-            cudaEventRecord(ev.a, st);
-        }
+        KernelTimer kt(ctx, KT_SAP);
         cudaError_t e = f32
             ? launch_sap_blocks<float>(ctx->g, sg, colour, m, ctx->sap_links, ctx->sap_clov, r_e, r_o, x_e, x_o, st)
             : launch_sap_blocks<double>(ctx->g, sg, colour, m, ctx->sap_links, ctx->sap_clov, r_e, r_o, x_e, x_o, st);
         if (e != cudaSuccess) return check_cuda(ctx, e, "sap_block_kernel attributes");
-        if (ctx->timing) { cudaEventRecord(ev.b, st); ctx->events.push_back(ev); }
         return after_launch(ctx);
     };
     for (int i = 0; i < n; ++i) {
@@ -1199,23 +1225,22 @@ extern "C" int ddamg_power_iteration(ddamg_ctx* ctx, void* v_e, int iters, doubl
     int s = need_ready(ctx, "ddamg_power_iteration");
     if (s != DDAMG_OK) return s;
     cudaStream_t st = ctx->stream;
-    const int vecN = (int)(16 / ctx->real_bytes);
-    const int bgrid = blas_grid(ctx->nreal / vecN);
+    int nblk = 0;
     double* scale = (double*)((char*)ctx->sc + offsetof(Scalars, scale));
     const bool f32 = ctx->prec == DDAMG_F32;
     // v <- v / ||v||
-    if (f32) launch_copy_norm<float>(ctx->nreal, v_e, v_e, ctx->partials, st);
-    else launch_copy_norm<double>(ctx->nreal, v_e, v_e, ctx->partials, st);
-    launch_finalize_norm(ctx->partials, bgrid, ctx->sc, 0, st);
+    nblk = f32 ? launch_copy_norm<float>(ctx->nreal, v_e, v_e, ctx->partials, st)
+               : launch_copy_norm<double>(ctx->nreal, v_e, v_e, ctx->partials, st);
+    launch_finalize_norm(ctx->partials, nblk, ctx->sc, 0, st);
     if (f32) launch_scale_by_dev<float>(ctx->nreal, v_e, scale, st);
     else launch_scale_by_dev<double>(ctx->nreal, v_e, scale, st);
     s = after_launch(ctx, 3); if (s != DDAMG_OK) return s;
     for (int i = 0; i < iters; ++i) {
         s = schur(ctx, v_e, ctx->tmp_e);                                     // w = D_S v
         if (s != DDAMG_OK) return s;
-        if (f32) launch_copy_norm<float>(ctx->nreal, ctx->tmp_e, v_e, ctx->partials, st);   // v = w, |w|^2
-        else launch_copy_norm<double>(ctx->nreal, ctx->tmp_e, v_e, ctx->partials, st);
-        launch_finalize_norm(ctx->partials, bgrid, ctx->sc, 0, st);          // lambda = ||w||
+        nblk = f32 ? launch_copy_norm<float>(ctx->nreal, ctx->tmp_e, v_e, ctx->partials, st)    // v = w, |w|^2
+                   : launch_copy_norm<double>(ctx->nreal, ctx->tmp_e, v_e, ctx->partials, st);
+        launch_finalize_norm(ctx->partials, nblk, ctx->sc, 0, st);           // lambda = ||w||
         if (f32) launch_scale_by_dev<float>(ctx->nreal, v_e, scale, st);
         else launch_scale_by_dev<double>(ctx->nreal, v_e, scale, st);
         s = after_launch(ctx, 3); if (s != DDAMG_OK) return s;
@@ -1267,6 +1292,8 @@ extern "C" int ddamg_set_option(ddamg_ctx* ctx, const char* name, double value)
 extern "C" int ddamg_kernel_timing(ddamg_ctx* ctx, int on)
 {
     ENTER(ctx);
+    if (on && ctx->events.empty() && !grow_event_pool(ctx, EV_POOL_CHUNK))      // all events are created here, not in timed calls
+        return fail(ctx, DDAMG_ECUDA, "ddamg_kernel_timing: cannot create the event pool");
     ctx->timing = on != 0;
     return DDAMG_OK;
 }
@@ -1277,7 +1304,8 @@ extern "C" int ddamg_kernel_time_ms(ddamg_ctx* ctx, int which, double* ms, long 
     CK(cudaStreamSynchronize(ctx->stream));
     double tot = 0.0;
     long long n = 0;
-    for (auto& ev : ctx->events) {
+    for (size_t i = 0; i < ctx->ev_used; ++i) {
+        const ddamg_ctx::Ev& ev = ctx->events[i];
         if (ev.which != which) continue;
         float t = 0.f;
         CK(cudaEventElapsedTime(&t, ev.a, ev.b));
@@ -1286,9 +1314,6 @@ extern "C" int ddamg_kernel_time_ms(ddamg_ctx* ctx, int which, double* ms, long 
     }
     if (ms) *ms = tot;
     if (launches) *launches = n;
-    if (reset) {
-        for (auto& ev : ctx->events) { cudaEventDestroy(ev.a); cudaEventDestroy(ev.b); }
-        ctx->events.clear();
-    }
+    if (reset) ctx->ev_used = 0;          // the pooled events are kept and re-recorded
     return DDAMG_OK;
 }

@@ -3,19 +3,51 @@
 //
 // BLAS-1 kernels see a half-lattice spinor as a flat array of 16-byte vectors; in the native
 // layout the two (fp64: one) complex numbers of a vector are (re, im) pairs, so complex inner
-// products can be formed without knowing the site structure.  All partial sums are fp64;
-// each block writes its partials, a single-block kernel finishes them in a fixed order
+// products can be formed without knowing the site structure.
+//
+// All of them are HBM streams: every kernel is ONE wave of resident CTAs
+// (grid = SMs x occupancy, grid-stride loop), every thread first issues ALL the 16-byte loads of
+// an iteration (NB + 1 vectors; small NB: several elements per iteration) and only then computes,
+// so that ~100 KB per SM are in flight.  fp32 data: the products of one 16-byte vector (4 reals)
+// are formed with fp32 FMAs and folded into fp64 accumulators once per vector -- the fp64 pipe
+// and the F2F conversion pipe see 2 operations per (vector, basis vector) instead of 12; axpy
+// forms are evaluated in fp32 (the result is stored in fp32 anyway).  fp64 data: fp64 throughout.
+// Each block writes its fp64 partials, a single-block kernel finishes them in a fixed order
 // (deterministic), and every scalar (norms, Hessenberg column, Givens rotations, the
 // least-squares solution) stays on the device: no host synchronisation inside a cycle.
 #include "ddamg_internal.h"
 
 namespace ddamg {
 
-int blas_grid(size_t nvec)
+static int sm_count()
 {
-    size_t b = (nvec + BLAS_THREADS - 1) / BLAS_THREADS;
-    const size_t cap = 148 * 8;
-    return (int)(b < cap ? (b ? b : 1) : cap);
+    static int n = 0;
+    if (n == 0) {
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) {
+            cudaGetLastError();
+            n = 148;
+        }
+    }
+    return n;
+}
+
+// upper bound of every BLAS-1 grid (sizes the partial-sum scratch): 2048 resident threads per SM
+int blas_grid_cap() { return sm_count() * (2048 / BLAS_THREADS); }
+
+// one wave: as many CTAs as are resident at once, at most one per BLAS_THREADS * unroll vectors
+template <typename K>
+static int wave_grid(K kernel, size_t nvec, int unroll)
+{
+    int per_sm = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, BLAS_THREADS, 0) != cudaSuccess || per_sm < 1) {
+        cudaGetLastError();
+        per_sm = 1;
+    }
+    const size_t per_cta = (size_t)BLAS_THREADS * unroll;
+    const size_t need = (nvec + per_cta - 1) / per_cta;
+    const size_t cap = (size_t)sm_count() * per_sm;
+    return (int)(need < cap ? (need ? need : 1) : cap);
 }
 
 __device__ __forceinline__ double warp_sum(double v)
@@ -44,8 +76,51 @@ __device__ __forceinline__ void block_sum_n(double (&v)[NV], double* out)
     }
 }
 
-__device__ __forceinline__ void cvt(const float4& v, double (&r)[4]) { r[0] = v.x; r[1] = v.y; r[2] = v.z; r[3] = v.w; }
-__device__ __forceinline__ void cvt(const double2& v, double (&r)[2]) { r[0] = v.x; r[1] = v.y; }
+// ---- per-vector arithmetic in the data precision (fp32 vectors: 4 reals = 2 complex numbers)
+__device__ __forceinline__ float4 ld_once(const float4* p) { return __ldcs(p); }
+__device__ __forceinline__ double2 ld_once(const double2* p) { return __ldcs(p); }
+
+// conj(v) . w over the complex numbers of one vector, added to (ar, ai)
+__device__ __forceinline__ void cdot_add(const float4& v, const float4& w, double& ar, double& ai)
+{
+    float pr = v.x * w.x;
+    pr = fmaf(v.y, w.y, pr); pr = fmaf(v.z, w.z, pr); pr = fmaf(v.w, w.w, pr);
+    float pi = v.x * w.y;
+    pi = fmaf(-v.y, w.x, pi); pi = fmaf(v.z, w.w, pi); pi = fmaf(-v.w, w.z, pi);
+    ar += (double)pr;
+    ai += (double)pi;
+}
+__device__ __forceinline__ void cdot_add(const double2& v, const double2& w, double& ar, double& ai)
+{
+    ar = fma(v.x, w.x, ar); ar = fma(v.y, w.y, ar);
+    ai = fma(v.x, w.y, ai); ai = fma(-v.y, w.x, ai);
+}
+// |v|^2 added to a
+__device__ __forceinline__ void norm_add(const float4& v, double& a)
+{
+    float p = v.x * v.x;
+    p = fmaf(v.y, v.y, p); p = fmaf(v.z, v.z, p); p = fmaf(v.w, v.w, p);
+    a += (double)p;
+}
+__device__ __forceinline__ void norm_add(const double2& v, double& a) { a = fma(v.x, v.x, a); a = fma(v.y, v.y, a); }
+// w += (cr + i ci) v, complex number by complex number
+__device__ __forceinline__ void caxpy(float cr, float ci, const float4& v, float4& w)
+{
+    w.x = fmaf(cr, v.x, w.x); w.x = fmaf(-ci, v.y, w.x);
+    w.y = fmaf(cr, v.y, w.y); w.y = fmaf(ci, v.x, w.y);
+    w.z = fmaf(cr, v.z, w.z); w.z = fmaf(-ci, v.w, w.z);
+    w.w = fmaf(cr, v.w, w.w); w.w = fmaf(ci, v.z, w.w);
+}
+__device__ __forceinline__ void caxpy(double cr, double ci, const double2& v, double2& w)
+{
+    w.x = fma(cr, v.x, w.x); w.x = fma(-ci, v.y, w.x);
+    w.y = fma(cr, v.y, w.y); w.y = fma(ci, v.x, w.y);
+}
+__device__ __forceinline__ void vscale(float s, float4& w) { w.x *= s; w.y *= s; w.z *= s; w.w *= s; }
+__device__ __forceinline__ void vscale(double s, double2& w) { w.x *= s; w.y *= s; }
+
+// elements per thread and iteration: enough independent 16-byte loads in flight for every NB
+__host__ __device__ constexpr int unroll_for(int nloads) { return nloads >= 7 ? 1 : nloads >= 4 ? 2 : nloads >= 2 ? 4 : 8; }
 
 // ------------------------------------------------------------------ norm finish
 __global__ void finalize_norm_kernel(const double* __restrict__ partials, int n, Scalars* sc, int append)
@@ -92,34 +167,42 @@ axpy_norm_kernel(size_t nvec, T alpha, const typename VecOf<T>::type* x,
                  typename VecOf<T>::type* y, double* __restrict__ partials)   // x may alias y
 {
     using V = typename VecOf<T>::type;
-    constexpr int N = VecOf<T>::N;
+    constexpr int U = 8;
     double acc[1] = { 0.0 };
-    for (size_t i = (size_t)blockIdx.x * BLAS_THREADS + threadIdx.x; i < nvec; i += (size_t)gridDim.x * BLAS_THREADS) {
-        const V v = x[i];
-        T r[N];
-        unpack(v, r);
+    const size_t step = (size_t)gridDim.x * BLAS_THREADS * U;
+    for (size_t base = (size_t)blockIdx.x * BLAS_THREADS * U + threadIdx.x; base < nvec; base += step) {
+        V v[U];
 #pragma unroll
-        for (int k = 0; k < N; ++k) { acc[0] += (double)r[k] * (double)r[k]; r[k] *= alpha; }
-        y[i] = pack(r);
+        for (int u = 0; u < U; ++u)
+            if (base + (size_t)u * BLAS_THREADS < nvec) v[u] = x[base + (size_t)u * BLAS_THREADS];
+#pragma unroll
+        for (int u = 0; u < U; ++u)
+            if (base + (size_t)u * BLAS_THREADS < nvec) {
+                norm_add(v[u], acc[0]);
+                vscale(alpha, v[u]);
+                y[base + (size_t)u * BLAS_THREADS] = v[u];
+            }
     }
     if (partials) block_sum_n<1>(acc, partials + blockIdx.x);
 }
 template <typename T>
-void launch_axpy_norm(size_t nreal, double alpha, const void* x, void* y, double* partials, cudaStream_t st)
+int launch_axpy_norm(size_t nreal, double alpha, const void* x, void* y, double* partials, cudaStream_t st)
 {
     using V = typename VecOf<T>::type;
     const size_t nvec = nreal / VecOf<T>::N;
-    axpy_norm_kernel<T><<<blas_grid(nvec), BLAS_THREADS, 0, st>>>(nvec, (T)alpha, (const V*)x, (V*)y, partials);
+    const int grid = wave_grid(axpy_norm_kernel<T>, nvec, 8);
+    axpy_norm_kernel<T><<<grid, BLAS_THREADS, 0, st>>>(nvec, (T)alpha, (const V*)x, (V*)y, partials);
+    return grid;
 }
 template <typename T>
-void launch_copy_norm(size_t nreal, const void* src, void* dst, double* partials, cudaStream_t st)
+int launch_copy_norm(size_t nreal, const void* src, void* dst, double* partials, cudaStream_t st)
 {
-    launch_axpy_norm<T>(nreal, 1.0, src, dst, partials, st);
+    return launch_axpy_norm<T>(nreal, 1.0, src, dst, partials, st);
 }
-template void launch_axpy_norm<float>(size_t, double, const void*, void*, double*, cudaStream_t);
-template void launch_axpy_norm<double>(size_t, double, const void*, void*, double*, cudaStream_t);
-template void launch_copy_norm<float>(size_t, const void*, void*, double*, cudaStream_t);
-template void launch_copy_norm<double>(size_t, const void*, void*, double*, cudaStream_t);
+template int launch_axpy_norm<float>(size_t, double, const void*, void*, double*, cudaStream_t);
+template int launch_axpy_norm<double>(size_t, double, const void*, void*, double*, cudaStream_t);
+template int launch_copy_norm<float>(size_t, const void*, void*, double*, cudaStream_t);
+template int launch_copy_norm<double>(size_t, const void*, void*, double*, cudaStream_t);
 
 // ------------------------------------------------------------------ v *= *scale (device scalar)
 template <typename T>
@@ -127,14 +210,20 @@ __global__ void __launch_bounds__(BLAS_THREADS)
 scale_kernel(size_t nvec, typename VecOf<T>::type* __restrict__ v, const double* __restrict__ scale)
 {
     using V = typename VecOf<T>::type;
-    constexpr int N = VecOf<T>::N;
+    constexpr int U = 8;
     const T s = (T)(*scale);
-    for (size_t i = (size_t)blockIdx.x * BLAS_THREADS + threadIdx.x; i < nvec; i += (size_t)gridDim.x * BLAS_THREADS) {
-        T r[N];
-        unpack(v[i], r);
+    const size_t step = (size_t)gridDim.x * BLAS_THREADS * U;
+    for (size_t base = (size_t)blockIdx.x * BLAS_THREADS * U + threadIdx.x; base < nvec; base += step) {
+        V r[U];
 #pragma unroll
-        for (int k = 0; k < N; ++k) r[k] *= s;
-        v[i] = pack(r);
+        for (int u = 0; u < U; ++u)
+            if (base + (size_t)u * BLAS_THREADS < nvec) r[u] = v[base + (size_t)u * BLAS_THREADS];
+#pragma unroll
+        for (int u = 0; u < U; ++u)
+            if (base + (size_t)u * BLAS_THREADS < nvec) {
+                vscale(s, r[u]);
+                v[base + (size_t)u * BLAS_THREADS] = r[u];
+            }
     }
 }
 template <typename T>
@@ -142,7 +231,7 @@ void launch_scale_by_dev(size_t nreal, void* v, const double* scale, cudaStream_
 {
     using V = typename VecOf<T>::type;
     const size_t nvec = nreal / VecOf<T>::N;
-    scale_kernel<T><<<blas_grid(nvec), BLAS_THREADS, 0, st>>>(nvec, (V*)v, scale);
+    scale_kernel<T><<<wave_grid(scale_kernel<T>, nvec, 8), BLAS_THREADS, 0, st>>>(nvec, (V*)v, scale);
 }
 template void launch_scale_by_dev<float>(size_t, void*, const double*, cudaStream_t);
 template void launch_scale_by_dev<double>(size_t, void*, const double*, cudaStream_t);
@@ -153,40 +242,49 @@ __global__ void __launch_bounds__(BLAS_THREADS)
 multi_dot_kernel(size_t nvec, const typename VecOf<T>::type* __restrict__ V0, size_t vstride,
                  const typename VecOf<T>::type* __restrict__ w, double* __restrict__ partials)
 {
-    constexpr int N = VecOf<T>::N;
+    using V = typename VecOf<T>::type;
+    constexpr int U = unroll_for(NB + 1);
     double acc[2 * NB];
 #pragma unroll
     for (int i = 0; i < 2 * NB; ++i) acc[i] = 0.0;
-    for (size_t i = (size_t)blockIdx.x * BLAS_THREADS + threadIdx.x; i < nvec; i += (size_t)gridDim.x * BLAS_THREADS) {
-        double wr[N];
-        cvt(w[i], wr);
+    const size_t step = (size_t)gridDim.x * BLAS_THREADS * U;
+    for (size_t base = (size_t)blockIdx.x * BLAS_THREADS * U + threadIdx.x; base < nvec; base += step) {
+        V wv[U], vv[U][NB];
 #pragma unroll
-        for (int b = 0; b < NB; ++b) {
-            double vr[N];
-            cvt(V0[(size_t)b * vstride + i], vr);
+        for (int u = 0; u < U; ++u) {
+            const size_t i = base + (size_t)u * BLAS_THREADS;
+            if (i < nvec) {
+                wv[u] = ld_once(w + i);
 #pragma unroll
-            for (int c = 0; c < N; c += 2) {          // conj(v) * w
-                acc[2 * b] += vr[c] * wr[c] + vr[c + 1] * wr[c + 1];
-                acc[2 * b + 1] += vr[c] * wr[c + 1] - vr[c + 1] * wr[c];
+                for (int b = 0; b < NB; ++b) vv[u][b] = ld_once(V0 + (size_t)b * vstride + i);
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            if (base + (size_t)u * BLAS_THREADS < nvec) {
+#pragma unroll
+                for (int b = 0; b < NB; ++b) cdot_add(vv[u][b], wv[u], acc[2 * b], acc[2 * b + 1]);    // conj(v) * w
             }
         }
     }
     block_sum_n<2 * NB>(acc, partials + (size_t)blockIdx.x * 2 * NB);
 }
 template <typename T>
-void launch_multi_dot(size_t nreal, int nb, const void* V, size_t vstride_real, const void* w, double* partials,
-                      cudaStream_t st)
+int launch_multi_dot(size_t nreal, int nb, const void* V, size_t vstride_real, const void* w, double* partials,
+                     cudaStream_t st)
 {
     using VT = typename VecOf<T>::type;
     const size_t nvec = nreal / VecOf<T>::N, vs = vstride_real / VecOf<T>::N;
-    const int grid = blas_grid(nvec);
-#define MD(NB) case NB: multi_dot_kernel<T, NB><<<grid, BLAS_THREADS, 0, st>>>(nvec, (const VT*)V, vs, (const VT*)w, partials); break;
+    int grid = 0;
+#define MD(NB) case NB: grid = wave_grid(multi_dot_kernel<T, NB>, nvec, unroll_for(NB + 1)); \
+        multi_dot_kernel<T, NB><<<grid, BLAS_THREADS, 0, st>>>(nvec, (const VT*)V, vs, (const VT*)w, partials); break;
     switch (nb) { MD(1) MD(2) MD(3) MD(4) MD(5) MD(6) MD(7) MD(8) MD(9) MD(10) MD(11) MD(12) }
     static_assert(MDOT_NB == 12, "one case per NB");
 #undef MD
+    return grid;
 }
-template void launch_multi_dot<float>(size_t, int, const void*, size_t, const void*, double*, cudaStream_t);
-template void launch_multi_dot<double>(size_t, int, const void*, size_t, const void*, double*, cudaStream_t);
+template int launch_multi_dot<float>(size_t, int, const void*, size_t, const void*, double*, cudaStream_t);
+template int launch_multi_dot<double>(size_t, int, const void*, size_t, const void*, double*, cudaStream_t);
 
 // hcol[first .. first+nb-1] = sum over blocks; negh = -hcol.  One warp per real component,
 // lanes stride over the blocks, fixed shuffle tree: deterministic.
@@ -232,56 +330,61 @@ void launch_finalize_dots_lazy(const double* partials, int nblocks, int nb, Scal
     finalize_dots_lazy_kernel<<<1, 32 * 2 * MDOT_NB, 0, st>>>(partials, nblocks, nb, sc, first, j);
 }
 
-// ------------------------------------------------------------------ w += sum_i coef_i v_i  (+ |w|^2)
+// ------------------------------------------------------------------ w <- ws w + sum_i coef_i v_i  (+ |w|^2)
 template <typename T, int NB>
 __global__ void __launch_bounds__(BLAS_THREADS)
 multi_axpy_kernel(size_t nvec, const typename VecOf<T>::type* __restrict__ V0, size_t vstride,
                   const double* __restrict__ coef, typename VecOf<T>::type* __restrict__ w,
                   double* __restrict__ partials, const double* __restrict__ wscale)
 {
-    constexpr int N = VecOf<T>::N;
-    double cr[NB], ci[NB];
+    using V = typename VecOf<T>::type;
+    constexpr int U = unroll_for(NB + 1);
+    T cr[NB], ci[NB];
 #pragma unroll
-    for (int b = 0; b < NB; ++b) { cr[b] = coef[2 * b]; ci[b] = coef[2 * b + 1]; }
-    const double ws = wscale ? *wscale : 1.0;        // w <- ws * w + sum_i coef_i v_i
+    for (int b = 0; b < NB; ++b) { cr[b] = (T)coef[2 * b]; ci[b] = (T)coef[2 * b + 1]; }
+    const T ws = wscale ? (T)(*wscale) : (T)1;
     double acc[1] = { 0.0 };
-    for (size_t i = (size_t)blockIdx.x * BLAS_THREADS + threadIdx.x; i < nvec; i += (size_t)gridDim.x * BLAS_THREADS) {
-        double wr[N];
-        cvt(w[i], wr);
-        if (wscale) {
+    const size_t step = (size_t)gridDim.x * BLAS_THREADS * U;
+    for (size_t base = (size_t)blockIdx.x * BLAS_THREADS * U + threadIdx.x; base < nvec; base += step) {
+        V wv[U], vv[U][NB];
 #pragma unroll
-            for (int c = 0; c < N; ++c) wr[c] *= ws;
-        }
+        for (int u = 0; u < U; ++u) {
+            const size_t i = base + (size_t)u * BLAS_THREADS;
+            if (i < nvec) {
+                wv[u] = w[i];
 #pragma unroll
-        for (int b = 0; b < NB; ++b) {
-            double vr[N];
-            cvt(V0[(size_t)b * vstride + i], vr);
-#pragma unroll
-            for (int c = 0; c < N; c += 2) {
-                wr[c] += cr[b] * vr[c] - ci[b] * vr[c + 1];
-                wr[c + 1] += cr[b] * vr[c + 1] + ci[b] * vr[c];
+                for (int b = 0; b < NB; ++b) vv[u][b] = ld_once(V0 + (size_t)b * vstride + i);
             }
         }
-        T o[N];
 #pragma unroll
-        for (int c = 0; c < N; ++c) { o[c] = (T)wr[c]; acc[0] += (double)o[c] * (double)o[c]; }
-        w[i] = pack(o);
+        for (int u = 0; u < U; ++u) {
+            const size_t i = base + (size_t)u * BLAS_THREADS;
+            if (i < nvec) {
+                if (wscale) vscale(ws, wv[u]);
+#pragma unroll
+                for (int b = 0; b < NB; ++b) caxpy(cr[b], ci[b], vv[u][b], wv[u]);
+                norm_add(wv[u], acc[0]);
+                w[i] = wv[u];
+            }
+        }
     }
     if (partials) block_sum_n<1>(acc, partials + blockIdx.x);
 }
 template <typename T>
-void launch_multi_axpy(size_t nreal, int nb, const void* V, size_t vstride_real, const double* coef, void* w,
-                       double* partials, cudaStream_t st, const double* wscale)
+int launch_multi_axpy(size_t nreal, int nb, const void* V, size_t vstride_real, const double* coef, void* w,
+                      double* partials, cudaStream_t st, const double* wscale)
 {
     using VT = typename VecOf<T>::type;
     const size_t nvec = nreal / VecOf<T>::N, vs = vstride_real / VecOf<T>::N;
-    const int grid = blas_grid(nvec);
-#define MA(NB) case NB: multi_axpy_kernel<T, NB><<<grid, BLAS_THREADS, 0, st>>>(nvec, (const VT*)V, vs, coef, (VT*)w, partials, wscale); break;
+    int grid = 0;
+#define MA(NB) case NB: grid = wave_grid(multi_axpy_kernel<T, NB>, nvec, unroll_for(NB + 1)); \
+        multi_axpy_kernel<T, NB><<<grid, BLAS_THREADS, 0, st>>>(nvec, (const VT*)V, vs, coef, (VT*)w, partials, wscale); break;
     switch (nb) { MA(1) MA(2) MA(3) MA(4) MA(5) MA(6) MA(7) MA(8) MA(9) MA(10) MA(11) MA(12) }
 #undef MA
+    return grid;
 }
-template void launch_multi_axpy<float>(size_t, int, const void*, size_t, const double*, void*, double*, cudaStream_t, const double*);
-template void launch_multi_axpy<double>(size_t, int, const void*, size_t, const double*, void*, double*, cudaStream_t, const double*);
+template int launch_multi_axpy<float>(size_t, int, const void*, size_t, const double*, void*, double*, cudaStream_t, const double*);
+template int launch_multi_axpy<double>(size_t, int, const void*, size_t, const double*, void*, double*, cudaStream_t, const double*);
 
 // ------------------------------------------------------------------ GCR (Alg. 3)
 // lines 11-14 in one pass:  z = w + sum_j beta_j z_j  (in place on w),  p = r + sum_j beta_j p_j,
@@ -295,64 +398,66 @@ gcr_form_kernel(size_t nvec, const typename VecOf<T>::type* __restrict__ Z0,
                 const typename VecOf<T>::type* __restrict__ r, typename VecOf<T>::type* __restrict__ p_out,
                 int init_p, double* __restrict__ partials)
 {
-    constexpr int N = VecOf<T>::N;
-    double cr[NB > 0 ? NB : 1], ci[NB > 0 ? NB : 1];
+    using V = typename VecOf<T>::type;
+    constexpr int NBA = NB > 0 ? NB : 1;
+    constexpr int U = unroll_for(2 * NB + 3);
+    T cr[NBA], ci[NBA];
 #pragma unroll
-    for (int b = 0; b < NB; ++b) { cr[b] = coef[2 * b]; ci[b] = coef[2 * b + 1]; }
+    for (int b = 0; b < NB; ++b) { cr[b] = (T)coef[2 * b]; ci[b] = (T)coef[2 * b + 1]; }
     double acc[3] = { 0.0, 0.0, 0.0 };
-    for (size_t i = (size_t)blockIdx.x * BLAS_THREADS + threadIdx.x; i < nvec; i += (size_t)gridDim.x * BLAS_THREADS) {
-        double zr[N], pr[N], rr[N];
-        cvt(z_io[i], zr);
-        cvt(r[i], rr);
-        if (init_p) {
+    const size_t step = (size_t)gridDim.x * BLAS_THREADS * U;
+    for (size_t base = (size_t)blockIdx.x * BLAS_THREADS * U + threadIdx.x; base < nvec; base += step) {
+        V zv[U], rv[U], pv[U], zb[U][NBA], pb[U][NBA];
 #pragma unroll
-            for (int c = 0; c < N; ++c) pr[c] = rr[c];
-        } else {
-            cvt(p_out[i], pr);
-        }
+        for (int u = 0; u < U; ++u) {
+            const size_t i = base + (size_t)u * BLAS_THREADS;
+            if (i < nvec) {
+                zv[u] = z_io[i];
+                rv[u] = r[i];
+                if (!init_p) pv[u] = p_out[i];
 #pragma unroll
-        for (int b = 0; b < NB; ++b) {
-            double zv[N], pv[N];
-            cvt(Z0[(size_t)b * vstride + i], zv);
-            cvt(P0[(size_t)b * vstride + i], pv);
-#pragma unroll
-            for (int c = 0; c < N; c += 2) {
-                zr[c] += cr[b] * zv[c] - ci[b] * zv[c + 1];
-                zr[c + 1] += cr[b] * zv[c + 1] + ci[b] * zv[c];
-                pr[c] += cr[b] * pv[c] - ci[b] * pv[c + 1];
-                pr[c + 1] += cr[b] * pv[c + 1] + ci[b] * pv[c];
+                for (int b = 0; b < NB; ++b) {
+                    zb[u][b] = ld_once(Z0 + (size_t)b * vstride + i);
+                    pb[u][b] = ld_once(P0 + (size_t)b * vstride + i);
+                }
             }
         }
-        T zo[N], po[N];
 #pragma unroll
-        for (int c = 0; c < N; ++c) { zo[c] = (T)zr[c]; po[c] = (T)pr[c]; }
-        if (NB > 0) z_io[i] = pack(zo);
-        p_out[i] = pack(po);
-        if (partials) {
+        for (int u = 0; u < U; ++u) {
+            const size_t i = base + (size_t)u * BLAS_THREADS;
+            if (i < nvec) {
+                if (init_p) pv[u] = rv[u];
 #pragma unroll
-            for (int c = 0; c < N; c += 2) {              // conj(z) * r
-                const double a = zo[c], bq = zo[c + 1];
-                acc[0] += a * a + bq * bq;
-                acc[1] += a * rr[c] + bq * rr[c + 1];
-                acc[2] += a * rr[c + 1] - bq * rr[c];
+                for (int b = 0; b < NB; ++b) {
+                    caxpy(cr[b], ci[b], zb[u][b], zv[u]);
+                    caxpy(cr[b], ci[b], pb[u][b], pv[u]);
+                }
+                if (NB > 0) z_io[i] = zv[u];
+                p_out[i] = pv[u];
+                if (partials) {
+                    norm_add(zv[u], acc[0]);
+                    cdot_add(zv[u], rv[u], acc[1], acc[2]);          // conj(z) * r
+                }
             }
         }
     }
     if (partials) block_sum_n<3>(acc, partials + (size_t)blockIdx.x * 3);
 }
 template <typename T>
-void launch_gcr_form(size_t nreal, int nb, const void* Z0, const void* P0, size_t vstride_real, const double* coef,
-                     void* z_io, const void* r, void* p_out, int init_p, double* partials, cudaStream_t st)
+int launch_gcr_form(size_t nreal, int nb, const void* Z0, const void* P0, size_t vstride_real, const double* coef,
+                    void* z_io, const void* r, void* p_out, int init_p, double* partials, cudaStream_t st)
 {
     using VT = typename VecOf<T>::type;
     const size_t nvec = nreal / VecOf<T>::N, vs = vstride_real / VecOf<T>::N;
-    const int grid = blas_grid(nvec);
-#define GF(NB) case NB: gcr_form_kernel<T, NB><<<grid, BLAS_THREADS, 0, st>>>(nvec, (const VT*)Z0, (const VT*)P0, vs, coef, (VT*)z_io, (const VT*)r, (VT*)p_out, init_p, partials); break;
+    int grid = 0;
+#define GF(NB) case NB: grid = wave_grid(gcr_form_kernel<T, NB>, nvec, unroll_for(2 * NB + 3)); \
+        gcr_form_kernel<T, NB><<<grid, BLAS_THREADS, 0, st>>>(nvec, (const VT*)Z0, (const VT*)P0, vs, coef, (VT*)z_io, (const VT*)r, (VT*)p_out, init_p, partials); break;
     switch (nb) { GF(0) GF(1) GF(2) GF(3) GF(4) GF(5) GF(6) GF(7) GF(8) GF(9) GF(10) GF(11) GF(12) }
 #undef GF
+    return grid;
 }
-template void launch_gcr_form<float>(size_t, int, const void*, const void*, size_t, const double*, void*, const void*, void*, int, double*, cudaStream_t);
-template void launch_gcr_form<double>(size_t, int, const void*, const void*, size_t, const double*, void*, const void*, void*, int, double*, cudaStream_t);
+template int launch_gcr_form<float>(size_t, int, const void*, const void*, size_t, const double*, void*, const void*, void*, int, double*, cudaStream_t);
+template int launch_gcr_form<double>(size_t, int, const void*, const void*, size_t, const double*, void*, const void*, void*, int, double*, cudaStream_t);
 
 // lines 6-7: delta_j = sum |z|^2, alpha = <z, r> / delta_j  (partials[block][3] from gcr_form)
 __global__ void gcr_alpha_kernel(const double* __restrict__ partials, int nblocks, Scalars* sc, int j)
@@ -395,37 +500,44 @@ gcr_update_kernel(size_t nvec, const double* __restrict__ alpha, const typename 
                   const typename VecOf<T>::type* __restrict__ z, typename VecOf<T>::type* __restrict__ x,
                   typename VecOf<T>::type* __restrict__ r, double* __restrict__ partials)
 {
-    constexpr int N = VecOf<T>::N;
-    const double ar = alpha[0], ai = alpha[1];
+    using V = typename VecOf<T>::type;
+    constexpr int U = 2;
+    const T ar = (T)alpha[0], ai = (T)alpha[1];
     double acc[1] = { 0.0 };
-    for (size_t i = (size_t)blockIdx.x * BLAS_THREADS + threadIdx.x; i < nvec; i += (size_t)gridDim.x * BLAS_THREADS) {
-        double xv[N], rv[N], pv[N], zv[N];
-        cvt(x[i], xv); cvt(r[i], rv); cvt(p[i], pv); cvt(z[i], zv);
-        T xo[N], ro[N];
+    const size_t step = (size_t)gridDim.x * BLAS_THREADS * U;
+    for (size_t base = (size_t)blockIdx.x * BLAS_THREADS * U + threadIdx.x; base < nvec; base += step) {
+        V xv[U], rv[U], pv[U], zv[U];
 #pragma unroll
-        for (int c = 0; c < N; c += 2) {
-            xo[c] = (T)(xv[c] + ar * pv[c] - ai * pv[c + 1]);
-            xo[c + 1] = (T)(xv[c + 1] + ar * pv[c + 1] + ai * pv[c]);
-            ro[c] = (T)(rv[c] - (ar * zv[c] - ai * zv[c + 1]));
-            ro[c + 1] = (T)(rv[c + 1] - (ar * zv[c + 1] + ai * zv[c]));
+        for (int u = 0; u < U; ++u) {
+            const size_t i = base + (size_t)u * BLAS_THREADS;
+            if (i < nvec) { xv[u] = x[i]; rv[u] = r[i]; pv[u] = ld_once(p + i); zv[u] = ld_once(z + i); }
         }
 #pragma unroll
-        for (int c = 0; c < N; ++c) acc[0] += (double)ro[c] * (double)ro[c];
-        x[i] = pack(xo);
-        r[i] = pack(ro);
+        for (int u = 0; u < U; ++u) {
+            const size_t i = base + (size_t)u * BLAS_THREADS;
+            if (i < nvec) {
+                caxpy(ar, ai, pv[u], xv[u]);
+                caxpy(-ar, -ai, zv[u], rv[u]);
+                norm_add(rv[u], acc[0]);
+                x[i] = xv[u];
+                r[i] = rv[u];
+            }
+        }
     }
     block_sum_n<1>(acc, partials + blockIdx.x);
 }
 template <typename T>
-void launch_gcr_update(size_t nreal, const double* alpha, const void* p, const void* z, void* x, void* r,
-                       double* partials, cudaStream_t st)
+int launch_gcr_update(size_t nreal, const double* alpha, const void* p, const void* z, void* x, void* r,
+                      double* partials, cudaStream_t st)
 {
     using VT = typename VecOf<T>::type;
     const size_t nvec = nreal / VecOf<T>::N;
-    gcr_update_kernel<T><<<blas_grid(nvec), BLAS_THREADS, 0, st>>>(nvec, alpha, (const VT*)p, (const VT*)z, (VT*)x, (VT*)r, partials);
+    const int grid = wave_grid(gcr_update_kernel<T>, nvec, 2);
+    gcr_update_kernel<T><<<grid, BLAS_THREADS, 0, st>>>(nvec, alpha, (const VT*)p, (const VT*)z, (VT*)x, (VT*)r, partials);
+    return grid;
 }
-template void launch_gcr_update<float>(size_t, const double*, const void*, const void*, void*, void*, double*, cudaStream_t);
-template void launch_gcr_update<double>(size_t, const double*, const void*, const void*, void*, void*, double*, cudaStream_t);
+template int launch_gcr_update<float>(size_t, const double*, const void*, const void*, void*, void*, double*, cudaStream_t);
+template int launch_gcr_update<double>(size_t, const double*, const void*, const void*, void*, void*, double*, cudaStream_t);
 
 // ------------------------------------------------------------------ small dense part (1 thread)
 __global__ void gmres_begin_cycle_kernel(Scalars* sc)

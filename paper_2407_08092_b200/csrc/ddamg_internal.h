@@ -81,9 +81,14 @@ template <typename T>
 void launch_unpack_spinor(const Geom& g, const void* x_e, const void* x_o, void* nat, cudaStream_t st);
 template <typename T>
 void launch_batch_interleave(const Geom& g, int nrhs, bool to_batch, void* halves, void* X, cudaStream_t st);
+// fast path (unpivoted LDL^H; *need_pivot_flag is raised when a block needs the pivoted rebuild) and the
+// pivoted Gauss-Jordan build (*singular_flag raised for a numerically singular block)
 template <typename T>
 void launch_build_clover(const Geom& g, double csw, double m0, const void* gauge, void* clov_e, void* clov_o,
-                         void* clov_o_plain, int* singular_flag, cudaStream_t st);
+                         void* clov_o_plain, int* need_pivot_flag, cudaStream_t st);
+template <typename T>
+void launch_build_clover_pivoted(const Geom& g, double csw, double m0, const void* gauge, void* clov_e, void* clov_o,
+                                 void* clov_o_plain, int* singular_flag, cudaStream_t st);
 template <typename T>
 void launch_get_clover(const Geom& g, const void* clov_e, const void* clov_o, void* A_nat, void* Ainv_nat,
                        cudaStream_t st);
@@ -107,35 +112,38 @@ struct Scalars {
     int nhist;
 };
 
-int blas_grid(size_t nvec);
+// Every BLAS-1 launch below is one wave of resident CTAs; the functions that write per-block
+// partial sums RETURN their grid (= number of partial blocks, <= blas_grid_cap()) for the
+// finalize_* kernel that follows.
+int blas_grid_cap();
 // dst = sqrt(sum partials); stores into sc->value, optionally appends to sc->hist, sets sc->scale = 1/value
 void launch_finalize_norm(const double* partials, int n, Scalars* sc, int append_hist, cudaStream_t st);
 void launch_finalize_norm_batch(const double* partials, int nblocks, int nrhs, Scalars* sc, int offset, cudaStream_t st);
 template <typename T>
-void launch_copy_norm(size_t nreal, const void* src, void* dst, double* partials, cudaStream_t st);
+int launch_copy_norm(size_t nreal, const void* src, void* dst, double* partials, cudaStream_t st);
 template <typename T>
 void launch_scale_by_dev(size_t nreal, void* v, const double* scale, cudaStream_t st);
 template <typename T>
-void launch_axpy_norm(size_t nreal, double alpha, const void* x, void* y, double* partials, cudaStream_t st); // y = alpha*x (+norm of x)
+int launch_axpy_norm(size_t nreal, double alpha, const void* x, void* y, double* partials, cudaStream_t st); // y = alpha*x (+norm of x)
 // partial complex dots <v_i, w>, i = 0..nb-1 (nb <= MDOT_NB): partials[block][2*nb]
 template <typename T>
-void launch_multi_dot(size_t nreal, int nb, const void* V, size_t vstride_real, const void* w, double* partials,
+int launch_multi_dot(size_t nreal, int nb, const void* V, size_t vstride_real, const void* w, double* partials,
                       cudaStream_t st);
 void launch_finalize_dots(const double* partials, int nblocks, int nb, Scalars* sc, int first, cudaStream_t st);
 void launch_finalize_dots_lazy(const double* partials, int nblocks, int nb, Scalars* sc, int first, int j, cudaStream_t st);
 // w <- (*wscale) w + sum_i coef[i] v_i (complex coef and real wscale on device, nb <= MDOT_NB;
 // wscale NULL = 1); optional |w|^2 partials
 template <typename T>
-void launch_multi_axpy(size_t nreal, int nb, const void* V, size_t vstride_real, const double* coef, void* w,
+int launch_multi_axpy(size_t nreal, int nb, const void* V, size_t vstride_real, const double* coef, void* w,
                        double* partials, cudaStream_t st, const double* wscale = nullptr);
 // GCR (Alg. 3)
 template <typename T>
-void launch_gcr_form(size_t nreal, int nb, const void* Z0, const void* P0, size_t vstride_real, const double* coef,
+int launch_gcr_form(size_t nreal, int nb, const void* Z0, const void* P0, size_t vstride_real, const double* coef,
                      void* z_io, const void* r, void* p_out, int init_p, double* partials, cudaStream_t st);
 void launch_gcr_alpha(const double* partials, int nblocks, Scalars* sc, int j, cudaStream_t st);
 void launch_gcr_beta(Scalars* sc, int first, int nb, cudaStream_t st);
 template <typename T>
-void launch_gcr_update(size_t nreal, const double* alpha, const void* p, const void* z, void* x, void* r,
+int launch_gcr_update(size_t nreal, const double* alpha, const void* p, const void* z, void* x, void* r,
                        double* partials, cudaStream_t st);
 void launch_gmres_begin_cycle(Scalars* sc, cudaStream_t st);                 // g = beta e_1 (beta = sc->value)
 void launch_gmres_givens(Scalars* sc, int j, cudaStream_t st);               // after the norm of w is in sc->value

@@ -91,13 +91,19 @@ __global__ void compress_gauge_kernel(Geom g, int bc, const T* __restrict__ gaug
             const T sgn = (bc == 1 && mu == 3 && s.t == g.T - 1) ? (T)-1 : (T)1;
             reconstruct_row2<T>(sgn, v);
 #pragma unroll
-            for (int k = 12; k < 18; ++k) dev = fmaxf(dev, fabsf((float)(v[k] - u[k])));
+            for (int k = 12; k < 18; ++k) {
+                const float d = fabsf((float)(v[k] - u[k]));
+                dev = (d > dev || !(d == d)) ? d : dev;          // NaN-propagating max (fmaxf would drop a NaN)
+            }
             store_link12(gauge12 + ((size_t)parity * 4 + mu) * (size_t)12 * g.Vh, g.Vh, cb, u);
         }
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) dev = fmaxf(dev, __shfl_xor_sync(0xffffffffu, dev, o));
-    if ((threadIdx.x & 31) == 0 && dev > 0.f) atomicMax(dev_max_bits, __float_as_uint(dev));
+    // fmaxf drops NaNs: a non-finite link must not pass as "deviation 0", so it is reported as +Inf
+    bool bad = !isfinite(dev);
+    bad = __any_sync(0xffffffffu, bad);
+    if ((threadIdx.x & 31) == 0 && (bad || dev > 0.f)) atomicMax(dev_max_bits, bad ? 0x7f800000u : __float_as_uint(dev));
 }
 
 template <typename T>
@@ -307,7 +313,7 @@ __device__ bool invert6(double (&mr)[6][6], double (&mi)[6][6])
 }
 
 template <typename T>
-__global__ void build_clover_kernel(Geom g, double csw, double m0, const T* __restrict__ gauge,
+__global__ void build_clover_pivoted_kernel(Geom g, double csw, double m0, const T* __restrict__ gauge,
                                     T* __restrict__ clov_e, T* __restrict__ clov_o, T* __restrict__ clov_o_plain,
                                     int* singular)
 {
@@ -386,16 +392,295 @@ __global__ void build_clover_kernel(Geom g, double csw, double m0, const T* __re
     }
 }
 
+
+// ---- a1, fast path.  One CTA = CLOV_SITES sites x 3 thread groups; group k (warp-uniform) forms the two
+// field strengths of the plane pair k  (F'_ij, F'_kt; (i, j, k) cyclic)  for its site with all 3x3
+// products fully unrolled in fp64 registers (no local arrays), and leaves the two Hermitian 3x3 matrices
+// G^-+_k = i (F'_ij -+ F'_kt)  in shared memory.  Groups 0 / 1 then assemble the upper / lower chirality block
+//   A = [[c - kap G_z, -kap (G_x - i G_y)], [-kap (G_x + i G_y), c + kap G_z]],  c = m0 + 4, kap = csw / 16,
+// directly in the packed Hermitian format and, on odd sites, invert it by an unpivoted LDL^H in registers.
+// A pivot below 1e-2 * max|A_ij| (never the case for a clover block with its dominant diagonal; possible for
+// an indefinite or singular block) raises *need_pivot: the host then rebuilds everything with the pivoted
+// Gauss-Jordan kernel above, which also decides DDAMG_ESINGULAR (reading C6: pivot < 1e-12 ||block||).
+constexpr int CLOV_SITES = 64;
+
+struct M3d { double re[9], im[9]; };
+struct X4 { int x, y, z, t; };
+
+__device__ __forceinline__ X4 shift4(const Geom& g, X4 c, int mu, int d)
+{
+    if (mu == 0) { c.x += d; c.x = c.x < 0 ? c.x + g.L : (c.x >= g.L ? c.x - g.L : c.x); }
+    else if (mu == 1) { c.y += d; c.y = c.y < 0 ? c.y + g.L : (c.y >= g.L ? c.y - g.L : c.y); }
+    else if (mu == 2) { c.z += d; c.z = c.z < 0 ? c.z + g.L : (c.z >= g.L ? c.z - g.L : c.z); }
+    else { c.t += d; c.t = c.t < 0 ? c.t + g.T : (c.t >= g.T ? c.t - g.T : c.t); }
+    return c;
+}
+
+// links are re-read by the neighbouring sites' leaves: cacheable loads (not the streaming ones of the hot path)
+__device__ __forceinline__ void link_cached(const Geom& g, const float* __restrict__ gauge, const X4& c, int mu, M3d& m)
+{
+    const int par = (c.x + c.y + c.z + c.t) & 1;
+    const int cb = (c.x >> 1) + g.Lh * (c.y + g.L * (c.z + g.L * c.t));
+    const float* blk = gauge + ((size_t)par * 4 + mu) * (size_t)18 * g.Vh;
+    const float4* p4 = reinterpret_cast<const float4*>(blk) + cb;
+    float u[18];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) unpack(__ldg(p4 + (size_t)k * g.Vh), &u[4 * k]);
+    const float2 v = __ldg(reinterpret_cast<const float2*>(blk + (size_t)16 * g.Vh) + cb);
+    u[16] = v.x; u[17] = v.y;
+#pragma unroll
+    for (int k = 0; k < 9; ++k) { m.re[k] = (double)u[2 * k]; m.im[k] = (double)u[2 * k + 1]; }
+}
+__device__ __forceinline__ void link_cached(const Geom& g, const double* __restrict__ gauge, const X4& c, int mu, M3d& m)
+{
+    const int par = (c.x + c.y + c.z + c.t) & 1;
+    const int cb = (c.x >> 1) + g.Lh * (c.y + g.L * (c.z + g.L * c.t));
+    const double2* p = reinterpret_cast<const double2*>(gauge + ((size_t)par * 4 + mu) * (size_t)18 * g.Vh) + cb;
+#pragma unroll
+    for (int k = 0; k < 9; ++k) { const double2 v = __ldg(p + (size_t)k * g.Vh); m.re[k] = v.x; m.im[k] = v.y; }
+}
+
+// c = op(a) * op(b), fully unrolled (every index is a compile-time constant: registers only)
+template <bool DA, bool DB>
+__device__ __forceinline__ void mm_u(const M3d& a, const M3d& b, M3d& c)
+{
+#pragma unroll
+    for (int i = 0; i < 3; ++i)
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+            double sr = 0.0, si = 0.0;
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                const int ia = DA ? 3 * k + i : 3 * i + k;
+                const int ib = DB ? 3 * j + k : 3 * k + j;
+                const double ar = a.re[ia], ai = DA ? -a.im[ia] : a.im[ia];
+                const double br = b.re[ib], bi = DB ? -b.im[ib] : b.im[ib];
+                sr = fma(ar, br, sr); sr = fma(-ai, bi, sr);
+                si = fma(ar, bi, si); si = fma(ai, br, si);
+            }
+            c.re[3 * i + j] = sr;
+            c.im[3 * i + j] = si;
+        }
+}
+
+// Q += op(U1) op(U2) op(U3) op(U4) with U_n = U_{d_n}(s_n)
+template <bool D1, bool D2, bool D3, bool D4, typename T>
+__device__ __forceinline__ void leaf(const Geom& g, const T* __restrict__ gauge, const X4& s1, int d1, const X4& s2, int d2,
+                                     const X4& s3, int d3, const X4& s4, int d4, M3d& Q)
+{
+    M3d a, b, t;
+    link_cached(g, gauge, s1, d1, a);
+    link_cached(g, gauge, s2, d2, b);
+    mm_u<D1, D2>(a, b, t);
+    link_cached(g, gauge, s3, d3, a);
+    mm_u<false, D3>(t, a, b);
+    link_cached(g, gauge, s4, d4, a);
+    mm_u<false, D4>(b, a, t);
+#pragma unroll
+    for (int k = 0; k < 9; ++k) { Q.re[k] += t.re[k]; Q.im[k] += t.im[k]; }
+}
+
+// F'_{mu nu}(x) = Q - Q^H (anti-Hermitian), Q = sum of the four leaves at x (reading R4).  Returned as the 9 reals
+// f[0..2] = Im F_aa,  f[3 + 2 e], f[4 + 2 e] = Re, Im of the strictly-lower entries e = (1,0), (2,0), (2,1).
+template <typename T>
+__device__ __forceinline__ void field_strength_u(const Geom& g, const T* __restrict__ gauge, const X4& x, int mu, int nu,
+                                                 double (&f)[9])
+{
+    M3d Q;
+#pragma unroll
+    for (int k = 0; k < 9; ++k) Q.re[k] = Q.im[k] = 0.0;
+    const X4 xpm = shift4(g, x, mu, +1), xpn = shift4(g, x, nu, +1);
+    const X4 xmm = shift4(g, x, mu, -1), xmn = shift4(g, x, nu, -1);
+    const X4 xmm_pn = shift4(g, xmm, nu, +1), xmm_mn = shift4(g, xmm, nu, -1), xpm_mn = shift4(g, xpm, nu, -1);
+    leaf<false, false, true, true>(g, gauge, x, mu, xpm, nu, xpn, mu, x, nu, Q);           // U_mu(x) U_nu(x+mu) U_mu(x+nu)^H U_nu(x)^H
+    leaf<false, true, true, false>(g, gauge, x, nu, xmm_pn, mu, xmm, nu, xmm, mu, Q);      // U_nu(x) U_mu(x-mu+nu)^H U_nu(x-mu)^H U_mu(x-mu)
+    leaf<true, true, false, false>(g, gauge, xmm, mu, xmm_mn, nu, xmm_mn, mu, xmn, nu, Q); // U_mu(x-mu)^H U_nu(x-mu-nu)^H U_mu(x-mu-nu) U_nu(x-nu)
+    leaf<true, false, false, true>(g, gauge, xmn, nu, xmn, mu, xpm_mn, nu, x, mu, Q);      // U_nu(x-nu)^H U_mu(x-nu) U_nu(x+mu-nu) U_mu(x)^H
+#pragma unroll
+    for (int a = 0; a < 3; ++a) f[a] = 2.0 * Q.im[4 * a];
+    f[3] = Q.re[3] - Q.re[1]; f[4] = Q.im[3] + Q.im[1];      // (1,0)
+    f[5] = Q.re[6] - Q.re[2]; f[6] = Q.im[6] + Q.im[2];      // (2,0)
+    f[7] = Q.re[7] - Q.re[5]; f[8] = Q.im[7] + Q.im[5];      // (2,1)
+}
+
+// packed Hermitian 6x6 (6 real diagonal entries, 15 complex strictly-lower entries row by row)
+__host__ __device__ constexpr int pk(int i, int j) { return 6 + 2 * (i * (i - 1) / 2 + j); }
+
+// In-place inverse of a packed Hermitian 6x6 by unpivoted LDL^H; false if a pivot is below 1e-2 * max|entry|.
+__device__ __forceinline__ bool invert6_ldl(double (&p)[36])
+{
+    double scale = 0.0;
+#pragma unroll
+    for (int i = 0; i < 6; ++i) scale = fmax(scale, fabs(p[i]));
+#pragma unroll
+    for (int k = 6; k < 36; ++k) scale = fmax(scale, fabs(p[k]));
+    double Lr[6][6], Li[6][6], D[6], Di[6];
+    bool ok = true;
+#pragma unroll
+    for (int j = 0; j < 6; ++j) {
+        double d = p[j];
+#pragma unroll
+        for (int k = 0; k < j; ++k) d -= (Lr[j][k] * Lr[j][k] + Li[j][k] * Li[j][k]) * D[k];
+        D[j] = d;
+        ok = ok && (fabs(d) > 1e-2 * scale);
+        Di[j] = 1.0 / d;
+#pragma unroll
+        for (int i = j + 1; i < 6; ++i) {
+            double sr = p[pk(i, j)], si = p[pk(i, j) + 1];
+#pragma unroll
+            for (int k = 0; k < j; ++k) {
+                // L_ik D_k conj(L_jk)
+                const double tr = Lr[i][k] * D[k], ti = Li[i][k] * D[k];
+                sr -= tr * Lr[j][k] + ti * Li[j][k];
+                si -= ti * Lr[j][k] - tr * Li[j][k];
+            }
+            Lr[i][j] = sr * Di[j];
+            Li[i][j] = si * Di[j];
+        }
+    }
+    // M = L^-1 (unit lower triangular), in place column by column
+    double Mr[6][6], Mi[6][6];
+#pragma unroll
+    for (int j = 0; j < 6; ++j)
+#pragma unroll
+        for (int i = j + 1; i < 6; ++i) {
+            double sr = Lr[i][j], si = Li[i][j];
+#pragma unroll
+            for (int k = j + 1; k < i; ++k) {
+                sr += Lr[i][k] * Mr[k][j] - Li[i][k] * Mi[k][j];
+                si += Lr[i][k] * Mi[k][j] + Li[i][k] * Mr[k][j];
+            }
+            Mr[i][j] = -sr;
+            Mi[i][j] = -si;
+        }
+    // A^-1 = M^H D^-1 M:  (i, j), i >= j:  sum_{k >= i} conj(M_ki) M_kj / D_k,  M_kk = 1
+#pragma unroll
+    for (int i = 0; i < 6; ++i) {
+        double d = Di[i];
+#pragma unroll
+        for (int k = i + 1; k < 6; ++k) d += (Mr[k][i] * Mr[k][i] + Mi[k][i] * Mi[k][i]) * Di[k];
+        p[i] = d;
+#pragma unroll
+        for (int j = 0; j < i; ++j) {
+            double sr = Mr[i][j] * Di[i], si = Mi[i][j] * Di[i];          // k = i term: conj(1) M_ij / D_i
+#pragma unroll
+            for (int k = i + 1; k < 6; ++k) {
+                const double tr = Mr[k][j] * Di[k], ti = Mi[k][j] * Di[k];
+                sr += Mr[k][i] * tr + Mi[k][i] * ti;                      // conj(M_ki) * M_kj
+                si += Mr[k][i] * ti - Mi[k][i] * tr;
+            }
+            p[pk(i, j)] = sr;
+            p[pk(i, j) + 1] = si;
+        }
+    }
+    return ok;
+}
+
+template <typename T>
+__global__ void __launch_bounds__(3 * CLOV_SITES)
+build_clover_kernel(Geom g, double csw, double m0, const T* __restrict__ gauge,
+                    T* __restrict__ clov_e, T* __restrict__ clov_o, T* __restrict__ clov_o_plain, int* need_pivot)
+{
+    // clov_e: A on even sites; clov_o: A^-1 on odd sites; clov_o_plain: A itself on odd sites
+    // (needed only by the full operator D = A + H).  A NULL output skips that part.
+    __shared__ double G[2][3][9][CLOV_SITES];        // [-+][k][entry][site]: diag 0..2, lower (re, im) 3..8
+    const int sl = threadIdx.x % CLOV_SITES, k = threadIdx.x / CLOV_SITES;
+    const int idx = blockIdx.x * CLOV_SITES + sl;
+    const bool live = idx < 2 * g.Vh;
+    const int parity = live ? idx / g.Vh : 0, cb = live ? idx % g.Vh : 0;
+    const bool wanted = live && (parity == 1 ? (clov_o || clov_o_plain) : clov_e != nullptr);
+    if (wanted) {
+        const Site s = site_of_cb(g, cb, parity);
+        X4 x;
+        x.x = 2 * s.xh + s.q; x.y = s.y; x.z = s.z; x.t = s.t;
+        const int i = k == 2 ? 0 : k + 1, j = k == 0 ? 2 : k - 1;      // (i, j, k) cyclic
+        double fij[9], fkt[9];
+        field_strength_u<T>(g, gauge, x, i, j, fij);
+        field_strength_u<T>(g, gauge, x, k, 3, fkt);
+        // G = i F:  diag = -Im F_aa;  lower: Re G = -Im F, Im G = Re F
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            G[0][k][a][sl] = -(fij[a] - fkt[a]);
+            G[1][k][a][sl] = -(fij[a] + fkt[a]);
+        }
+#pragma unroll
+        for (int e = 0; e < 3; ++e) {
+            G[0][k][3 + 2 * e][sl] = -(fij[4 + 2 * e] - fkt[4 + 2 * e]);
+            G[0][k][4 + 2 * e][sl] = fij[3 + 2 * e] - fkt[3 + 2 * e];
+            G[1][k][3 + 2 * e][sl] = -(fij[4 + 2 * e] + fkt[4 + 2 * e]);
+            G[1][k][4 + 2 * e][sl] = fij[3 + 2 * e] + fkt[3 + 2 * e];
+        }
+    }
+    __syncthreads();
+    if (!wanted || k >= 2) return;
+    const int h = k;                                  // chirality block: 0 = upper (G^-), 1 = lower (G^+)
+    double gx[9], gy[9], gz[9];
+#pragma unroll
+    for (int e = 0; e < 9; ++e) { gx[e] = G[h][0][e][sl]; gy[e] = G[h][1][e][sl]; gz[e] = G[h][2][e][sl]; }
+    const double kap = csw / 16.0, c0 = m0 + 4.0;
+    double p[36];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) { p[a] = c0 - kap * gz[a]; p[3 + a] = c0 + kap * gz[a]; }
+    // diagonal 3x3 blocks: -+ kap G_z (strictly-lower entries (1,0), (2,0), (2,1))
+#pragma unroll
+    for (int e = 0; e < 3; ++e) {
+        const int a = e == 0 ? 1 : 2, b = e == 2 ? 1 : 0;
+        p[pk(a, b)] = -kap * gz[3 + 2 * e];         p[pk(a, b) + 1] = -kap * gz[4 + 2 * e];
+        p[pk(3 + a, 3 + b)] = kap * gz[3 + 2 * e];  p[pk(3 + a, 3 + b) + 1] = kap * gz[4 + 2 * e];
+    }
+    // lower-left 3x3 block (3 + a, b) = -kap (G_x + i G_y)[a][b]
+#pragma unroll
+    for (int a = 0; a < 3; ++a)
+#pragma unroll
+        for (int b = 0; b < 3; ++b) {
+            double xr, xi, yr, yi;
+            if (a == b) { xr = gx[a]; xi = 0.0; yr = gy[a]; yi = 0.0; }
+            else {
+                const int hi = a > b ? a : b, lo = a > b ? b : a;
+                const int e = hi == 1 ? 0 : (lo == 0 ? 1 : 2);
+                const double sgn = a > b ? 1.0 : -1.0;               // upper entries are the conjugates
+                xr = gx[3 + 2 * e]; xi = sgn * gx[4 + 2 * e];
+                yr = gy[3 + 2 * e]; yi = sgn * gy[4 + 2 * e];
+            }
+            p[pk(3 + a, b)] = -kap * (xr - yi);
+            p[pk(3 + a, b) + 1] = -kap * (xi + yr);
+        }
+    T c[36];
+    T* plain = parity ? clov_o_plain : clov_e;
+    if (plain) {
+#pragma unroll
+        for (int q = 0; q < 36; ++q) c[q] = (T)p[q];
+        store_clover_block<T>(plain, g.Vh, cb, h, c);
+    }
+    if (parity == 1 && clov_o) {
+        if (!invert6_ldl(p)) atomicOr(need_pivot, 1);
+#pragma unroll
+        for (int q = 0; q < 36; ++q) c[q] = (T)p[q];
+        store_clover_block<T>(clov_o, g.Vh, cb, h, c);
+    }
+}
+
 template <typename T>
 void launch_build_clover(const Geom& g, double csw, double m0, const void* gauge, void* clov_e, void* clov_o,
-                         void* clov_o_plain, int* singular_flag, cudaStream_t st)
+                         void* clov_o_plain, int* need_pivot_flag, cudaStream_t st)
 {
     const int n = 2 * g.Vh;
-    build_clover_kernel<T><<<(n + 63) / 64, 64, 0, st>>>(g, csw, m0, (const T*)gauge, (T*)clov_e, (T*)clov_o,
-                                                          (T*)clov_o_plain, singular_flag);
+    build_clover_kernel<T><<<(n + CLOV_SITES - 1) / CLOV_SITES, 3 * CLOV_SITES, 0, st>>>(
+        g, csw, m0, (const T*)gauge, (T*)clov_e, (T*)clov_o, (T*)clov_o_plain, need_pivot_flag);
 }
 template void launch_build_clover<float>(const Geom&, double, double, const void*, void*, void*, void*, int*, cudaStream_t);
 template void launch_build_clover<double>(const Geom&, double, double, const void*, void*, void*, void*, int*, cudaStream_t);
+
+template <typename T>
+void launch_build_clover_pivoted(const Geom& g, double csw, double m0, const void* gauge, void* clov_e, void* clov_o,
+                                 void* clov_o_plain, int* singular_flag, cudaStream_t st)
+{
+    const int n = 2 * g.Vh;
+    build_clover_pivoted_kernel<T><<<(n + 63) / 64, 64, 0, st>>>(g, csw, m0, (const T*)gauge, (T*)clov_e, (T*)clov_o,
+                                                                  (T*)clov_o_plain, singular_flag);
+}
+template void launch_build_clover_pivoted<float>(const Geom&, double, double, const void*, void*, void*, void*, int*, cudaStream_t);
+template void launch_build_clover_pivoted<double>(const Geom&, double, double, const void*, void*, void*, void*, int*, cudaStream_t);
 
 // ------------------------------------------------------------------ debug: dense clover out
 template <typename T>
