@@ -279,14 +279,13 @@ int ddamg_get_clover(ddamg_ctx* ctx, void* A_nat, void* Ainv_nat);
  *                     on 18-real links.  Results change by rounding only (third rows are
  *                     rebuilt from rounded rows).  Clover build and SAP block solves always
  *                     use the full links.
- *   "fused_sweep"     0 (default) or 1.  1 = ddamg_apply_schur and every sweep of
- *                     ddamg_richardson run kernel A and kernel B / B' as ONE launch, pipelined
- *                     time slice by time slice (SURVEY.md 8(d) "A->B slab pipelining in L2").
- *                     Bit-identical results.  Used only when a time slice (L^3/2 sites) is a
- *                     multiple of 128 sites, else the two-launch path runs.  Measured slower
- *                     than two launches on B200 at 32^3x64 .. 64^3x128.
- *   "sweep_lag"       1..64 (default 2): time slices kernel A runs ahead of kernel B in the
- *                     fused sweep.
+ *   "cuda_graph"      -1 (default, auto), 0 or 1.  A history-free ddamg_richardson call (res_hist NULL,
+ *                     nu > 1: the smoother use) is 2 nu kernel launches with no host work between
+ *                     them; with 1 they are captured once into a CUDA graph and replayed by one
+ *                     graph launch per call (re-captured when b_e, x_e, nu, omega, zero_init or the
+ *                     link format change).  Auto = on for lattices up to 2^19 sites per parity,
+ *                     where the kernels are short enough for launch gaps to show.  Same kernels,
+ *                     same order: bit-identical results.  Off while ddamg_kernel_timing is on.
  * EINVAL for an unknown name or a bad value.
  */
 int ddamg_set_option(ddamg_ctx* ctx, const char* name, double value);
@@ -301,7 +300,7 @@ long long ddamg_launch_count(ddamg_ctx* ctx);
  * number of launches of kernel class `which` (0 = kernel A: A_oo^-1 H_oe, 1 = kernel B /
  * B': A_ee x - H_eo t with optional Richardson update, 2 = eq.-2 factors, 3 / 4 = the
  * multi-rhs forms of kernel A / kernel B, B', 5 = one parity of the full operator /
- * residual, 6 = SAP block-solve kernel, 7 = fused sweep, 8 = fused multi-dot, 9 = fused
+ * residual, 6 = SAP block-solve kernel, 8 = fused multi-dot, 9 = fused
  * multi-axpy (+ norm), 10 = the other streaming BLAS-1 passes of GMRES / GCR) since the last
  * reset, after synchronising the stream.  The event pairs come from a pool created by
  * ddamg_kernel_timing(ctx, 1) (4096 pairs, grown in chunks if a measurement records more):

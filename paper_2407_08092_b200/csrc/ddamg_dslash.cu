@@ -12,7 +12,6 @@
 // One thread per output site; consecutive threads = consecutive checkerboard indices, so
 // every plane access of a warp is one contiguous 512-byte (16-byte vectors) run.
 #include "ddamg_dslash_kernel.cuh"
-#include "ddamg_sweep_kernel.cuh"
 
 namespace ddamg {
 
@@ -47,41 +46,6 @@ template void launch_dslash<float>(const Geom&, int, bool, int, const void*, con
                                    const void*, const void*, void*, double, double*, int, double, int, int, cudaStream_t);
 template void launch_dslash<double>(const Geom&, int, bool, int, const void*, const void*, const void*, const void*,
                                     const void*, const void*, void*, double, double*, int, double, int, int, cudaStream_t);
-
-template cudaError_t launch_sweep_recon<float, 18>(const Geom&, int, bool, const void*, void*, const void*, const void*,
-                                                   const void*, const void*, const void*, void*, double, double*,
-                                                   unsigned int*, int, int, cudaStream_t);
-template cudaError_t launch_sweep_recon<double, 18>(const Geom&, int, bool, const void*, void*, const void*, const void*,
-                                                    const void*, const void*, const void*, void*, double, double*,
-                                                    unsigned int*, int, int, cudaStream_t);
-
-extern template cudaError_t launch_sweep_recon<float, 12>(const Geom&, int, bool, const void*, void*, const void*,
-                                                          const void*, const void*, const void*, const void*, void*,
-                                                          double, double*, unsigned int*, int, int, cudaStream_t);
-extern template cudaError_t launch_sweep_recon<double, 12>(const Geom&, int, bool, const void*, void*, const void*,
-                                                           const void*, const void*, const void*, const void*, void*,
-                                                           double, double*, unsigned int*, int, int, cudaStream_t);
-
-bool sweep_eligible(const Geom& g) { return (g.Lh * g.L * g.L) % DSLASH_THREADS == 0; }
-
-template <typename T>
-cudaError_t launch_sweep(const Geom& g, int epi_b, bool norm, const void* x, void* t, const void* gauge_e,
-                         const void* gauge_o, const void* clov_e, const void* clov_oinv, const void* rhs, void* out,
-                         double omega, double* partials, unsigned int* sync, int lag, int recon, int apbc,
-                         cudaStream_t st)
-{
-    if (recon == 12)
-        return launch_sweep_recon<T, 12>(g, epi_b, norm, x, t, gauge_e, gauge_o, clov_e, clov_oinv, rhs, out, omega,
-                                         partials, sync, lag, apbc, st);
-    return launch_sweep_recon<T, 18>(g, epi_b, norm, x, t, gauge_e, gauge_o, clov_e, clov_oinv, rhs, out, omega,
-                                     partials, sync, lag, apbc, st);
-}
-template cudaError_t launch_sweep<float>(const Geom&, int, bool, const void*, void*, const void*, const void*, const void*,
-                                         const void*, const void*, void*, double, double*, unsigned int*, int, int, int,
-                                         cudaStream_t);
-template cudaError_t launch_sweep<double>(const Geom&, int, bool, const void*, void*, const void*, const void*, const void*,
-                                          const void*, const void*, void*, double, double*, unsigned int*, int, int, int,
-                                          cudaStream_t);
 
 // out = Cl in on one parity (right factor of eq. 2: t_o = A_oo^-1 b_o)
 template <typename T>

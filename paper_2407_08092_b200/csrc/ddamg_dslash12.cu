@@ -3,7 +3,6 @@
 // rebuilt in registers as conj(row0 x row1).  A separate translation unit so that the two
 // instantiation sets compile in parallel.
 #include "ddamg_dslash_kernel.cuh"
-#include "ddamg_sweep_kernel.cuh"
 
 namespace ddamg {
 
@@ -11,12 +10,5 @@ template void launch_dslash_recon<float, 12>(const Geom&, int, bool, int, const 
                                              const void*, const void*, void*, double, double*, int, double, int, cudaStream_t);
 template void launch_dslash_recon<double, 12>(const Geom&, int, bool, int, const void*, const void*, const void*, const void*,
                                               const void*, const void*, void*, double, double*, int, double, int, cudaStream_t);
-
-template cudaError_t launch_sweep_recon<float, 12>(const Geom&, int, bool, const void*, void*, const void*, const void*,
-                                                   const void*, const void*, const void*, void*, double, double*,
-                                                   unsigned int*, int, int, cudaStream_t);
-template cudaError_t launch_sweep_recon<double, 12>(const Geom&, int, bool, const void*, void*, const void*, const void*,
-                                                    const void*, const void*, const void*, void*, double, double*,
-                                                    unsigned int*, int, int, cudaStream_t);
 
 }  // namespace ddamg

@@ -40,15 +40,6 @@ void launch_dslash(const Geom& g, int epi, bool norm, int parity, const void* in
 template <typename T>
 void launch_compress_gauge(const Geom& g, int bc, const void* gauge, void* gauge12, unsigned int* dev_max_bits,
                            cudaStream_t st);
-// One Schur apply / Richardson sweep as one launch, kernels A and B pipelined slice by slice
-// through L2 (ddamg_sweep_kernel.cuh).  Only when sweep_eligible(g): a time slice is a whole
-// number of CTA tiles.  sync: T + 1 device words.
-bool sweep_eligible(const Geom& g);
-template <typename T>
-cudaError_t launch_sweep(const Geom& g, int epi_b, bool norm, const void* x, void* t, const void* gauge_e,
-                         const void* gauge_o, const void* clov_e, const void* clov_oinv, const void* rhs, void* out,
-                         double omega, double* partials, unsigned int* sync, int lag, int recon, int apbc,
-                         cudaStream_t st);
 template <typename T>
 void launch_clover_apply(const Geom& g, const void* clov, const void* in, void* out, int nrhs, cudaStream_t st);
 int dslash_grid(const Geom& g, int nrhs = 1);

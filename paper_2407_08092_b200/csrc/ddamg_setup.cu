@@ -402,7 +402,13 @@ __global__ void build_clover_pivoted_kernel(Geom g, double csw, double m0, const
 // A pivot below 1e-2 * max|A_ij| (never the case for a clover block with its dominant diagonal; possible for
 // an indefinite or singular block) raises *need_pivot: the host then rebuilds everything with the pivoted
 // Gauss-Jordan kernel above, which also decides DDAMG_ESINGULAR (reading C6: pivot < 1e-12 ||block||).
-constexpr int CLOV_SITES = 64;
+#ifndef DDAMG_CLOV_SITES
+#define DDAMG_CLOV_SITES 64
+#endif
+#ifndef DDAMG_CLOV_MINB
+#define DDAMG_CLOV_MINB 2
+#endif
+constexpr int CLOV_SITES = DDAMG_CLOV_SITES;
 
 struct M3d { double re[9], im[9]; };
 struct X4 { int x, y, z, t; };
@@ -514,70 +520,87 @@ __device__ __forceinline__ bool invert6_ldl(double (&p)[36])
     for (int i = 0; i < 6; ++i) scale = fmax(scale, fabs(p[i]));
 #pragma unroll
     for (int k = 6; k < 36; ++k) scale = fmax(scale, fabs(p[k]));
+    // every loop below has compile-time bounds 0..5 and the triangular structure is expressed by guards that
+    // fold away after unrolling, so that all arrays stay in registers
     double Lr[6][6], Li[6][6], D[6], Di[6];
     bool ok = true;
 #pragma unroll
     for (int j = 0; j < 6; ++j) {
         double d = p[j];
 #pragma unroll
-        for (int k = 0; k < j; ++k) d -= (Lr[j][k] * Lr[j][k] + Li[j][k] * Li[j][k]) * D[k];
+        for (int k = 0; k < 6; ++k)
+            if (k < j) d -= (Lr[j][k] * Lr[j][k] + Li[j][k] * Li[j][k]) * D[k];
         D[j] = d;
         ok = ok && (fabs(d) > 1e-2 * scale);
         Di[j] = 1.0 / d;
 #pragma unroll
-        for (int i = j + 1; i < 6; ++i) {
-            double sr = p[pk(i, j)], si = p[pk(i, j) + 1];
+        for (int i = 0; i < 6; ++i) {
+            if (i > j) {
+                double sr = p[pk(i, j)], si = p[pk(i, j) + 1];
 #pragma unroll
-            for (int k = 0; k < j; ++k) {
-                // L_ik D_k conj(L_jk)
-                const double tr = Lr[i][k] * D[k], ti = Li[i][k] * D[k];
-                sr -= tr * Lr[j][k] + ti * Li[j][k];
-                si -= ti * Lr[j][k] - tr * Li[j][k];
+                for (int k = 0; k < 6; ++k) {
+                    if (k < j) {
+                        // L_ik D_k conj(L_jk)
+                        const double tr = Lr[i][k] * D[k], ti = Li[i][k] * D[k];
+                        sr -= tr * Lr[j][k] + ti * Li[j][k];
+                        si -= ti * Lr[j][k] - tr * Li[j][k];
+                    }
+                }
+                Lr[i][j] = sr * Di[j];
+                Li[i][j] = si * Di[j];
             }
-            Lr[i][j] = sr * Di[j];
-            Li[i][j] = si * Di[j];
         }
     }
-    // M = L^-1 (unit lower triangular), in place column by column
+    // M = L^-1 (unit lower triangular), column by column
     double Mr[6][6], Mi[6][6];
 #pragma unroll
-    for (int j = 0; j < 6; ++j)
+    for (int j = 0; j < 6; ++j) {
 #pragma unroll
-        for (int i = j + 1; i < 6; ++i) {
-            double sr = Lr[i][j], si = Li[i][j];
+        for (int i = 0; i < 6; ++i) {
+            if (i > j) {
+                double sr = Lr[i][j], si = Li[i][j];
 #pragma unroll
-            for (int k = j + 1; k < i; ++k) {
-                sr += Lr[i][k] * Mr[k][j] - Li[i][k] * Mi[k][j];
-                si += Lr[i][k] * Mi[k][j] + Li[i][k] * Mr[k][j];
+                for (int k = 0; k < 6; ++k) {
+                    if (k > j && k < i) {
+                        sr += Lr[i][k] * Mr[k][j] - Li[i][k] * Mi[k][j];
+                        si += Lr[i][k] * Mi[k][j] + Li[i][k] * Mr[k][j];
+                    }
+                }
+                Mr[i][j] = -sr;
+                Mi[i][j] = -si;
             }
-            Mr[i][j] = -sr;
-            Mi[i][j] = -si;
         }
+    }
     // A^-1 = M^H D^-1 M:  (i, j), i >= j:  sum_{k >= i} conj(M_ki) M_kj / D_k,  M_kk = 1
 #pragma unroll
     for (int i = 0; i < 6; ++i) {
         double d = Di[i];
 #pragma unroll
-        for (int k = i + 1; k < 6; ++k) d += (Mr[k][i] * Mr[k][i] + Mi[k][i] * Mi[k][i]) * Di[k];
+        for (int k = 0; k < 6; ++k)
+            if (k > i) d += (Mr[k][i] * Mr[k][i] + Mi[k][i] * Mi[k][i]) * Di[k];
         p[i] = d;
 #pragma unroll
-        for (int j = 0; j < i; ++j) {
-            double sr = Mr[i][j] * Di[i], si = Mi[i][j] * Di[i];          // k = i term: conj(1) M_ij / D_i
+        for (int j = 0; j < 6; ++j) {
+            if (j < i) {
+                double sr = Mr[i][j] * Di[i], si = Mi[i][j] * Di[i];          // k = i term: conj(1) M_ij / D_i
 #pragma unroll
-            for (int k = i + 1; k < 6; ++k) {
-                const double tr = Mr[k][j] * Di[k], ti = Mi[k][j] * Di[k];
-                sr += Mr[k][i] * tr + Mi[k][i] * ti;                      // conj(M_ki) * M_kj
-                si += Mr[k][i] * ti - Mi[k][i] * tr;
+                for (int k = 0; k < 6; ++k) {
+                    if (k > i) {
+                        const double tr = Mr[k][j] * Di[k], ti = Mi[k][j] * Di[k];
+                        sr += Mr[k][i] * tr + Mi[k][i] * ti;                  // conj(M_ki) * M_kj
+                        si += Mr[k][i] * ti - Mi[k][i] * tr;
+                    }
+                }
+                p[pk(i, j)] = sr;
+                p[pk(i, j) + 1] = si;
             }
-            p[pk(i, j)] = sr;
-            p[pk(i, j) + 1] = si;
         }
     }
     return ok;
 }
 
 template <typename T>
-__global__ void __launch_bounds__(3 * CLOV_SITES)
+__global__ void __launch_bounds__(3 * CLOV_SITES, DDAMG_CLOV_MINB)
 build_clover_kernel(Geom g, double csw, double m0, const T* __restrict__ gauge,
                     T* __restrict__ clov_e, T* __restrict__ clov_o, T* __restrict__ clov_o_plain, int* need_pivot)
 {

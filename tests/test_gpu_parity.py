@@ -234,6 +234,43 @@ def test_richardson_matches_oracle(cfg, prec, nu, L, T):
     assert rel_l2(p.to_np(x_e3, None), x0_ref) <= (1e-11 if p.f64 else 2e-5)
 
 
+def test_richardson_cuda_graph_replay_is_bit_identical():
+    """Option cuda_graph: the history-free call replays its 2 nu launches through a captured CUDA graph
+    (SURVEY.md 3.4); same kernels, same order -> same bits, also after the arguments change (re-capture)."""
+    p = make_pair(2, "f32", 8, 8)
+    _, b_d = p.spinor(11)
+    _, c_d = p.spinor(12)
+    _, x_d = p.spinor(13)
+    b_e, _ = p.ctx.pack(b_d)
+    c_e, _ = p.ctx.pack(c_d)
+    outs = {}
+    for mode in (0, 1):
+        p.ctx.set_option("cuda_graph", mode)
+        res = []
+        for rhs, nu, omega, zi in ((b_e, 4, 0.3, False), (b_e, 4, 0.3, False), (c_e, 4, 0.3, False), (c_e, 3, 0.25, True),
+                                   (b_e, 4, 0.3, False)):
+            x_e, _ = p.ctx.pack(x_d)
+            l0 = p.ctx.launch_count()
+            p.ctx.richardson(rhs, x_e, nu, omega, zero_init=zi)
+            torch.cuda.synchronize()
+            res.append((x_e.clone(), p.ctx.launch_count() - l0))
+        outs[mode] = res
+    for (xa, la), (xb, lb) in zip(outs[0], outs[1]):
+        assert torch.equal(xa, xb)
+        assert la == lb                                   # the launch accounting counts the kernels inside the graph
+    p.ctx.set_option("cuda_graph", 1)
+    p.ctx.set_option("gauge_recon", 12)                   # link format is part of the capture key
+    x12, _ = p.ctx.pack(x_d)
+    p.ctx.richardson(b_e, x12, 4, 0.3)
+    p.ctx.set_option("cuda_graph", 0)
+    y12, _ = p.ctx.pack(x_d)
+    p.ctx.richardson(b_e, y12, 4, 0.3)
+    torch.cuda.synchronize()
+    assert torch.equal(x12, y12)
+    with pytest.raises(p.dd.DdamgError):
+        p.ctx.set_option("cuda_graph", 2)
+
+
 def test_richardson_nu_zero_is_identity():
     p = make_pair(1, "f64")
     _, b_d = p.spinor(1)
