@@ -223,11 +223,21 @@ int ddamg_unpack_spinor(ddamg_ctx* ctx, const void* x_e, const void* x_o, void* 
  * many vectors" / multiple right-hand sides as the way to raise cache reuse).  The same D_S is
  * applied to nrhs (1..32, V/2 * nrhs < 2^31) right-hand sides in one pass: links and clover
  * blocks, 78 % of the bytes of a single-rhs pass, are fetched once per site for all of them.
- * A BATCH is a DEVICE buffer of ddamg_batch_spinor_bytes(ctx, nrhs) = nrhs * half-spinor bytes
- * holding nrhs native half spinors interleaved per site: plane j, vector index cb * nrhs + r
- * (r = rhs index, fastest).  Callers build batches with ddamg_batch_interleave from nrhs
- * native half spinors stored back to back (halves = [r][native half spinor]) and read them
- * back with ddamg_batch_deinterleave; both are asynchronous, neither may alias.
+ * A BATCH is a DEVICE buffer of ddamg_batch_spinor_bytes(ctx, nrhs) bytes holding nrhs native
+ * half spinors interleaved per site.
+ *   fp64 context: nrhs * half-spinor bytes; plane j (double2), vector index cb * nrhs + r
+ *     (r = rhs index, fastest).
+ *   fp32 context: right-hand sides travel in PAIRS (2p, 2p+1), one thread per (site, pair), every
+ *     operation a packed f32x2 instruction whose two lanes are the two right-hand sides (links,
+ *     rebuilt third rows, clover entries and index arithmetic are shared by the pair):
+ *     2 * ceil(nrhs / 2) * half-spinor bytes; 12 half-planes of float4; half-plane h (= complex
+ *     number h = 3 * spin + colour of the site), vector index cb * npairs + p =
+ *     (re of rhs 2p, re of rhs 2p+1, im of rhs 2p, im of rhs 2p+1).  With an odd nrhs the second
+ *     lane of the last pair is padding (written as 0 by ddamg_batch_interleave, ignored by
+ *     ddamg_batch_deinterleave and by the residual history).
+ * Callers build batches with ddamg_batch_interleave from nrhs native half spinors stored back
+ * to back (halves = [r][native half spinor]) and read them back with ddamg_batch_deinterleave;
+ * both are asynchronous, neither may alias.
  * Every *_batch function computes, for each r independently, exactly what its single-rhs
  * namesake computes (same arithmetic, same order: results are bit-identical per rhs).
  */

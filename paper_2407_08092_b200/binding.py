@@ -256,14 +256,20 @@ class Ddamg:
         return lam.value
 
     # -- multi-rhs batching (NEXT-2) ------------------------------------------------
+    def batch_numel(self, nrhs: int) -> int:
+        """Reals in a batch buffer of nrhs right-hand sides (ddamg_batch_spinor_bytes: an fp32 batch holds
+        PAIRS of right-hand sides, so an odd nrhs is padded by one slot)."""
+        nbytes = self.lib.ddamg_batch_spinor_bytes(self._h, nrhs)
+        return nbytes // (4 if self.rdtype == torch.float32 else 8)
+
     def batch_spinor(self, nrhs: int, zero: bool = False) -> torch.Tensor:
         """A batch buffer: nrhs native half spinors interleaved per site (flat real tensor)."""
-        assert self.lib.ddamg_batch_spinor_bytes(self._h, nrhs) == nrhs * self.half_bytes
-        return (torch.zeros if zero else torch.empty)(nrhs * 12 * self.V, dtype=self.rdtype, device=self.device)
+        return (torch.zeros if zero else torch.empty)(self.batch_numel(nrhs), dtype=self.rdtype, device=self.device)
 
     def _chk_batch(self, nrhs, *ts):
+        n = self.batch_numel(nrhs)
         for t in ts:
-            assert t.is_cuda and t.dtype == self.rdtype and t.is_contiguous() and t.numel() == nrhs * 12 * self.V, \
+            assert t.is_cuda and t.dtype == self.rdtype and t.is_contiguous() and t.numel() == n, \
                 "expected a batch of nrhs native half spinors of this context"
 
     def batch_interleave(self, halves, X: Optional[torch.Tensor] = None) -> torch.Tensor:
@@ -272,7 +278,8 @@ class Ddamg:
         nrhs = H.shape[0]
         H = H.contiguous().view(-1)
         X = self.batch_spinor(nrhs) if X is None else X
-        self._chk_batch(nrhs, H, X)
+        assert H.is_cuda and H.dtype == self.rdtype and H.numel() == nrhs * 12 * self.V
+        self._chk_batch(nrhs, X)
         self._ck(self.lib.ddamg_batch_interleave(self._h, nrhs, _ptr(H), _ptr(X)), "ddamg_batch_interleave")
         return X
 

@@ -388,19 +388,20 @@ extern "C" int ddamg_get_clover(ddamg_ctx* ctx, void* A_nat, void* Ainv_nat)
 
 // --------------------------------------------------------------------------- hot path
 // One fused hopping launch.  parity = parity of the output sites.
+// units: 0 = single right-hand side, >= 1 = multi-rhs batch of that many threads per site (batch_units())
 static int dslash(ddamg_ctx* ctx, int epi, bool norm, int parity, const void* in, const void* own, const void* rhs,
-                  void* out, double omega, int which, int nrhs = 1, size_t partials_offset = 0,
+                  void* out, double omega, int which, int units = 0, size_t partials_offset = 0,
                   const void* clov_override = nullptr)
 {
-    double* partials = (nrhs > 1 ? ctx->partials_batch : ctx->partials) + partials_offset;
+    double* partials = (units > 0 ? ctx->partials_batch : ctx->partials) + partials_offset;
     const void* clov = clov_override ? clov_override : ctx->clov[parity];
     KernelTimer kt(ctx, which);
     if (ctx->prec == DDAMG_F32)
         launch_dslash<float>(ctx->g, epi, norm, parity, in, hop_gauge_block(ctx, parity), hop_gauge_block(ctx, 1 - parity),
-                             clov, own, rhs, out, omega, partials, nrhs, ctx->batch_l2_bytes, ctx->recon, ctx->bc == 1, ctx->stream);
+                             clov, own, rhs, out, omega, partials, units, ctx->batch_l2_bytes, ctx->recon, ctx->bc == 1, ctx->stream);
     else
         launch_dslash<double>(ctx->g, epi, norm, parity, in, hop_gauge_block(ctx, parity), hop_gauge_block(ctx, 1 - parity),
-                              clov, own, rhs, out, omega, partials, nrhs, ctx->batch_l2_bytes, ctx->recon, ctx->bc == 1, ctx->stream);
+                              clov, own, rhs, out, omega, partials, units, ctx->batch_l2_bytes, ctx->recon, ctx->bc == 1, ctx->stream);
     return after_launch(ctx);
 }
 
@@ -546,8 +547,8 @@ extern "C" int ddamg_prepare_rhs(ddamg_ctx* ctx, const void* b_e, const void* b_
     if (!b_e || !b_o || !bhat_e) return fail(ctx, DDAMG_EINVAL, "ddamg_prepare_rhs: NULL argument");
     int s = need_ready(ctx, "ddamg_prepare_rhs");
     if (s != DDAMG_OK) return s;
-    if (ctx->prec == DDAMG_F32) launch_clover_apply<float>(ctx->g, ctx->clov[1], b_o, ctx->tmp_o, 1, ctx->stream);     // t_o = A_oo^-1 b_o
-    else launch_clover_apply<double>(ctx->g, ctx->clov[1], b_o, ctx->tmp_o, 1, ctx->stream);
+    if (ctx->prec == DDAMG_F32) launch_clover_apply<float>(ctx->g, ctx->clov[1], b_o, ctx->tmp_o, 0, ctx->stream);     // t_o = A_oo^-1 b_o
+    else launch_clover_apply<double>(ctx->g, ctx->clov[1], b_o, ctx->tmp_o, 0, ctx->stream);
     s = after_launch(ctx);
     if (s != DDAMG_OK) return s;
     return dslash(ctx, EPI_RHS_MINUS_HOP, false, 0, ctx->tmp_o, nullptr, b_e, bhat_e, 0.0, 2);         // b_e - H_eo t_o
@@ -566,8 +567,9 @@ static int batch_ready(ddamg_ctx* ctx, int nrhs, const char* who)
         CK(cudaStreamSynchronize(ctx->stream));
         cudaFree(ctx->tmp_batch); cudaFree(ctx->partials_batch);
         ctx->tmp_batch = nullptr; ctx->partials_batch = nullptr; ctx->batch_cap = 0;
-        cudaError_t e = cudaMalloc(&ctx->tmp_batch, (size_t)nrhs * ctx->half_bytes);
-        if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->partials_batch, sizeof(double) * (size_t)dslash_grid(ctx->g, nrhs) * nrhs);
+        const int slots = batch_slots(nrhs, ctx->real_bytes), units = batch_units(nrhs, ctx->real_bytes);
+        cudaError_t e = cudaMalloc(&ctx->tmp_batch, (size_t)slots * ctx->half_bytes);
+        if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->partials_batch, sizeof(double) * (size_t)dslash_grid(ctx->g, units) * slots);
         if (e != cudaSuccess) {
             cudaGetLastError();
             cudaFree(ctx->tmp_batch); ctx->tmp_batch = nullptr;
@@ -580,7 +582,7 @@ static int batch_ready(ddamg_ctx* ctx, int nrhs, const char* who)
 
 extern "C" size_t ddamg_batch_spinor_bytes(ddamg_ctx* ctx, int nrhs)
 {
-    return (ctx && nrhs > 0) ? (size_t)nrhs * ctx->half_bytes : 0;
+    return (ctx && nrhs > 0) ? (size_t)batch_slots(nrhs, ctx->real_bytes) * ctx->half_bytes : 0;
 }
 
 static int batch_interleave(ddamg_ctx* ctx, int nrhs, bool to_batch, void* halves, void* X, const char* who)
@@ -610,9 +612,10 @@ extern "C" int ddamg_apply_schur_batch(ddamg_ctx* ctx, int nrhs, const void* X_e
     if (!X_e || !Y_e || X_e == Y_e) return fail(ctx, DDAMG_EINVAL, "ddamg_apply_schur_batch: NULL or aliased arguments");
     int s = batch_ready(ctx, nrhs, "ddamg_apply_schur_batch");
     if (s != DDAMG_OK) return s;
-    s = dslash(ctx, EPI_CLOV_HOP, false, 1, X_e, nullptr, nullptr, ctx->tmp_batch, 0.0, 3, nrhs);
+    const int units = batch_units(nrhs, ctx->real_bytes);
+    s = dslash(ctx, EPI_CLOV_HOP, false, 1, X_e, nullptr, nullptr, ctx->tmp_batch, 0.0, 3, units);
     if (s != DDAMG_OK) return s;
-    return dslash(ctx, EPI_SCHUR, false, 0, ctx->tmp_batch, X_e, nullptr, Y_e, 0.0, 4, nrhs);
+    return dslash(ctx, EPI_SCHUR, false, 0, ctx->tmp_batch, X_e, nullptr, Y_e, 0.0, 4, units);
 }
 
 extern "C" int ddamg_richardson_batch(ddamg_ctx* ctx, int nrhs, const void* B_e, void* X_e, int nu, double omega,
@@ -626,14 +629,15 @@ extern "C" int ddamg_richardson_batch(ddamg_ctx* ctx, int nrhs, const void* B_e,
     if (hist && (long long)nu * nrhs > HIST_MAX) return fail(ctx, DDAMG_EINVAL, "ddamg_richardson_batch: nu * nrhs exceeds the history capacity");
     if (hist) { s = reset_hist(ctx); if (s != DDAMG_OK) return s; }
     // x^(0) = 0 is run as a full sweep on a zeroed batch (bit-identical to x = omega b)
-    if (zero_init) CK(cudaMemsetAsync(X_e, 0, (size_t)nrhs * ctx->half_bytes, ctx->stream));
+    const int units = batch_units(nrhs, ctx->real_bytes), slots = batch_slots(nrhs, ctx->real_bytes);
+    if (zero_init) CK(cudaMemsetAsync(X_e, 0, (size_t)slots * ctx->half_bytes, ctx->stream));
     for (int i = 0; i < nu; ++i) {
-        s = dslash(ctx, EPI_CLOV_HOP, false, 1, X_e, nullptr, nullptr, ctx->tmp_batch, 0.0, 3, nrhs);
+        s = dslash(ctx, EPI_CLOV_HOP, false, 1, X_e, nullptr, nullptr, ctx->tmp_batch, 0.0, 3, units);
         if (s != DDAMG_OK) return s;
-        s = dslash(ctx, EPI_RICHARDSON, hist, 0, ctx->tmp_batch, X_e, B_e, X_e, omega, 4, nrhs);
+        s = dslash(ctx, EPI_RICHARDSON, hist, 0, ctx->tmp_batch, X_e, B_e, X_e, omega, 4, units);
         if (s != DDAMG_OK) return s;
         if (hist) {
-            launch_finalize_norm_batch(nrhs > 1 ? ctx->partials_batch : ctx->partials, dslash_grid(ctx->g, nrhs), nrhs, ctx->sc, i * nrhs, ctx->stream);
+            launch_finalize_norm_batch(ctx->partials_batch, dslash_grid(ctx->g, units), nrhs, slots, ctx->sc, i * nrhs, ctx->stream);
             s = after_launch(ctx);
             if (s != DDAMG_OK) return s;
         }
@@ -648,7 +652,7 @@ extern "C" int ddamg_reconstruct_odd_batch(ddamg_ctx* ctx, int nrhs, const void*
     if (!B_o || !X_e || !X_o) return fail(ctx, DDAMG_EINVAL, "ddamg_reconstruct_odd_batch: NULL argument");
     int s = batch_ready(ctx, nrhs, "ddamg_reconstruct_odd_batch");
     if (s != DDAMG_OK) return s;
-    return dslash(ctx, EPI_CLOV_RHS_MINUS_HOP, false, 1, X_e, nullptr, B_o, X_o, 0.0, 2, nrhs);
+    return dslash(ctx, EPI_CLOV_RHS_MINUS_HOP, false, 1, X_e, nullptr, B_o, X_o, 0.0, 2, batch_units(nrhs, ctx->real_bytes));
 }
 
 extern "C" int ddamg_prepare_rhs_batch(ddamg_ctx* ctx, int nrhs, const void* B_e, const void* B_o, void* Bhat_e)
@@ -657,11 +661,12 @@ extern "C" int ddamg_prepare_rhs_batch(ddamg_ctx* ctx, int nrhs, const void* B_e
     if (!B_e || !B_o || !Bhat_e) return fail(ctx, DDAMG_EINVAL, "ddamg_prepare_rhs_batch: NULL argument");
     int s = batch_ready(ctx, nrhs, "ddamg_prepare_rhs_batch");
     if (s != DDAMG_OK) return s;
-    if (ctx->prec == DDAMG_F32) launch_clover_apply<float>(ctx->g, ctx->clov[1], B_o, ctx->tmp_batch, nrhs, ctx->stream);
-    else launch_clover_apply<double>(ctx->g, ctx->clov[1], B_o, ctx->tmp_batch, nrhs, ctx->stream);
+    const int units = batch_units(nrhs, ctx->real_bytes);
+    if (ctx->prec == DDAMG_F32) launch_clover_apply<float>(ctx->g, ctx->clov[1], B_o, ctx->tmp_batch, units, ctx->stream);
+    else launch_clover_apply<double>(ctx->g, ctx->clov[1], B_o, ctx->tmp_batch, units, ctx->stream);
     s = after_launch(ctx);
     if (s != DDAMG_OK) return s;
-    return dslash(ctx, EPI_RHS_MINUS_HOP, false, 0, ctx->tmp_batch, nullptr, B_e, Bhat_e, 0.0, 2, nrhs);
+    return dslash(ctx, EPI_RHS_MINUS_HOP, false, 0, ctx->tmp_batch, nullptr, B_e, Bhat_e, 0.0, 2, units);
 }
 
 // --------------------------------------------------------------------------- GMRES
@@ -951,7 +956,7 @@ static int apply_full(ddamg_ctx* ctx, const void* x_e, const void* x_o, void* y_
 {
     int s = dslash(ctx, EPI_FULL, false, 0, x_o, x_e, nullptr, y_e, 0.0, 5);
     if (s != DDAMG_OK) return s;
-    return dslash(ctx, EPI_FULL, false, 1, x_e, x_o, nullptr, y_o, 0.0, 5, 1, 0, ctx->clov_oo);
+    return dslash(ctx, EPI_FULL, false, 1, x_e, x_o, nullptr, y_o, 0.0, 5, 0, 0, ctx->clov_oo);
 }
 
 extern "C" int ddamg_apply_full(ddamg_ctx* ctx, const void* x_e, const void* x_o, void* y_e, void* y_o)
@@ -1019,7 +1024,7 @@ static int fgmres_impl(ddamg_ctx* ctx, const void* b_e, const void* b_o, void* x
     auto residual = [&]() -> int {
         int q = dslash(ctx, EPI_FULL_RESIDUAL, true, 0, x_o, x_e, b_e, Ve(0), 0.0, 5);
         if (q != DDAMG_OK) return q;
-        q = dslash(ctx, EPI_FULL_RESIDUAL, true, 1, x_e, x_o, b_o, Vo(0), 0.0, 5, 1, (size_t)dgrid, ctx->clov_oo);
+        q = dslash(ctx, EPI_FULL_RESIDUAL, true, 1, x_e, x_o, b_o, Vo(0), 0.0, 5, 0, (size_t)dgrid, ctx->clov_oo);
         if (q != DDAMG_OK) return q;
         launch_finalize_norm(ctx->partials, 2 * dgrid, sc, 1, st);
         return after_launch(ctx);
@@ -1208,7 +1213,7 @@ extern "C" int ddamg_sap(ddamg_ctx* ctx, const void* b_e, const void* b_o, void*
     auto residual = [&](bool norm) -> int {
         int q = dslash(ctx, EPI_FULL_RESIDUAL, norm, 0, x_o, x_e, b_e, ctx->tmp_e, 0.0, 5);
         if (q != DDAMG_OK) return q;
-        q = dslash(ctx, EPI_FULL_RESIDUAL, norm, 1, x_e, x_o, b_o, ctx->tmp_o, 0.0, 5, 1, (size_t)dgrid, ctx->clov_oo);
+        q = dslash(ctx, EPI_FULL_RESIDUAL, norm, 1, x_e, x_o, b_o, ctx->tmp_o, 0.0, 5, 0, (size_t)dgrid, ctx->clov_oo);
         if (q != DDAMG_OK) return q;
         if (norm) { launch_finalize_norm(ctx->partials, 2 * dgrid, ctx->sc, 1, st); q = after_launch(ctx); }
         return q;

@@ -142,22 +142,22 @@ void launch_finalize_norm(const double* partials, int n, Scalars* sc, int append
     finalize_norm_kernel<<<1, BLAS_THREADS, 0, st>>>(partials, n, sc, append_hist);
 }
 
-// multi-rhs: partials[block][nrhs]; block r of this kernel finishes rhs r into hist[offset + r]
-__global__ void finalize_norm_batch_kernel(const double* __restrict__ partials, int nblocks, int nrhs, Scalars* sc,
+// multi-rhs: partials[block][stride]; block r < nrhs of this kernel finishes rhs r into hist[offset + r]
+__global__ void finalize_norm_batch_kernel(const double* __restrict__ partials, int nblocks, int nrhs, int stride, Scalars* sc,
                                            int offset)
 {
     const int r = blockIdx.x;
     double v[1] = { 0.0 };
-    for (int i = threadIdx.x; i < nblocks; i += BLAS_THREADS) v[0] += partials[(size_t)i * nrhs + r];
+    for (int i = threadIdx.x; i < nblocks; i += BLAS_THREADS) v[0] += partials[(size_t)i * stride + r];
     __shared__ double tot[1];
     block_sum_n<1>(v, tot);
     __syncthreads();
     if (threadIdx.x == 0 && offset + r < HIST_MAX) sc->hist[offset + r] = sqrt(tot[0]);
     if (threadIdx.x == 0 && r == nrhs - 1) sc->nhist = (offset + nrhs < HIST_MAX) ? offset + nrhs : HIST_MAX;
 }
-void launch_finalize_norm_batch(const double* partials, int nblocks, int nrhs, Scalars* sc, int offset, cudaStream_t st)
+void launch_finalize_norm_batch(const double* partials, int nblocks, int nrhs, int stride, Scalars* sc, int offset, cudaStream_t st)
 {
-    finalize_norm_batch_kernel<<<nrhs, BLAS_THREADS, 0, st>>>(partials, nblocks, nrhs, sc, offset);
+    finalize_norm_batch_kernel<<<nrhs, BLAS_THREADS, 0, st>>>(partials, nblocks, nrhs, stride, sc, offset);
 }
 
 // ------------------------------------------------------------------ y = alpha * x, partial |x|^2

@@ -42,6 +42,40 @@ __device__ __forceinline__ void unpack(const double2& v, double* r) { r[0] = v.x
 __device__ __forceinline__ float4 pack(const float* r) { return make_float4(r[0], r[1], r[2], r[3]); }
 __device__ __forceinline__ double2 pack(const double* r) { return make_double2(r[0], r[1]); }
 
+// ----------------------------------------------------------------- packed fp32 pairs
+// Blackwell executes two fp32 operations per instruction on an aligned register pair (FADD2 /
+// FMUL2 / FFMA2, PTX add/mul/fma.rn.f32x2); one operand may be a plain 32-bit register that the
+// instruction broadcasts to both lanes, with a sign modifier, at no extra cost.  Each lane is an
+// ordinary IEEE fp32 operation, so a packed evaluation is bit-identical to the scalar one as
+// long as the order of operations per element is the same.  P2 carries two independent values
+// through the hopping / clover code: the two spin components of a half spinor (single rhs), or
+// the same spinor component of two right-hand sides (multi-rhs).
+struct P2 { float2 v; };
+__device__ __forceinline__ P2 mkp(float a, float b) { P2 r; r.v = make_float2(a, b); return r; }
+__device__ __forceinline__ P2 operator+(P2 a, P2 b) { P2 r; r.v = __fadd2_rn(a.v, b.v); return r; }
+__device__ __forceinline__ P2 operator-(P2 a, P2 b) { P2 r; r.v = __fadd2_rn(a.v, make_float2(-b.v.x, -b.v.y)); return r; }
+__device__ __forceinline__ P2 operator-(P2 a) { return mkp(-a.v.x, -a.v.y); }
+
+// value-type generic arithmetic: S = float, double (one value) or P2 (two fp32 values); the
+// coefficient c is always a scalar of the storage precision (a link / clover entry, omega, 1/2)
+__device__ __forceinline__ float vmul(float c, float a) { return c * a; }
+__device__ __forceinline__ double vmul(double c, double a) { return c * a; }
+__device__ __forceinline__ P2 vmul(float c, P2 a) { P2 r; r.v = __fmul2_rn(make_float2(c, c), a.v); return r; }
+__device__ __forceinline__ float vfma(float c, float a, float b) { return fmaf(c, a, b); }
+__device__ __forceinline__ double vfma(double c, double a, double b) { return fma(c, a, b); }
+__device__ __forceinline__ P2 vfma(float c, P2 a, P2 b) { P2 r; r.v = __ffma2_rn(make_float2(c, c), a.v, b.v); return r; }
+__device__ __forceinline__ float vzero(float) { return 0.f; }
+__device__ __forceinline__ double vzero(double) { return 0.0; }
+__device__ __forceinline__ P2 vzero(P2) { return mkp(0.f, 0.f); }
+// |r|^2 accumulated per lane in fp64 (nrm[0]: the value / lane 0, nrm[1]: lane 1 of a P2)
+__device__ __forceinline__ void vnorm_add(float r, double (&nrm)[2]) { nrm[0] += (double)r * (double)r; }
+__device__ __forceinline__ void vnorm_add(double r, double (&nrm)[2]) { nrm[0] += r * r; }
+__device__ __forceinline__ void vnorm_add(P2 r, double (&nrm)[2])
+{
+    nrm[0] += (double)r.v.x * (double)r.v.x;
+    nrm[1] += (double)r.v.y * (double)r.v.y;
+}
+
 // 24 reals of one site of a native half-lattice spinor
 template <typename T, bool STREAM = false>
 __device__ __forceinline__ void load_spinor(const T* __restrict__ base, int Vh, int cb, T (&s)[24])
@@ -64,6 +98,29 @@ __device__ __forceinline__ void store_spinor(T* __restrict__ base, int Vh, int c
     V* p = reinterpret_cast<V*>(base) + cb;
 #pragma unroll
     for (int k = 0; k < 24 / N; ++k) p[(size_t)k * Vh] = pack(&s[k * N]);
+}
+
+// Multi-rhs batch of fp32 spinors, two right-hand sides per thread: the
+// batch is stored as 12 half-planes of float4; half-plane h, vector index cb * npairs + p holds
+// complex number h of the site for the rhs pair p as (re of rhs 2p, re of rhs 2p+1, im of rhs 2p,
+// im of rhs 2p+1), so that one 16-byte load leaves two ready-made register pairs.  Vs = Vh * npairs.
+template <typename T, bool STREAM = false>
+__device__ __forceinline__ void load_spinor(const float* __restrict__ base, int Vs, int idx, P2 (&s)[24])
+{
+    const float4* p = reinterpret_cast<const float4*>(base) + idx;
+#pragma unroll
+    for (int h = 0; h < 12; ++h) {
+        const float4 v = STREAM ? ld_stream(p + (size_t)h * Vs) : ld_reuse(p + (size_t)h * Vs);
+        s[2 * h] = mkp(v.x, v.y);
+        s[2 * h + 1] = mkp(v.z, v.w);
+    }
+}
+template <typename T>
+__device__ __forceinline__ void store_spinor(float* __restrict__ base, int Vs, int idx, const P2 (&s)[24])
+{
+    float4* p = reinterpret_cast<float4*>(base) + idx;
+#pragma unroll
+    for (int h = 0; h < 12; ++h) p[(size_t)h * Vs] = make_float4(s[2 * h].v.x, s[2 * h].v.y, s[2 * h + 1].v.x, s[2 * h + 1].v.y);
 }
 
 // 18 reals of one link; blk = start of the (parity, mu) block

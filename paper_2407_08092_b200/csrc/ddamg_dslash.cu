@@ -32,46 +32,50 @@ extern template void launch_dslash_recon<double, 12>(const Geom&, int, bool, int
 template <typename T>
 void launch_dslash(const Geom& g, int epi, bool norm, int parity, const void* in, const void* gauge_own,
                    const void* gauge_opp, const void* clov, const void* own, const void* rhs, void* out,
-                   double omega, double* partials, int nrhs, double batch_l2_bytes, int recon, int apbc,
+                   double omega, double* partials, int units, double batch_l2_bytes, int recon, int apbc,
                    cudaStream_t st)
 {
     if (recon == 12)
         launch_dslash_recon<T, 12>(g, epi, norm, parity, in, gauge_own, gauge_opp, clov, own, rhs, out, omega, partials,
-                                   nrhs, batch_l2_bytes, apbc, st);
+                                   units, batch_l2_bytes, apbc, st);
     else
         launch_dslash_recon<T, 18>(g, epi, norm, parity, in, gauge_own, gauge_opp, clov, own, rhs, out, omega, partials,
-                                   nrhs, batch_l2_bytes, apbc, st);
+                                   units, batch_l2_bytes, apbc, st);
 }
 template void launch_dslash<float>(const Geom&, int, bool, int, const void*, const void*, const void*, const void*,
                                    const void*, const void*, void*, double, double*, int, double, int, int, cudaStream_t);
 template void launch_dslash<double>(const Geom&, int, bool, int, const void*, const void*, const void*, const void*,
                                     const void*, const void*, void*, double, double*, int, double, int, int, cudaStream_t);
 
-// out = Cl in on one parity (right factor of eq. 2: t_o = A_oo^-1 b_o)
-template <typename T>
+// out = Cl in on one parity (right factor of eq. 2: t_o = A_oo^-1 b_o); units as in launch_dslash
+template <typename T, bool BATCH>
 __global__ void __launch_bounds__(DSLASH_THREADS)
-clover_apply_kernel(Geom g, int nrhs, const T* __restrict__ clov, const T* __restrict__ in, T* __restrict__ out)
+clover_apply_kernel(Geom g, int units, const T* __restrict__ clov, const T* __restrict__ in, T* __restrict__ out)
 {
+    using S = typename ValueOf<T, BATCH>::type;
     const int tid = blockIdx.x * DSLASH_THREADS + threadIdx.x;
-    const int cb = tid / nrhs;
+    const int cb = tid / units;
     if (cb >= g.Vh) return;
-    T v[24], res[24];
-    load_spinor<T, true>(in, g.Vh * nrhs, tid, v);
+    S v[24], res[24];
+    load_spinor<T, true>(in, g.Vh * units, tid, v);
     clover_site_mul<T>(clov, g.Vh, cb, v, res);
-    store_spinor<T>(out, g.Vh * nrhs, tid, res);
+    store_spinor<T>(out, g.Vh * units, tid, res);
 }
 
 template <typename T>
-void launch_clover_apply(const Geom& g, const void* clov, const void* in, void* out, int nrhs, cudaStream_t st)
+void launch_clover_apply(const Geom& g, const void* clov, const void* in, void* out, int units, cudaStream_t st)
 {
-    clover_apply_kernel<T><<<dslash_grid(g, nrhs), DSLASH_THREADS, 0, st>>>(g, nrhs, (const T*)clov, (const T*)in, (T*)out);
+    if (units > 0)
+        clover_apply_kernel<T, true><<<dslash_grid(g, units), DSLASH_THREADS, 0, st>>>(g, units, (const T*)clov, (const T*)in, (T*)out);
+    else
+        clover_apply_kernel<T, false><<<dslash_grid(g, 1), DSLASH_THREADS, 0, st>>>(g, 1, (const T*)clov, (const T*)in, (T*)out);
 }
 template void launch_clover_apply<float>(const Geom&, const void*, const void*, void*, int, cudaStream_t);
 template void launch_clover_apply<double>(const Geom&, const void*, const void*, void*, int, cudaStream_t);
 
-int dslash_grid(const Geom& g, int nrhs)
+int dslash_grid(const Geom& g, int units)
 {
-    return (int)(((long long)g.Vh * nrhs + DSLASH_THREADS - 1) / DSLASH_THREADS);
+    return (int)(((long long)g.Vh * units + DSLASH_THREADS - 1) / DSLASH_THREADS);
 }
 
 }  // namespace ddamg

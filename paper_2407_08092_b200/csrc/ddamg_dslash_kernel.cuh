@@ -19,8 +19,8 @@ struct DslashArgs {
     const T* rhs;            // b (EPI_RICHARDSON / RESIDUAL / *_RHS_*)
     T* out;
     T omega;
-    double* partials;        // per-block sum of |r|^2 (NORM) or nullptr; batch: [block][nrhs]
-    int nrhs;                // BATCH kernels: right-hand sides interleaved per site (else 1)
+    double* partials;        // per-block sum of |r|^2 (NORM) or nullptr; batch: [block][units * lanes]
+    int nrhs;                // BATCH kernels: threads (units) per site = rhs pairs (fp32) or rhs (fp64); else 1
     int zc;                  // BATCH: z-chunk of the CTA traversal (0 = plain lexicographic order)
     int cpp;                 // BATCH: CTAs per (z,t) plane = Lh * L * nrhs / DSLASH_THREADS (when zc > 0)
     int apbc;                // RECON = 12: antiperiodic time boundary (sign of the rebuilt third row of U_t(T-1))
@@ -56,15 +56,25 @@ __device__ __forceinline__ double block_sum(double v)
 #define DDAMG_MAXREG_BATCH 128     // multi-rhs kernels
 #endif
 
-// BATCH (multi-rhs): one thread per (site, rhs), rhs fastest, so that the
-// nrhs threads of a site share every link / clover vector they load while all spinor planes
-// stay contiguous per warp (vector index cb * nrhs + r).
+// spinor value type of a kernel: one value per thread, or (fp32 multi-rhs) a packed pair of
+// right-hand sides per thread
+template <typename T, bool BATCH> struct ValueOf { using type = T; static constexpr int LANES = 1; };
+template <> struct ValueOf<float, true> { using type = P2; static constexpr int LANES = 2; };
+
+// BATCH (multi-rhs): one thread per (site, unit), unit fastest, so that the
+// threads of a site share every link / clover vector they load while all spinor planes stay
+// contiguous per warp (vector index cb * units + r).  fp32: a unit is a PAIR of right-hand
+// sides carried through the whole site update as the two lanes of packed f32x2 instructions
+// (links, the rebuilt third rows, clover entries and every index computation are shared by
+// the pair); fp64: a unit is one right-hand side.  a.nrhs = units per site.
 template <typename T, int EPI, bool NORM, bool BATCH, int RECON>
 __global__ void __launch_bounds__(DSLASH_THREADS)
 __maxnreg__(sizeof(T) == 4 ? (BATCH ? DDAMG_MAXREG_BATCH : EPI <= EPI_RHS_MINUS_HOP ? DDAMG_MAXREG_A : DDAMG_MAXREG_B) : 255)
 dslash_kernel(const DslashArgs<T> a)
 {
-    // BATCH: with nrhs spinors per site one time slice of neighbour spinors no longer fits L2
+    using S = typename ValueOf<T, BATCH>::type;
+    constexpr int LANES = ValueOf<T, BATCH>::LANES;
+    // BATCH: with several spinors per site one time slice of neighbour spinors no longer fits L2
     // (64^3: nrhs * 12.6 MB), so the t-1 neighbours would be re-fetched from HBM.  CTAs therefore
     // walk the lattice in z-chunks: for each chunk of zc z-planes, t runs over the whole time
     // extent before the next chunk starts, which keeps three t-slabs of the chunk L2-resident.
@@ -77,34 +87,34 @@ dslash_kernel(const DslashArgs<T> a)
         blk = (t * a.g.L + z) * a.cpp + within;
     }
     const int tid = blk * DSLASH_THREADS + threadIdx.x;
-    const int nrhs = BATCH ? a.nrhs : 1;
-    const int cb = BATCH ? tid / nrhs : tid;
-    const int rr = BATCH ? tid - cb * nrhs : 0;
-    const int Vs = a.g.Vh * nrhs;          // vectors per spinor plane
-    const int sv = cb * nrhs + rr;         // this thread's vector index in a spinor plane (== tid)
-    double nrm = 0.0;
+    const int units = BATCH ? a.nrhs : 1;
+    const int cb = BATCH ? tid / units : tid;
+    const int rr = BATCH ? tid - cb * units : 0;
+    const int Vs = a.g.Vh * units;         // vectors per spinor plane
+    const int sv = cb * units + rr;        // this thread's vector index in a spinor plane (== tid)
+    double nrm[2] = { 0.0, 0.0 };
     if (cb < a.g.Vh) {
         const Site s = site_of_cb(a.g, cb, a.parity);
-        T acc[24];
-        hop_site<T, RECON>(a.g, cb, s, a.in, nrhs, rr, a.gauge_own, a.gauge_opp, acc, a.apbc);
-        T res[24];
+        S acc[24];
+        hop_site<T, RECON, S>(a.g, cb, s, a.in, units, rr, a.gauge_own, a.gauge_opp, acc, a.apbc);
+        S res[24];
         if (EPI == EPI_CLOV_HOP) {
 #pragma unroll
-            for (int i = 0; i < 24; ++i) acc[i] *= (T)(-0.5);
+            for (int i = 0; i < 24; ++i) acc[i] = vmul((T)(-0.5), acc[i]);
             clover_site_mul<T>(a.clov, a.g.Vh, cb, acc, res);
         } else if (EPI == EPI_CLOV_RHS_MINUS_HOP) {
-            T b[24];
+            S b[24];
             load_spinor<T, true>(a.rhs, Vs, sv, b);
 #pragma unroll
-            for (int i = 0; i < 24; ++i) acc[i] = b[i] + (T)0.5 * acc[i];
+            for (int i = 0; i < 24; ++i) acc[i] = vfma((T)0.5, acc[i], b[i]);
             clover_site_mul<T>(a.clov, a.g.Vh, cb, acc, res);
         } else if (EPI == EPI_RHS_MINUS_HOP) {
-            T b[24];
+            S b[24];
             load_spinor<T, true>(a.rhs, Vs, sv, b);
 #pragma unroll
-            for (int i = 0; i < 24; ++i) res[i] = b[i] + (T)0.5 * acc[i];
+            for (int i = 0; i < 24; ++i) res[i] = vfma((T)0.5, acc[i], b[i]);
         } else {
-            T x[24], ax[24];
+            S x[24], ax[24];
             load_spinor<T, true>(a.own, Vs, sv, x);
             clover_site_mul<T>(a.clov, a.g.Vh, cb, x, ax);
             // H = -1/2 acc:  Schur forms subtract H t (+1/2 acc), the full operator adds H x (-1/2 acc)
@@ -112,15 +122,15 @@ dslash_kernel(const DslashArgs<T> a)
             const T hs = FULL ? (T)(-0.5) : (T)0.5;
             if (EPI == EPI_SCHUR || EPI == EPI_FULL) {
 #pragma unroll
-                for (int i = 0; i < 24; ++i) res[i] = ax[i] + hs * acc[i];     // A x - H t   or   A x + H x'
+                for (int i = 0; i < 24; ++i) res[i] = vfma(hs, acc[i], ax[i]);     // A x - H t   or   A x + H x'
             } else {
-                T b[24];
+                S b[24];
                 load_spinor<T, true>(a.rhs, Vs, sv, b);
 #pragma unroll
                 for (int i = 0; i < 24; ++i) {
-                    const T r = b[i] - (ax[i] + hs * acc[i]);
-                    if (NORM) nrm += (double)r * (double)r;
-                    res[i] = (EPI == EPI_RICHARDSON) ? x[i] + a.omega * r : r;
+                    const S r = b[i] - vfma(hs, acc[i], ax[i]);
+                    if (NORM) vnorm_add(r, nrm);
+                    res[i] = (EPI == EPI_RICHARDSON) ? vfma(a.omega, r, x[i]) : r;
                 }
             }
         }
@@ -128,20 +138,23 @@ dslash_kernel(const DslashArgs<T> a)
     }
     if (NORM) {
         if (BATCH) {
-            // per-rhs partial sums of this block: thread q < nrhs adds the entries of rhs q
-            __shared__ double per_thread[DSLASH_THREADS];
-            per_thread[threadIdx.x] = nrm;
+            // per-rhs partial sums of this block: thread q < units * LANES adds the entries of rhs q
+            // (rhs = unit * LANES + lane); partials[block][units * LANES]
+            __shared__ double per_thread[LANES][DSLASH_THREADS];
+            per_thread[0][threadIdx.x] = nrm[0];
+            if (LANES == 2) per_thread[LANES - 1][threadIdx.x] = nrm[1];
             __syncthreads();
-            if ((int)threadIdx.x < nrhs) {
-                const int first = (int)(((long long)blk * DSLASH_THREADS) % nrhs);          // rhs of thread 0
-                int i = (int)threadIdx.x - first;
-                if (i < 0) i += nrhs;
+            if ((int)threadIdx.x < units * LANES) {
+                const int unit = (int)threadIdx.x / LANES, lane = (int)threadIdx.x - unit * LANES;
+                const int first = (int)(((long long)blk * DSLASH_THREADS) % units);          // unit of thread 0
+                int i = unit - first;
+                if (i < 0) i += units;
                 double tot = 0.0;
-                for (; i < DSLASH_THREADS; i += nrhs) tot += per_thread[i];
-                a.partials[(size_t)blk * nrhs + threadIdx.x] = tot;
+                for (; i < DSLASH_THREADS; i += units) tot += per_thread[lane][i];
+                a.partials[(size_t)blk * units * LANES + threadIdx.x] = tot;
             }
         } else {
-            const double tot = block_sum(nrm);
+            const double tot = block_sum(nrm[0]);
             if (threadIdx.x == 0) a.partials[blockIdx.x] = tot;
         }
     }
@@ -150,25 +163,27 @@ dslash_kernel(const DslashArgs<T> a)
 template <typename T, int EPI, bool NORM, int RECON>
 static void launch(const DslashArgs<T>& a, cudaStream_t st)
 {
-    const int grid = dslash_grid(a.g, a.nrhs);
-    if (a.nrhs > 1) dslash_kernel<T, EPI, NORM, true, RECON><<<grid, DSLASH_THREADS, 0, st>>>(a);
-    else dslash_kernel<T, EPI, NORM, false, RECON><<<grid, DSLASH_THREADS, 0, st>>>(a);
+    if (a.nrhs > 0) dslash_kernel<T, EPI, NORM, true, RECON><<<dslash_grid(a.g, a.nrhs), DSLASH_THREADS, 0, st>>>(a);
+    else dslash_kernel<T, EPI, NORM, false, RECON><<<dslash_grid(a.g, 1), DSLASH_THREADS, 0, st>>>(a);
 }
 
 template <typename T, int RECON>
 void launch_dslash_recon(const Geom& g, int epi, bool norm, int parity, const void* in, const void* gauge_own,
                          const void* gauge_opp, const void* clov, const void* own, const void* rhs, void* out,
-                         double omega, double* partials, int nrhs, double batch_l2_bytes, int apbc, cudaStream_t st)
+                         double omega, double* partials, int units, double batch_l2_bytes, int apbc, cudaStream_t st)
 {
+    // units = 0: one right-hand side in the native half-spinor layout; units >= 1: multi-rhs batch with
+    // that many threads per site (fp32: rhs pairs, fp64: rhs)
     DslashArgs<T> a;
     a.apbc = apbc;
-    a.nrhs = nrhs;
+    a.nrhs = units;
     a.zc = 0;
     a.cpp = 0;
-    const long long plane_threads = (long long)g.Lh * g.L * nrhs;
-    if (nrhs > 1 && plane_threads % DSLASH_THREADS == 0) {
+    const long long plane_threads = (long long)g.Lh * g.L * units;
+    const int lanes = sizeof(T) == 4 ? 2 : 1;
+    if (units * lanes > 1 && plane_threads % DSLASH_THREADS == 0) {
         // largest divisor zc of L whose three t-slabs of spinors (zc planes each) fit the L2 budget
-        const double plane_bytes = (double)g.Lh * g.L * nrhs * 24 * sizeof(T);
+        const double plane_bytes = (double)g.Lh * g.L * units * lanes * 24 * sizeof(T);
         int zc = 0;
         for (int d = 1; d <= g.L; ++d)
             if (g.L % d == 0 && 3.0 * d * plane_bytes <= batch_l2_bytes) zc = d;

@@ -32,8 +32,12 @@ enum {
 template <typename T>
 void launch_dslash(const Geom& g, int epi, bool norm, int parity, const void* in, const void* gauge_own,
                    const void* gauge_opp, const void* clov, const void* own, const void* rhs, void* out,
-                   double omega, double* partials, int nrhs, double batch_l2_bytes, int recon, int apbc,
+                   double omega, double* partials, int units, double batch_l2_bytes, int recon, int apbc,
                    cudaStream_t st);
+// `units`: 0 = one right-hand side in the native half-spinor layout; >= 1 = multi-rhs batch processed by that
+// many threads per site: fp32 -> pairs of right-hand sides (pair layout, batch_units()), fp64 -> right-hand sides
+inline int batch_units(int nrhs, size_t real_bytes) { return real_bytes == 4 ? (nrhs + 1) / 2 : nrhs; }
+inline int batch_slots(int nrhs, size_t real_bytes) { return real_bytes == 4 ? 2 * ((nrhs + 1) / 2) : nrhs; }   // rhs slots incl. padding
 // two-row copy of the packed gauge field (option "gauge_recon" = 12) + max deviation of the
 // stored third rows from conj(row0 x row1): *dev_max_bits = bit pattern of the largest
 // absolute deviation as a non-negative float (atomicMax on the bits; zero it first)
@@ -41,8 +45,8 @@ template <typename T>
 void launch_compress_gauge(const Geom& g, int bc, const void* gauge, void* gauge12, unsigned int* dev_max_bits,
                            cudaStream_t st);
 template <typename T>
-void launch_clover_apply(const Geom& g, const void* clov, const void* in, void* out, int nrhs, cudaStream_t st);
-int dslash_grid(const Geom& g, int nrhs = 1);
+void launch_clover_apply(const Geom& g, const void* clov, const void* in, void* out, int units, cudaStream_t st);
+int dslash_grid(const Geom& g, int units = 1);
 
 // ---- SAP block solves (ddamg_sap.cu)
 struct SapGeom {
@@ -109,7 +113,8 @@ struct Scalars {
 int blas_grid_cap();
 // dst = sqrt(sum partials); stores into sc->value, optionally appends to sc->hist, sets sc->scale = 1/value
 void launch_finalize_norm(const double* partials, int n, Scalars* sc, int append_hist, cudaStream_t st);
-void launch_finalize_norm_batch(const double* partials, int nblocks, int nrhs, Scalars* sc, int offset, cudaStream_t st);
+// multi-rhs: partials[block][stride], the first nrhs of each row are right-hand sides (the rest padding)
+void launch_finalize_norm_batch(const double* partials, int nblocks, int nrhs, int stride, Scalars* sc, int offset, cudaStream_t st);
 template <typename T>
 int launch_copy_norm(size_t nreal, const void* src, void* dst, double* partials, cudaStream_t st);
 template <typename T>

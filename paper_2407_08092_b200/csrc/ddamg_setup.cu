@@ -169,13 +169,12 @@ template void launch_unpack_spinor<float>(const Geom&, const void*, const void*,
 template void launch_unpack_spinor<double>(const Geom&, const void*, const void*, void*, cudaStream_t);
 
 // ------------------------------------------------------------------ multi-rhs interleave
-// X[plane][cb * nrhs + r] = halves[r][plane][cb]  (TO_BATCH) or the inverse.  One thread per
+// fp64:  X[plane][cb * nrhs + r] = halves[r][plane][cb]  (TO_BATCH) or the inverse.  One thread per
 // vector of the batch; writes (TO_BATCH) / reads (inverse) of the batch are contiguous.
-template <typename T, bool TO_BATCH>
-__global__ void batch_interleave_kernel(int Vh, int nrhs, typename VecOf<T>::type* __restrict__ halves,
-                                        typename VecOf<T>::type* __restrict__ X)
+template <bool TO_BATCH>
+__global__ void batch_interleave_kernel(int Vh, int nrhs, double2* __restrict__ halves, double2* __restrict__ X)
 {
-    constexpr int NP = 24 / VecOf<T>::N;
+    constexpr int NP = 12;
     const size_t per_plane = (size_t)Vh * nrhs;
     const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= per_plane * NP) return;
@@ -186,17 +185,51 @@ __global__ void batch_interleave_kernel(int Vh, int nrhs, typename VecOf<T>::typ
     if (TO_BATCH) X[i] = halves[h];
     else halves[h] = X[i];
 }
-template <typename T>
-void launch_batch_interleave(const Geom& g, int nrhs, bool to_batch, void* halves, void* X, cudaStream_t st)
+// fp32 pair layout (ddamg_common.cuh, load_spinor of P2): 12 half-planes of float4; half-plane h, vector
+// cb * npairs + p = (re, re', im, im') of complex number h of the site for the rhs 2p and 2p+1.  An odd nrhs
+// leaves the second lane of the last pair as padding: written as 0 (TO_BATCH), ignored (inverse).
+template <bool TO_BATCH>
+__global__ void batch_interleave_pairs_kernel(int Vh, int nrhs, float2* __restrict__ halves, float4* __restrict__ X)
 {
-    using V = typename VecOf<T>::type;
-    const size_t n = (size_t)g.Vh * nrhs * (24 / VecOf<T>::N);
-    const unsigned grid = (unsigned)((n + 255) / 256);
-    if (to_batch) batch_interleave_kernel<T, true><<<grid, 256, 0, st>>>(g.Vh, nrhs, (V*)halves, (V*)X);
-    else batch_interleave_kernel<T, false><<<grid, 256, 0, st>>>(g.Vh, nrhs, (V*)halves, (V*)X);
+    const int npairs = (nrhs + 1) / 2;
+    const size_t per_plane = (size_t)Vh * npairs;
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= per_plane * 12) return;
+    const int h = (int)(i / per_plane);
+    const size_t rem = i - (size_t)h * per_plane;
+    const int cb = (int)(rem / npairs), p = (int)(rem - (size_t)cb * npairs);
+    // complex number h of a native half spinor = float2 number (h & 1) of the float4 at plane h / 2
+    const size_t per_rhs = (size_t)12 * Vh;                       // float2 per half spinor
+    const size_t src = ((size_t)(h >> 1) * Vh + cb) * 2 + (h & 1);
+    const int r0 = 2 * p, r1 = 2 * p + 1;
+    if (TO_BATCH) {
+        const float2 a = halves[(size_t)r0 * per_rhs + src];
+        const float2 b = r1 < nrhs ? halves[(size_t)r1 * per_rhs + src] : make_float2(0.f, 0.f);
+        X[i] = make_float4(a.x, b.x, a.y, b.y);
+    } else {
+        const float4 v = X[i];
+        halves[(size_t)r0 * per_rhs + src] = make_float2(v.x, v.z);
+        if (r1 < nrhs) halves[(size_t)r1 * per_rhs + src] = make_float2(v.y, v.w);
+    }
 }
-template void launch_batch_interleave<float>(const Geom&, int, bool, void*, void*, cudaStream_t);
-template void launch_batch_interleave<double>(const Geom&, int, bool, void*, void*, cudaStream_t);
+template <typename T>
+void launch_batch_interleave(const Geom& g, int nrhs, bool to_batch, void* halves, void* X, cudaStream_t st);
+template <>
+void launch_batch_interleave<double>(const Geom& g, int nrhs, bool to_batch, void* halves, void* X, cudaStream_t st)
+{
+    const size_t n = (size_t)g.Vh * nrhs * 12;
+    const unsigned grid = (unsigned)((n + 255) / 256);
+    if (to_batch) batch_interleave_kernel<true><<<grid, 256, 0, st>>>(g.Vh, nrhs, (double2*)halves, (double2*)X);
+    else batch_interleave_kernel<false><<<grid, 256, 0, st>>>(g.Vh, nrhs, (double2*)halves, (double2*)X);
+}
+template <>
+void launch_batch_interleave<float>(const Geom& g, int nrhs, bool to_batch, void* halves, void* X, cudaStream_t st)
+{
+    const size_t n = (size_t)g.Vh * ((nrhs + 1) / 2) * 12;
+    const unsigned grid = (unsigned)((n + 255) / 256);
+    if (to_batch) batch_interleave_pairs_kernel<true><<<grid, 256, 0, st>>>(g.Vh, nrhs, (float2*)halves, (float4*)X);
+    else batch_interleave_pairs_kernel<false><<<grid, 256, 0, st>>>(g.Vh, nrhs, (float2*)halves, (float4*)X);
+}
 
 // ------------------------------------------------------------------ a1: clover build
 struct M3 { double re[9], im[9]; };

@@ -31,10 +31,19 @@ def test_batch_interleave_layout_and_roundtrip(prec, nrhs):
     _, halves = _spinors(p, nrhs, 7000)
     H = torch.stack([h[0] for h in halves])                  # (nrhs, 24 * Vh)
     X = p.ctx.batch_interleave(H)
-    nv = 4 if prec == "f32" else 2                           # reals per 16-byte vector
     Vh = p.ctx.V // 2
-    # documented layout: plane j, vector index cb * nrhs + r
-    expect = H.view(nrhs, 24 // nv, Vh, nv).permute(1, 2, 0, 3).contiguous().view(-1)
+    if prec == "f64":
+        # documented layout (include/ddamg.h): plane j of double2, vector index cb * nrhs + r
+        expect = H.view(nrhs, 12, Vh, 2).permute(1, 2, 0, 3).contiguous().view(-1)
+    else:
+        # documented fp32 layout: 12 half-planes of float4; half-plane h, vector cb * npairs + p =
+        # (re, re', im, im') of complex number h of the site for the rhs 2p, 2p+1 (odd nrhs: zero padding)
+        npairs = (nrhs + 1) // 2
+        Hp = torch.zeros(2 * npairs, 24 * Vh, dtype=H.dtype, device=H.device)
+        Hp[:nrhs] = H
+        c = Hp.view(npairs, 2, 6, Vh, 2, 2)                  # pair, lane, plane, cb, complex-in-vector, re/im
+        expect = c.permute(2, 4, 3, 0, 5, 1).contiguous().view(-1)     # plane, complex, cb, pair, re/im, lane
+    assert X.numel() == expect.numel()
     assert torch.equal(X, expect)
     assert torch.equal(p.ctx.batch_deinterleave(nrhs, X), H)
 
@@ -101,7 +110,7 @@ def test_batch_richardson_matches_oracle(cfg, prec, L, T, nrhs, nu):
     # x0 = 0
     Z = torch.full_like(X_e, 3.0)
     p.ctx.richardson_batch(nrhs, B_e, Z, 1, omega, zero_init=True)
-    assert torch.equal(Z, B_e * omega)
+    assert torch.equal(Z, B_e * omega)                      # (padding lanes of an odd fp32 batch are 0 in both)
 
 
 def test_batch_error_codes():

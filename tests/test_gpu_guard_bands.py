@@ -71,7 +71,7 @@ def test_outputs_stay_inside_their_buffers(L, T, prec, recon):
     ctx.lib.ddamg_unpack_spinor(ctx._h, x_e.data_ptr(), x_o.data_ptr(), gn.view.data_ptr()); gn.check("unpack_spinor")
     # multi-rhs
     nrhs = 3
-    gb = Guarded(ctx, nrhs * n, rdt)
+    gb = Guarded(ctx, ctx.batch_numel(nrhs), rdt)               # fp32: rhs pairs, the odd rhs is padded
     X = ctx.batch_interleave([x_e, b_e, x_e])
     ctx.apply_schur_batch(nrhs, X, gb.view); gb.check("apply_schur_batch")
     gb.view.copy_(X)
