@@ -45,6 +45,8 @@ struct ddamg_ctx {
     void* sap_links;            // SAP: block-ordered copy of the links (launch_sap_reorder), or NULL
     void* sap_clov;             // SAP: block-ordered copy of A_ee / A_oo^-1
     int sap_built[4];           // block extents the two copies were built for ({0,..} = stale)
+    int sap_built_recon;        // link format (18 / 12 reals) of the block-ordered link copy
+    void* sap_e;                // SAP: the update e of the last solved colour, even half then odd half
     int sap_block[4];           // SAP block extents used when SAP is the FGMRES smoother (options "sap_block_x".."_t")
     // CUDA-graph replay of a history-free Richardson call (option "cuda_graph"): the 2 nu launches are captured
     // once on cap_stream (nothing ever executes there) and replayed on the context's stream
@@ -229,7 +231,7 @@ extern "C" int ddamg_create(ddamg_ctx** out, int L, int T, double csw, double m0
     ctx->clov_oo = nullptr; ctx->sc2 = nullptr; ctx->fgm_basis = nullptr; ctx->fgm_cap = 0;
     ctx->tmp_batch = nullptr; ctx->partials_batch = nullptr; ctx->batch_cap = 0; ctx->batch_l2_bytes = 40e6;
     for (int mu = 0; mu < 4; ++mu) ctx->sap_block[mu] = 4;
-    ctx->sap_links = ctx->sap_clov = nullptr;
+    ctx->sap_links = ctx->sap_clov = ctx->sap_e = nullptr; ctx->sap_built_recon = 0;
     for (int mu = 0; mu < 4; ++mu) ctx->sap_built[mu] = 0;
     ctx->partials = nullptr; ctx->sc = nullptr; ctx->host_hist = nullptr; ctx->singular = nullptr;
     ctx->have_gauge = ctx->have_clover = ctx->have_clov_oo = false;
@@ -274,7 +276,7 @@ extern "C" int ddamg_destroy(ddamg_ctx* ctx)
     if (ctx->rich_exec) cudaGraphExecDestroy(ctx->rich_exec);
     if (ctx->cap_stream) cudaStreamDestroy(ctx->cap_stream);
     cudaFree(ctx->gauge12); cudaFree(ctx->recon_dev);
-    cudaFree(ctx->sap_links); cudaFree(ctx->sap_clov);
+    cudaFree(ctx->sap_links); cudaFree(ctx->sap_clov); cudaFree(ctx->sap_e);
     cudaFree(ctx->gauge); cudaFree(ctx->clov[0]); cudaFree(ctx->clov[1]);
     cudaFree(ctx->tmp_o); cudaFree(ctx->tmp_e); cudaFree(ctx->krylov);
     cudaFree(ctx->tmp_batch); cudaFree(ctx->partials_batch);
@@ -1165,7 +1167,7 @@ static int sap_geometry(ddamg_ctx* ctx, const int* block, SapGeom* sg, const cha
     int dev = 0, optin = 0;
     if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) != cudaSuccess)
         return check_cuda(ctx, cudaGetLastError(), "cudaDeviceGetAttribute");
-    if (sap_smem_bytes(*sg, ctx->real_bytes) > (size_t)optin)
+    if (sap_smem_bytes(*sg, ctx->real_bytes, ctx->recon) > (size_t)optin)
         return fail(ctx, DDAMG_EINVAL, std::string(who) + ": the block's links do not fit in shared memory at this precision");
     return DDAMG_OK;
 }
@@ -1186,61 +1188,105 @@ extern "C" int ddamg_sap(ddamg_ctx* ctx, const void* b_e, const void* b_o, void*
     const bool hist = res_hist != nullptr;
     const bool f32 = ctx->prec == DDAMG_F32;
     const int dgrid = dslash_grid(ctx->g);
+    const int recon = ctx->recon;             // two-row links (validated SU(3)) are also staged as two rows in shared memory
     // block-ordered links and clover blocks for this geometry (built once, kept until the
-    // gauge field, the clover term or the block extents change)
-    if (m > 0 && memcmp(ctx->sap_built, sg.B, sizeof(int) * 4) != 0) {
+    // gauge field, the clover term, the link format or the block extents change)
+    if (m > 0 && (memcmp(ctx->sap_built, sg.B, sizeof(int) * 4) != 0 || ctx->sap_built_recon != recon)) {
         if (!ctx->sap_links) {
             cudaError_t e = cudaMalloc(&ctx->sap_links, (size_t)2 * 4 * 18 * ctx->g.Vh * ctx->real_bytes);
             if (e == cudaSuccess) e = cudaMalloc(&ctx->sap_clov, (size_t)2 * 72 * ctx->g.Vh * ctx->real_bytes);
+            if (e == cudaSuccess) e = cudaMalloc(&ctx->sap_e, 2 * ctx->half_bytes);
             if (e != cudaSuccess) {
                 cudaGetLastError();
                 cudaFree(ctx->sap_links); ctx->sap_links = nullptr;
+                cudaFree(ctx->sap_clov); ctx->sap_clov = nullptr;
                 return fail(ctx, DDAMG_ENOMEM, "ddamg_sap: cannot allocate the block-ordered operand copies");
             }
         }
-        if (f32) launch_sap_reorder<float>(ctx->g, sg, ctx->gauge, ctx->clov[0], ctx->clov[1], ctx->sap_links, ctx->sap_clov, st);
-        else launch_sap_reorder<double>(ctx->g, sg, ctx->gauge, ctx->clov[0], ctx->clov[1], ctx->sap_links, ctx->sap_clov, st);
+        if (f32) launch_sap_reorder<float>(ctx->g, sg, recon, ctx->gauge, ctx->clov[0], ctx->clov[1], ctx->sap_links, ctx->sap_clov, st);
+        else launch_sap_reorder<double>(ctx->g, sg, recon, ctx->gauge, ctx->clov[0], ctx->clov[1], ctx->sap_links, ctx->sap_clov, st);
         s = after_launch(ctx);
         if (s != DDAMG_OK) return s;
         memcpy(ctx->sap_built, sg.B, sizeof(int) * 4);
+        ctx->sap_built_recon = recon;
     }
     if (hist) { s = reset_hist(ctx); if (s != DDAMG_OK) return s; }
     if (zero_init) {
         CK(cudaMemsetAsync(x_e, 0, ctx->half_bytes, st));
         CK(cudaMemsetAsync(x_o, 0, ctx->half_bytes, st));
     }
-    // r = b - D x into (tmp_e, tmp_o); with a history also ||r||
-    auto residual = [&](bool norm) -> int {
-        int q = dslash(ctx, EPI_FULL_RESIDUAL, norm, 0, x_o, x_e, b_e, ctx->tmp_e, 0.0, 5);
-        if (q != DDAMG_OK) return q;
-        q = dslash(ctx, EPI_FULL_RESIDUAL, norm, 1, x_e, x_o, b_o, ctx->tmp_o, 0.0, 5, 0, (size_t)dgrid, ctx->clov_oo);
-        if (q != DDAMG_OK) return q;
-        if (norm) { launch_finalize_norm(ctx->partials, 2 * dgrid, ctx->sc, 1, st); q = after_launch(ctx); }
-        return q;
+    void* r_e = ctx->tmp_e;                                  // the residual r = b - D x, kept up to date incrementally
+    void* r_o = ctx->tmp_o;
+    void* e_e = ctx->sap_e;
+    void* e_o = ctx->sap_e ? (char*)ctx->sap_e + ctx->half_bytes : nullptr;
+    // ||r|| of the maintained residual -> history
+    auto append_norm = [&]() -> int {
+        const int n1 = f32 ? launch_copy_norm<float>(ctx->nreal, r_e, r_e, ctx->partials, st)
+                           : launch_copy_norm<double>(ctx->nreal, r_e, r_e, ctx->partials, st);
+        const int n2 = f32 ? launch_copy_norm<float>(ctx->nreal, r_o, r_o, ctx->partials + n1, st)
+                           : launch_copy_norm<double>(ctx->nreal, r_o, r_o, ctx->partials + n1, st);
+        launch_finalize_norm(ctx->partials, n1 + n2, ctx->sc, 1, st);
+        return after_launch(ctx, 3);
     };
-    auto blocks = [&](int colour, const void* r_e, const void* r_o) -> int {
-        if (m == 0) return DDAMG_OK;                       // zero Minimal Residual iterations: e_k = 0
-        KernelTimer kt(ctx, KT_SAP);
-        cudaError_t e = f32
-            ? launch_sap_blocks<float>(ctx->g, sg, colour, m, ctx->sap_links, ctx->sap_clov, r_e, r_o, x_e, x_o, st)
-            : launch_sap_blocks<double>(ctx->g, sg, colour, m, ctx->sap_links, ctx->sap_clov, r_e, r_o, x_e, x_o, st);
-        if (e != cudaSuccess) return check_cuda(ctx, e, "sap_block_kernel attributes");
+    // block solves of one colour (Alg. 1 lines 4-6 / 8-10), then the residual of the other colour's sites (line 7 / 2)
+    auto half_iteration = [&](int colour, const void* rin_e, const void* rin_o, bool update_other) -> int {
+        {
+            KernelTimer kt(ctx, KT_SAP);
+            cudaError_t e = f32
+                ? launch_sap_blocks<float>(ctx->g, sg, recon, colour, m, ctx->sap_links, ctx->sap_clov, rin_e, rin_o, r_e, r_o, e_e, e_o, x_e, x_o, st)
+                : launch_sap_blocks<double>(ctx->g, sg, recon, colour, m, ctx->sap_links, ctx->sap_clov, rin_e, rin_o, r_e, r_o, e_e, e_o, x_e, x_o, st);
+            if (e != cudaSuccess) return check_cuda(ctx, e, "sap_block_kernel attributes");
+        }
+        int q = after_launch(ctx);
+        if (q != DDAMG_OK || !update_other) return q;
+        {
+            KernelTimer kt(ctx, KT_FULL);
+            if (f32) launch_sap_boundary<float>(ctx->g, sg, recon, 1 - colour, ctx->bc == 1, hop_gauge_block(ctx, 0), e_e, e_o, rin_e, rin_o, r_e, r_o, st);
+            else launch_sap_boundary<double>(ctx->g, sg, recon, 1 - colour, ctx->bc == 1, hop_gauge_block(ctx, 0), e_e, e_o, rin_e, rin_o, r_e, r_o, st);
+        }
         return after_launch(ctx);
     };
-    for (int i = 0; i < n; ++i) {
-        if (i == 0 && zero_init && !hist) {
-            // line 2 with x = 0: r = b - D 0 = b exactly, so the red blocks read b itself (the smoother
-            // use: one residual evaluation of 2n saved)
-            s = blocks(0, b_e, b_o); if (s != DDAMG_OK) return s;
-        } else {
-            s = residual(hist); if (s != DDAMG_OK) return s;         // line 2
-            s = blocks(0, ctx->tmp_e, ctx->tmp_o); if (s != DDAMG_OK) return s;   // lines 4-6: red blocks
+    if (m == 0 || n == 0) {
+        // zero Minimal Residual iterations: every e_k = 0, SAP is the identity; the history repeats ||b - D x||
+        if (hist) {
+            s = dslash(ctx, EPI_FULL_RESIDUAL, true, 0, x_o, x_e, b_e, r_e, 0.0, 5);
+            if (s != DDAMG_OK) return s;
+            s = dslash(ctx, EPI_FULL_RESIDUAL, true, 1, x_e, x_o, b_o, r_o, 0.0, 5, 0, (size_t)dgrid, ctx->clov_oo);
+            if (s != DDAMG_OK) return s;
+            for (int i = 0; i <= n; ++i) { launch_finalize_norm(ctx->partials, 2 * dgrid, ctx->sc, 1, st); s = after_launch(ctx); if (s != DDAMG_OK) return s; }
+            return copy_hist(ctx, res_hist, n + 1, nullptr);
         }
-        s = residual(false); if (s != DDAMG_OK) return s;            // line 7
-        s = blocks(1, ctx->tmp_e, ctx->tmp_o); if (s != DDAMG_OK) return s;       // lines 8-10: black blocks
+        return DDAMG_OK;
+    }
+    // Alg. 1 line 2, first iteration: r = b - D x, evaluated in full once (x = 0: r = b itself, read in place --
+    // the smoother use); afterwards every block solve and boundary pass keeps r current
+    const void* rin_e = b_e;
+    const void* rin_o = b_o;
+    if (!zero_init) {
+        s = dslash(ctx, EPI_FULL_RESIDUAL, hist, 0, x_o, x_e, b_e, r_e, 0.0, 5);
+        if (s != DDAMG_OK) return s;
+        s = dslash(ctx, EPI_FULL_RESIDUAL, hist, 1, x_e, x_o, b_o, r_o, 0.0, 5, 0, (size_t)dgrid, ctx->clov_oo);
+        if (s != DDAMG_OK) return s;
+        if (hist) { launch_finalize_norm(ctx->partials, 2 * dgrid, ctx->sc, 1, st); s = after_launch(ctx); if (s != DDAMG_OK) return s; }
+        rin_e = r_e; rin_o = r_o;
+    } else if (hist) {
+        // ||b||: reduce b without touching it
+        const int n1 = f32 ? launch_copy_norm<float>(ctx->nreal, b_e, r_e, ctx->partials, st) : launch_copy_norm<double>(ctx->nreal, b_e, r_e, ctx->partials, st);
+        const int n2 = f32 ? launch_copy_norm<float>(ctx->nreal, b_o, r_o, ctx->partials + n1, st) : launch_copy_norm<double>(ctx->nreal, b_o, r_o, ctx->partials + n1, st);
+        launch_finalize_norm(ctx->partials, n1 + n2, ctx->sc, 1, st);
+        s = after_launch(ctx, 3); if (s != DDAMG_OK) return s;
+        rin_e = r_e; rin_o = r_o;
+    }
+    for (int i = 0; i < n; ++i) {
+        if (i > 0 && hist) { s = append_norm(); if (s != DDAMG_OK) return s; }       // line 2: ||r|| before iteration i
+        s = half_iteration(0, rin_e, rin_o, true);                                     // red blocks, then r on the black sites
+        if (s != DDAMG_OK) return s;
+        rin_e = r_e; rin_o = r_o;
+        s = half_iteration(1, r_e, r_o, i + 1 < n || hist);                            // black blocks, then r on the red sites
+        if (s != DDAMG_OK) return s;
     }
     if (hist) {
-        s = residual(true); if (s != DDAMG_OK) return s;             // final true residual
+        s = append_norm(); if (s != DDAMG_OK) return s;                                // final residual
         return copy_hist(ctx, res_hist, n + 1, nullptr);
     }
     return DDAMG_OK;

@@ -20,6 +20,15 @@
 // clover blocks are re-read through L1/L2 (73 KB per 4^4 block: L2-resident).  All dot
 // products are block-local: one CTA-wide fp64 reduction per MR iteration, no
 // global reduction, no host involvement.
+//
+// The residual is kept up to date INCREMENTALLY (what DD-alphaAMG itself does; R24): after its
+// solve the block kernel also writes e_k and the new residual of its own sites -- (rho, 0): the odd rows of
+// D_k e_k = r_k hold exactly, the even rows are left with the last Minimal Residual residual -- and
+// sap_boundary_kernel subtracts H e from the sites of the OTHER colour that touch a solved block (the hops
+// that cross a block face, on average 2 of 8 per site for 4^4 blocks).  Alg. 1's lines 2 and 7 thus cost one
+// partial hopping pass instead of two full operator applications per colour.
+// RECON = 12: the block's links are staged as two rows (48 instead of 72 bytes per link in fp32; third row
+// rebuilt on use), which brings a 4^4 fp32 block to 74 KB of shared memory: 3 CTAs per SM instead of 2.
 #include "ddamg_internal.h"
 #include "ddamg_hop.cuh"
 
@@ -31,10 +40,14 @@ struct SapArgs {
     SapGeom sg;
     int colour;              // colour of the blocks this launch solves (0 = red)
     int m;                   // Minimal Residual iterations (>= 1)
-    const T* blk_links;      // block-ordered links:  [block][parity][mu][18 * n]   (sap_reorder_kernel)
+    const T* blk_links;      // block-ordered links:  [block][parity][mu][RECON * n]   (sap_reorder_kernel)
     const T* blk_clov;       // block-ordered A_ee / A_oo^-1 blocks:  [block][parity][72 * n]
-    const T* r_e;            // global residual r = b - D x
+    const T* r_e;            // global residual r = b - D x (read on the blocks of this colour)
     const T* r_o;
+    T* rn_e;                 // residual after the update, written on the blocks of this colour: (rho, 0)
+    T* rn_o;
+    T* e_e;                  // the update e_k, written on the blocks of this colour (read by sap_boundary_kernel)
+    T* e_o;
     T* x_e;                  // iterate, updated in place on the blocks of this colour
     T* x_o;
 };
@@ -72,6 +85,22 @@ __device__ __forceinline__ void lds_link(const double* blk, int n, int i, double
 #pragma unroll
     for (int k = 0; k < 9; ++k) unpack(p[k * n], &u[2 * k]);
 }
+// two-row links in shared memory (RECON = 12): rows 0, 1 as 3 float4 / 6 double2 planes, third row rebuilt.
+// No boundary sign: a hop inside a block never uses the wrap-around link of the time boundary.
+__device__ __forceinline__ void lds_link12(const float* blk, int n, int i, float (&u)[18])
+{
+    const float4* p4 = reinterpret_cast<const float4*>(blk) + i;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) unpack(p4[k * n], &u[4 * k]);
+    reconstruct_row2<float>(1.f, u);
+}
+__device__ __forceinline__ void lds_link12(const double* blk, int n, int i, double (&u)[18])
+{
+    const double2* p = reinterpret_cast<const double2*>(blk) + i;
+#pragma unroll
+    for (int k = 0; k < 6; ++k) unpack(p[k * n], &u[2 * k]);
+    reconstruct_row2<double>(1.0, u);
+}
 __device__ __forceinline__ void sts_link(float* blk, int n, int i, const float (&u)[18])
 {
     float4* p4 = reinterpret_cast<float4*>(blk) + i;
@@ -108,12 +137,12 @@ __device__ __forceinline__ LSite lsite_of(const SapGeom& sg, int lcb, int parity
 // acc = sum over the neighbours INSIDE the block (without the -1/2): the hopping term of
 // D_k = P_k D P_k^T.  in: opposite-parity half-block spinor, links_own / links_opp: the block's
 // forward links of this site's / the other parity, all in shared memory.
-template <typename T>
+template <typename T, int RECON>
 __device__ __forceinline__ void hop_block(const SapGeom& sg, int lcb, const LSite& s, const T* in,
                                           const T* links_own, const T* links_opp, T (&acc)[24])
 {
     const int n = sg.Vbh;
-    const int lblk = 18 * n;
+    const int lblk = RECON * n;
 #pragma unroll
     for (int i = 0; i < 24; ++i) acc[i] = 0;
     T psi[24], u[18];
@@ -121,12 +150,14 @@ __device__ __forceinline__ void hop_block(const SapGeom& sg, int lcb, const LSit
 #define DDAMG_BHOP(MU, IN_F, NB_F, IN_B, NB_B)                               \
     if (IN_F) {                                                              \
         lds_spinor<T>(in, n, (NB_F), psi);                                   \
-        lds_link(links_own + MU * lblk, n, lcb, u);                          \
+        if (RECON == 12) lds_link12(links_own + MU * lblk, n, lcb, u);       \
+        else lds_link(links_own + MU * lblk, n, lcb, u);                     \
         hop_dir<MU, true>(psi, u, acc);                                      \
     }                                                                        \
     if (IN_B) {                                                              \
         lds_spinor<T>(in, n, (NB_B), psi);                                   \
-        lds_link(links_opp + MU * lblk, n, (NB_B), u);                       \
+        if (RECON == 12) lds_link12(links_opp + MU * lblk, n, (NB_B), u);    \
+        else lds_link(links_opp + MU * lblk, n, (NB_B), u);                  \
         hop_dir<MU, false>(psi, u, acc);                                     \
     }
     DDAMG_BHOP(0, s.lx + 1 < sg.B[0], lcb + s.q, s.lx > 0, lcb + s.q - 1)
@@ -136,14 +167,27 @@ __device__ __forceinline__ void hop_block(const SapGeom& sg, int lcb, const LSit
 #undef DDAMG_BHOP
 }
 
-template <typename T>
-__global__ void __launch_bounds__(SAP_MAX_THREADS, 1) sap_block_kernel(const SapArgs<T> a)
+// MAXT = 128: blocks of up to 256 sites (the 4^4 default), two (18-real links) or three (two-row links, fp32)
+// CTAs per SM; MAXT = 256: blocks of up to 512 sites.  B4: the block is 4^4 (Table 6's aggregate size, the
+// default): every extent, stride and shared-memory plane offset is a compile-time constant, which removes the
+// address arithmetic of the ~90 shared-memory and ~20 global accesses of a half step.
+#ifndef DDAMG_SAP_B4_SPECIALISE
+#define DDAMG_SAP_B4_SPECIALISE 1
+#endif
+template <typename T, int RECON, int MAXT, bool B4>
+__global__ void __launch_bounds__(MAXT, MAXT == 128 ? (RECON == 12 && sizeof(T) == 4 ? 3 : 2) : 1)
+sap_block_kernel(const SapArgs<T> a)
 {
     extern __shared__ __align__(16) unsigned char sap_smem[];
-    const SapGeom& sg = a.sg;
+    SapGeom sg = a.sg;
+    if (B4) {                                                  // constants the compiler propagates
+        sg.B[0] = sg.B[1] = sg.B[2] = sg.B[3] = 4;
+        sg.Bxh = 2;
+        sg.Vbh = 128;
+    }
     const int n = sg.Vbh;
-    T* links = reinterpret_cast<T*>(sap_smem);                 // [parity][mu][18 * n]
-    T* S_e = links + 2 * 4 * 18 * n;                           // even-site half-block spinor
+    T* links = reinterpret_cast<T*>(sap_smem);                 // [parity][mu][RECON * n]
+    T* S_e = links + 2 * 4 * RECON * n;                        // even-site half-block spinor
     T* S_o = S_e + 24 * n;                                     // odd-site half-block spinor
     double* red = reinterpret_cast<double*>(S_o + 24 * n);     // [warp][3]
     const int tid = threadIdx.x;
@@ -172,7 +216,7 @@ __global__ void __launch_bounds__(SAP_MAX_THREADS, 1) sap_block_kernel(const Sap
             cbg[p] = ((ox + ls[p].lx) >> 1) + a.g.Lh * ((oy + ls[p].ly) + a.g.L * ((oz + ls[p].lz) + a.g.L * (ot + ls[p].lt)));
         }
     }
-    const int sblk = 4 * 18 * n;                               // one parity's four link blocks in shared memory
+    const int sblk = 4 * RECON * n;                            // one parity's four link blocks in shared memory
     {
         // ---- stage the block's links (read once from HBM per launch): the block-ordered copy has
         // the shared-memory layout, so this is one contiguous, fully coalesced 16-byte-vector copy
@@ -203,7 +247,7 @@ __global__ void __launch_bounds__(SAP_MAX_THREADS, 1) sap_block_kernel(const Sap
         const int par = hs & 1;
         T acc[24];
         if (active)
-            hop_block<T>(sg, tid, ls[par], par ? S_e : S_o, links + par * sblk, links + (1 - par) * sblk, acc);
+            hop_block<T, RECON>(sg, tid, ls[par], par ? S_e : S_o, links + par * sblk, links + (1 - par) * sblk, acc);
         if (par) {
             if (active) {
                 T v[24], t[24];
@@ -225,6 +269,13 @@ __global__ void __launch_bounds__(SAP_MAX_THREADS, 1) sap_block_kernel(const Sap
 #pragma unroll
                     for (int i = 0; i < 24; ++i) v[i] += e[i];
                     store_spinor<T>(a.x_e, a.g.Vh, cbg[0], v);
+                    // the update and the residual it leaves on this block: r_k - D_k e_k = (rho, 0)
+                    store_spinor<T>(a.e_o, a.g.Vh, cbg[1], t);
+                    store_spinor<T>(a.e_e, a.g.Vh, cbg[0], e);
+                    store_spinor<T>(a.rn_e, a.g.Vh, cbg[0], rho);
+#pragma unroll
+                    for (int i = 0; i < 24; ++i) v[i] = 0;
+                    store_spinor<T>(a.rn_o, a.g.Vh, cbg[1], v);
                 } else {
                     sts_spinor<T>(S_o, n, tid, t);
                 }
@@ -245,14 +296,17 @@ __global__ void __launch_bounds__(SAP_MAX_THREADS, 1) sap_block_kernel(const Sap
                 clover_site_mul<T, false>(clov_e, n, tid, rho, q);
 #pragma unroll
                 for (int i = 0; i < 24; ++i) q[i] = q[i] + (T)0.5 * acc[i];
-                // <q, rho> = q^H rho and <q, q>, this site's share
+                // <q, rho> = q^H rho and <q, q>, this site's share: the 12 complex products of the site in the
+                // data precision, the sums over the block's sites in fp64
+                T snr = 0, sni = 0, sdd = 0;
 #pragma unroll
                 for (int c = 0; c < 12; ++c) {
-                    const double qr = q[2 * c], qi = q[2 * c + 1], pr = rho[2 * c], pi = rho[2 * c + 1];
-                    nr += qr * pr + qi * pi;
-                    ni += qr * pi - qi * pr;
-                    dd += qr * qr + qi * qi;
+                    const T qr = q[2 * c], qi = q[2 * c + 1], pr = rho[2 * c], pi = rho[2 * c + 1];
+                    snr = vfma(qr, pr, snr); snr = vfma(qi, pi, snr);
+                    sni = vfma(qr, pi, sni); sni = vfma(-qi, pr, sni);
+                    sdd = vfma(qr, qr, sdd); sdd = vfma(qi, qi, sdd);
                 }
+                nr = snr; ni = sni; dd = sdd;
             }
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) {
@@ -289,7 +343,7 @@ __global__ void __launch_bounds__(SAP_MAX_THREADS, 1) sap_block_kernel(const Sap
 // r1c_ncu_full_sap.md).  Here every block's links and clover blocks are stored contiguously in
 // the block's own SoA order (plane-major, n = V_b/2 sites per plane), block id = cx + nbx (cy +
 // nby (cz + nbz ct)) over the blocks of BOTH colours.
-template <typename T>
+template <typename T, int RECON>
 __global__ void sap_reorder_kernel(Geom g, SapGeom sg, const T* __restrict__ gauge, const T* __restrict__ clov_e,
                                    const T* __restrict__ clov_oinv, T* __restrict__ blk_links, T* __restrict__ blk_clov)
 {
@@ -311,7 +365,8 @@ __global__ void sap_reorder_kernel(Geom g, SapGeom sg, const T* __restrict__ gau
         for (int mu = 0; mu < 4; ++mu) {
             T u[18];
             load_link(gauge + (size_t)(p * 4 + mu) * gblk, g.Vh, cbg, u);
-            store_link(blk_links + (bid * 8 + p * 4 + mu) * 18 * n, n, i, u);
+            if (RECON == 12) store_link12(blk_links + (bid * 8 + p * 4 + mu) * 12 * n, n, i, u);
+            else store_link(blk_links + (bid * 8 + p * 4 + mu) * 18 * n, n, i, u);
         }
         const T* src = p ? clov_oinv : clov_e;
 #pragma unroll 1
@@ -324,42 +379,135 @@ __global__ void sap_reorder_kernel(Geom g, SapGeom sg, const T* __restrict__ gau
 }
 
 template <typename T>
-void launch_sap_reorder(const Geom& g, const SapGeom& sg, const void* gauge, const void* clov_e, const void* clov_oinv,
-                        void* blk_links, void* blk_clov, cudaStream_t st)
+void launch_sap_reorder(const Geom& g, const SapGeom& sg, int recon, const void* gauge, const void* clov_e,
+                        const void* clov_oinv, void* blk_links, void* blk_clov, cudaStream_t st)
 {
     const int threads = (sg.Vbh + 31) / 32 * 32;
     const int grid = sg.nb[0] * sg.nb[1] * sg.nb[2] * sg.nb[3];
-    sap_reorder_kernel<T><<<grid, threads, 0, st>>>(g, sg, (const T*)gauge, (const T*)clov_e, (const T*)clov_oinv,
-                                                    (T*)blk_links, (T*)blk_clov);
+    if (recon == 12)
+        sap_reorder_kernel<T, 12><<<grid, threads, 0, st>>>(g, sg, (const T*)gauge, (const T*)clov_e, (const T*)clov_oinv,
+                                                            (T*)blk_links, (T*)blk_clov);
+    else
+        sap_reorder_kernel<T, 18><<<grid, threads, 0, st>>>(g, sg, (const T*)gauge, (const T*)clov_e, (const T*)clov_oinv,
+                                                            (T*)blk_links, (T*)blk_clov);
 }
-template void launch_sap_reorder<float>(const Geom&, const SapGeom&, const void*, const void*, const void*, void*, void*, cudaStream_t);
-template void launch_sap_reorder<double>(const Geom&, const SapGeom&, const void*, const void*, const void*, void*, void*, cudaStream_t);
+template void launch_sap_reorder<float>(const Geom&, const SapGeom&, int, const void*, const void*, const void*, void*, void*, cudaStream_t);
+template void launch_sap_reorder<double>(const Geom&, const SapGeom&, int, const void*, const void*, const void*, void*, void*, cudaStream_t);
 
-size_t sap_smem_bytes(const SapGeom& sg, size_t real_bytes)
+size_t sap_smem_bytes(const SapGeom& sg, size_t real_bytes, int recon)
 {
-    return (size_t)(2 * 4 * 18 + 48) * sg.Vbh * real_bytes + (size_t)32 * 3 * sizeof(double);
+    return (size_t)(2 * 4 * recon + 48) * sg.Vbh * real_bytes + (size_t)32 * 3 * sizeof(double);
+}
+
+template <typename T, int RECON, int MAXT, bool B4>
+static cudaError_t launch_blocks_as(const SapArgs<T>& a, int threads, int grid, size_t smem, cudaStream_t st)
+{
+    cudaError_t e = cudaFuncSetAttribute(sap_block_kernel<T, RECON, MAXT, B4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    sap_block_kernel<T, RECON, MAXT, B4><<<grid, threads, smem, st>>>(a);
+    return cudaSuccess;
 }
 
 template <typename T>
-cudaError_t launch_sap_blocks(const Geom& g, const SapGeom& sg, int colour, int m, const void* blk_links,
-                              const void* blk_clov, const void* r_e, const void* r_o,
-                              void* x_e, void* x_o, cudaStream_t st)
+cudaError_t launch_sap_blocks(const Geom& g, const SapGeom& sg, int recon, int colour, int m, const void* blk_links,
+                              const void* blk_clov, const void* r_e, const void* r_o, void* rn_e, void* rn_o,
+                              void* e_e, void* e_o, void* x_e, void* x_o, cudaStream_t st)
 {
     SapArgs<T> a;
     a.g = g; a.sg = sg; a.colour = colour; a.m = m;
     a.blk_links = (const T*)blk_links; a.blk_clov = (const T*)blk_clov;
-    a.r_e = (const T*)r_e; a.r_o = (const T*)r_o; a.x_e = (T*)x_e; a.x_o = (T*)x_o;
-    const size_t smem = sap_smem_bytes(sg, sizeof(T));
-    cudaError_t e = cudaFuncSetAttribute(sap_block_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
+    a.r_e = (const T*)r_e; a.r_o = (const T*)r_o; a.rn_e = (T*)rn_e; a.rn_o = (T*)rn_o;
+    a.e_e = (T*)e_e; a.e_o = (T*)e_o; a.x_e = (T*)x_e; a.x_o = (T*)x_o;
+    const size_t smem = sap_smem_bytes(sg, sizeof(T), recon);
     const int threads = (sg.Vbh + 31) / 32 * 32;
     const int grid = sg.nbxh * sg.nb[1] * sg.nb[2] * sg.nb[3];
-    sap_block_kernel<T><<<grid, threads, smem, st>>>(a);
-    return cudaSuccess;
+    const bool b4 = DDAMG_SAP_B4_SPECIALISE && sg.B[0] == 4 && sg.B[1] == 4 && sg.B[2] == 4 && sg.B[3] == 4;
+    if (b4)
+        return recon == 12 ? launch_blocks_as<T, 12, 128, true>(a, threads, grid, smem, st)
+                           : launch_blocks_as<T, 18, 128, true>(a, threads, grid, smem, st);
+    if (threads <= 128)
+        return recon == 12 ? launch_blocks_as<T, 12, 128, false>(a, threads, grid, smem, st)
+                           : launch_blocks_as<T, 18, 128, false>(a, threads, grid, smem, st);
+    return recon == 12 ? launch_blocks_as<T, 12, SAP_MAX_THREADS, false>(a, threads, grid, smem, st)
+                       : launch_blocks_as<T, 18, SAP_MAX_THREADS, false>(a, threads, grid, smem, st);
 }
-template cudaError_t launch_sap_blocks<float>(const Geom&, const SapGeom&, int, int, const void*, const void*,
-                                              const void*, const void*, void*, void*, cudaStream_t);
-template cudaError_t launch_sap_blocks<double>(const Geom&, const SapGeom&, int, int, const void*, const void*,
-                                               const void*, const void*, void*, void*, cudaStream_t);
+template cudaError_t launch_sap_blocks<float>(const Geom&, const SapGeom&, int, int, int, const void*, const void*,
+                                              const void*, const void*, void*, void*, void*, void*, void*, void*, cudaStream_t);
+template cudaError_t launch_sap_blocks<double>(const Geom&, const SapGeom&, int, int, int, const void*, const void*,
+                                               const void*, const void*, void*, void*, void*, void*, void*, void*, cudaStream_t);
+
+// ---- incremental residual (Alg. 1 lines 2 / 7 after the first evaluation): for every site of colour `target`
+//   rn(x) = r(x) - sum over the neighbours y of x in OTHER blocks of H_xy e(y)
+// Every block across a face has the other colour, i.e. was just solved and carries its update in e; hops inside
+// the site's own block see no update (e is stale there and must not be read).  One thread per lattice site; the
+// lanes of the other colour idle, which costs issue slots but no memory traffic (32-byte sectors: the 2-site
+// x-runs of a 4-wide block are exactly one sector per plane).
+template <typename T, int RECON>
+__global__ void __launch_bounds__(DSLASH_THREADS)
+sap_boundary_kernel(Geom g, SapGeom sg, int target, int apbc, const T* __restrict__ gauge, const T* __restrict__ e_e,
+                    const T* __restrict__ e_o, const T* r_e, const T* r_o, T* rn_e, T* rn_o)
+{
+    const int idx = blockIdx.x * DSLASH_THREADS + threadIdx.x;
+    if (idx >= 2 * g.Vh) return;
+    const int parity = idx >= g.Vh ? 1 : 0, cb = idx - parity * g.Vh;
+    const Site s = site_of_cb(g, cb, parity);
+    const int x = 2 * s.xh + s.q;
+    const int bx = x / sg.B[0], by = s.y / sg.B[1], bz = s.z / sg.B[2], bt = s.t / sg.B[3];
+    if (((bx + by + bz + bt) & 1) != target) return;
+    const int lx = x - bx * sg.B[0], ly = s.y - by * sg.B[1], lz = s.z - bz * sg.B[2], lt = s.t - bt * sg.B[3];
+    const T* in = parity ? e_e : e_o;                          // neighbours have the opposite parity
+    const size_t lblk = (size_t)RECON * g.Vh;
+    const T* gauge_own = gauge + (size_t)parity * 4 * lblk;
+    const T* gauge_opp = gauge + (size_t)(1 - parity) * 4 * lblk;
+    const T sgn_f3 = (apbc && s.t == g.T - 1) ? (T)-1 : (T)1;
+    const T sgn_b3 = (apbc && s.t == 0) ? (T)-1 : (T)1;
+    T acc[24], psi[24], u[18];
+#pragma unroll
+    for (int i = 0; i < 24; ++i) acc[i] = 0;
+#define DDAMG_XHOP(MU, OUT_F, OUT_B)                                                           \
+    if (OUT_F) {                                                                               \
+        load_spinor<T>(in, g.Vh, neighbour_cb<MU, +1>(g, cb, s), psi);                         \
+        if (RECON == 12) load_link12(gauge_own + MU * lblk, g.Vh, cb, MU == 3 ? sgn_f3 : (T)1, u); \
+        else load_link(gauge_own + MU * lblk, g.Vh, cb, u);                                    \
+        hop_dir<MU, true>(psi, u, acc);                                                        \
+    }                                                                                          \
+    if (OUT_B) {                                                                               \
+        const int nb = neighbour_cb<MU, -1>(g, cb, s);                                         \
+        load_spinor<T>(in, g.Vh, nb, psi);                                                     \
+        if (RECON == 12) load_link12(gauge_opp + MU * lblk, g.Vh, nb, MU == 3 ? sgn_b3 : (T)1, u); \
+        else load_link(gauge_opp + MU * lblk, g.Vh, nb, u);                                    \
+        hop_dir<MU, false>(psi, u, acc);                                                       \
+    }
+    DDAMG_XHOP(0, lx == sg.B[0] - 1, lx == 0)
+    DDAMG_XHOP(1, ly == sg.B[1] - 1, ly == 0)
+    DDAMG_XHOP(2, lz == sg.B[2] - 1, lz == 0)
+    DDAMG_XHOP(3, lt == sg.B[3] - 1, lt == 0)
+#undef DDAMG_XHOP
+    const T* r = parity ? r_o : r_e;
+    T* rn = parity ? rn_o : rn_e;
+    T v[24];
+    load_spinor<T, true>(r, g.Vh, cb, v);
+#pragma unroll
+    for (int i = 0; i < 24; ++i) v[i] = vfma((T)0.5, acc[i], v[i]);          // r - H e,  H = -1/2 acc
+    store_spinor<T>(rn, g.Vh, cb, v);
+}
+
+template <typename T>
+void launch_sap_boundary(const Geom& g, const SapGeom& sg, int recon, int target, int apbc, const void* gauge,
+                         const void* e_e, const void* e_o, const void* r_e, const void* r_o, void* rn_e, void* rn_o,
+                         cudaStream_t st)
+{
+    const int grid = (2 * g.Vh + DSLASH_THREADS - 1) / DSLASH_THREADS;
+    if (recon == 12)
+        sap_boundary_kernel<T, 12><<<grid, DSLASH_THREADS, 0, st>>>(g, sg, target, apbc, (const T*)gauge, (const T*)e_e,
+                                                                    (const T*)e_o, (const T*)r_e, (const T*)r_o, (T*)rn_e, (T*)rn_o);
+    else
+        sap_boundary_kernel<T, 18><<<grid, DSLASH_THREADS, 0, st>>>(g, sg, target, apbc, (const T*)gauge, (const T*)e_e,
+                                                                    (const T*)e_o, (const T*)r_e, (const T*)r_o, (T*)rn_e, (T*)rn_o);
+}
+template void launch_sap_boundary<float>(const Geom&, const SapGeom&, int, int, int, const void*, const void*, const void*,
+                                         const void*, const void*, void*, void*, cudaStream_t);
+template void launch_sap_boundary<double>(const Geom&, const SapGeom&, int, int, int, const void*, const void*, const void*,
+                                          const void*, const void*, void*, void*, cudaStream_t);
 
 }  // namespace ddamg
