@@ -128,8 +128,10 @@ int ddamg_richardson(ddamg_ctx* ctx, const void* b_e, void* x_e, int nu, double 
  *              ||b_e - D_S x|| at its start followed by the k residual estimates, then the
  *              true residual norm at the end.  *n_hist (may be NULL) = entries written.
  * Orthogonalisation: classical Gram-Schmidt in two fused passes (one multi-dot, one
- * multi-axpy + norm), partial sums in fp64 (reading R15).  The basis is kept lazily
- * normalised (vector + device scalar, reading R15b): no separate normalisation pass.
+ * multi-axpy + norm), partial sums in fp64 (reading R15); for k > 12 or tol > 0 the two
+ * passes are repeated once (CGS2) so that the Givens residual estimates stay reliable in fp32.
+ * The basis is kept lazily normalised (vector + device scalar, reading R15b): no separate
+ * normalisation pass.
  * EINVAL if k < 1, cycles < 1 or b_e aliases x_e.  ENOMEM if the Krylov basis
  * ((k+1) half spinors) cannot be allocated.
  */

@@ -689,6 +689,8 @@ static int gmres_impl(ddamg_ctx* ctx, const void* b_e, void* x_e, int k, int cyc
     double* coef_ys = (double*)((char*)ctx->sc + offsetof(Scalars, ys));
     double* coef_negh = (double*)((char*)ctx->sc + offsetof(Scalars, negh));
     double* vs = (double*)((char*)ctx->sc + offsetof(Scalars, vs));
+    // a second Gram-Schmidt pass (CGS2) where a long cycle or a tolerance exit relies on the Givens estimates
+    const bool cgs2 = k > MDOT_NB || tol > 0.0;
     int s = reset_hist(ctx);
     if (s != DDAMG_OK) return s;
     double bnorm = 0.0;
@@ -744,6 +746,22 @@ static int gmres_impl(ddamg_ctx* ctx, const void* b_e, void* x_e, int k, int cyc
                                                 i0 == 0 ? vs + j : nullptr);
                 }
                 s = after_launch(ctx); if (s != DDAMG_OK) return s;
+            }
+            if (cgs2) {
+                // second pass: one classical Gram-Schmidt pass loses orthogonality like eps * cond(basis)^2, which in
+                // fp32 shows in the Givens estimates of long cycles; the correction h' = <v_i, w> is added to h_ij
+                for (int i0 = 0; i0 <= j; i0 += MDOT_NB) {
+                    const int nb = (j + 1 - i0) < MDOT_NB ? (j + 1 - i0) : MDOT_NB;
+                    { KernelTimer kt(ctx, KT_MDOT); nblk = launch_multi_dot<T>(nreal, nb, Vj(i0), nreal, Vj(j + 1), ctx->partials, st); }
+                    launch_finalize_dots_lazy2(ctx->partials, nblk, nb, ctx->sc, i0, st);
+                    s = after_launch(ctx, 2); if (s != DDAMG_OK) return s;
+                }
+                for (int i0 = 0; i0 <= j; i0 += MDOT_NB) {
+                    const int nb = (j + 1 - i0) < MDOT_NB ? (j + 1 - i0) : MDOT_NB;
+                    const bool last = i0 + MDOT_NB > j;
+                    { KernelTimer kt(ctx, KT_MAXPY); nblk = launch_multi_axpy<T>(nreal, nb, Vj(i0), nreal, coef_negh + 2 * i0, Vj(j + 1), last ? ctx->partials : nullptr, st); }
+                    s = after_launch(ctx); if (s != DDAMG_OK) return s;
+                }
             }
             launch_finalize_norm(ctx->partials, nblk, ctx->sc, 0, st);
             launch_gmres_givens(ctx->sc, j, st);                         // also vs[j+1] = 1 / h_{j+1,j}

@@ -330,6 +330,28 @@ void launch_finalize_dots_lazy(const double* partials, int nblocks, int nb, Scal
     finalize_dots_lazy_kernel<<<1, 32 * 2 * MDOT_NB, 0, st>>>(partials, nblocks, nb, sc, first, j);
 }
 
+// Second Gram-Schmidt pass (CGS2): the raw sums are <stored_i, w> with w already orthogonalised once and in true
+// units, so the correction is  h'_i = vs[i] sum;  h_ij += h'_i;  coefficient of stored_i:  -h'_i vs[i].
+__global__ void finalize_dots_lazy2_kernel(const double* __restrict__ partials, int nblocks, int nb, Scalars* sc, int first)
+{
+    const int c = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (c < 2 * nb) {
+        double s = 0;
+        for (int b = lane; b < nblocks; b += 32) s += partials[(size_t)b * 2 * nb + c];
+        s = warp_sum(s);
+        if (lane == 0) {
+            const double si = sc->vs[first + (c >> 1)];
+            const double h = s * si;
+            sc->hcol[2 * first + c] += h;
+            sc->negh[2 * first + c] = -h * si;
+        }
+    }
+}
+void launch_finalize_dots_lazy2(const double* partials, int nblocks, int nb, Scalars* sc, int first, cudaStream_t st)
+{
+    finalize_dots_lazy2_kernel<<<1, 32 * 2 * MDOT_NB, 0, st>>>(partials, nblocks, nb, sc, first);
+}
+
 // ------------------------------------------------------------------ w <- ws w + sum_i coef_i v_i  (+ |w|^2)
 template <typename T, int NB>
 __global__ void __launch_bounds__(BLAS_THREADS)

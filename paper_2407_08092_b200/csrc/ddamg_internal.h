@@ -134,6 +134,7 @@ int launch_multi_dot(size_t nreal, int nb, const void* V, size_t vstride_real, c
                       cudaStream_t st);
 void launch_finalize_dots(const double* partials, int nblocks, int nb, Scalars* sc, int first, cudaStream_t st);
 void launch_finalize_dots_lazy(const double* partials, int nblocks, int nb, Scalars* sc, int first, int j, cudaStream_t st);
+void launch_finalize_dots_lazy2(const double* partials, int nblocks, int nb, Scalars* sc, int first, cudaStream_t st);   // CGS2 correction
 // w <- (*wscale) w + sum_i coef[i] v_i (complex coef and real wscale on device, nb <= MDOT_NB;
 // wscale NULL = 1); optional |w|^2 partials
 template <typename T>

@@ -299,7 +299,8 @@ def _check_history(got, ref, bnorm, f64):
     (4, "f32", 10, 2, 8, 8),          # config 4 recipe GMRES(2,10) on a small lattice
     (4, "f64", 10, 2, 8, 8),
     (4, "f32", 10, 2, 16, 32),        # config 4 recipe GMRES(2,10), T = 2L shape, 65,536 even sites (512 CTAs)
-    (2, "f32", 14, 1, None, None),    # k > 12: more than one fused multi-dot chunk
+    (2, "f32", 14, 1, None, None),    # k > 12: more than one fused multi-dot chunk, second Gram-Schmidt pass (CGS2)
+    (3, "f32", 40, 1, 8, 8),          # a long fp32 cycle: four chunks, CGS2 keeps the Givens estimates on the oracle's
 ])
 def test_gmres_matches_oracle(cfg, prec, k, cycles, L, T):
     oracle, _ = _mods()
