@@ -22,7 +22,7 @@ cpu_baseline = the fp64 oracle (oracle/, as it stands) timed on the host cores o
              apply and one Richardson sweep at 16^4 and 32^3 x 64, all cores and 1 thread, with the
              CPU model string
 --rows     = 'all' (default), 'main' (the step only) or a comma list of side rows:
-             links18,schur,smoother,gmres,sap,multi_rhs,paper,f64,cfg3,cfg4
+             links18,schur,smoother,gmres,gcr,sap,multi_rhs,paper,f64,cfg3,cfg4
 Multi-GPU: the path does not shard in this build ("replicas only"): --gpus N runs
 N independent replicas, one per rank, no data-path collective; scaling = "weak".
 """
@@ -56,7 +56,7 @@ FLOP_PER_SITE = 1824    # 1320 (hop) + 504 (2 x 6x6 Hermitian mat-vec), per latt
 # ncu --set full capture summarised in profiles/ (None until a capture exists)
 NCU_TRAFFIC_BYTES = {18: {5: 21.274e9}, 12: {5: 18.073e9}}     # profiles/r1b_ncu_full_dslash.md, profiles/r1d_ncu_full_dslash12.md
 NOMINAL_HBM_GBS = 8000.0    # north_star's "~8 TB/s HBM peak" (DGX figure; HGX 7.7 TB/s), quoted beside the measured copy peak
-SIDE_ROWS = ("links18", "schur", "smoother", "gmres", "sap", "multi_rhs", "paper", "f64", "cfg3", "cfg4")
+SIDE_ROWS = ("links18", "schur", "smoother", "gmres", "gcr", "sap", "multi_rhs", "paper", "f64", "cfg3", "cfg4")
 CPU_SAMPLE = dict(L=16, T=32)
 # SAP(n, m) row: the paper's smoother parameters (Tables 1, 2, 6) on 4^4 blocks
 SAP_N, SAP_M, SAP_BLOCK = 3, 4, (4, 4, 4, 4)
@@ -610,6 +610,22 @@ def main():
                         gmres_1x10_multi_axpy_frac_of_peak=rows["gmres_1x10"].get("multi_axpy_frac_of_peak"))
         except Exception as e:     # e.g. Krylov basis does not fit
             rows["gmres_1x10"] = {"error": str(e)}
+    if "gcr" in sel:
+        # ---- GCR(1, 10) (NEXT-4, Alg. 3): same operator applications as GMRES, fused form / update passes
+        try:
+            ctx.gcr_oe(pool_b[0][0], x_e, 10, 1, zero_init=True)           # warm-up (allocates the 2k + 1 vectors)
+            ctx.kernel_timing(True)
+            ctx.kernel_time_ms(0, reset=True)
+            ms = timed(lambda i: ctx.gcr_oe(pool_b[0][0], x_e, 10, 1, zero_init=True), 2, 0) / 2
+            tk = {w: ctx.kernel_time_ms(w, reset=False)[0] for w in (0, 1, 8, 10)}
+            ctx.kernel_time_ms(0, reset=True)
+            ctx.kernel_timing(False)
+            rows["gcr_1x10"] = {"ms": ms, "ms_per_step": ms / 10, "apply_ms_per_step": (tk[0] + tk[1]) / 20,
+                                "blas1_ms_per_step": (tk[8] + tk[10]) / 20,
+                                "note": "blas1 = multi-dot against the z_j + fused form pass (z, p, next delta) + update pass"}
+            flat["gcr_1x10_ms_per_step"] = ms / 10
+        except Exception as e:
+            rows["gcr_1x10"] = {"error": str(e)[:200]}
     if "sap" in sel:
         # ---- SAP(3,4) on 4^4 blocks (NEXT-3; the smoother of the paper's Tables 2 and 6)
         try:
