@@ -54,7 +54,7 @@ BYTES_BR = 1248         # kernel B': kernel B + b_e 96
 FLOP_PER_SITE = 1824    # 1320 (hop) + 504 (2 x 6x6 Hermitian mat-vec), per lattice site
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of kernel B' at config 5, from the
 # ncu --set full capture summarised in profiles/ (None until a capture exists)
-NCU_TRAFFIC_BYTES = {18: {5: 21.274e9}, 12: {5: 18.073e9}}     # profiles/r1b_ncu_full_dslash.md, profiles/r1d_ncu_full_dslash12.md
+NCU_TRAFFIC_BYTES = {18: {5: 21.274e9}, 12: {5: 18.038e9}}     # profiles/r1b_ncu_full_dslash.md, profiles/r2_ncu_full_dslash12.md
 NOMINAL_HBM_GBS = 8000.0    # north_star's "~8 TB/s HBM peak" (DGX figure; HGX 7.7 TB/s), quoted beside the measured copy peak
 SIDE_ROWS = ("links18", "schur", "smoother", "gmres", "gcr", "sap", "multi_rhs", "paper", "f64", "cfg3", "cfg4")
 CPU_SAMPLE = dict(L=16, T=32)
@@ -790,6 +790,37 @@ def main():
            "h2d_bytes_per_step": 2 * ctx.half_bytes, "d2h_bytes_per_step": ctx.half_bytes,
            "note": "through Ddamg.richardson with pinned HOST buffers; per step H2D of b_e and x0, the call, D2H of x^(nu); "
                    "copies of neighbouring steps overlap the compute (two copy streams, double-buffered inputs)"}
+
+    if "smoother" in sel and rank == 0 and world == 1:
+        # ---- what a caller with NATURAL-layout host fields pays for one whole smoother call (eq. 2): H2D of the
+        # full-lattice rhs b (T,L,L,L,4,3 complex64), pack, prepare_rhs, Richardson(nu=4) from x0 = 0,
+        # reconstruct_odd, unpack, D2H of the full-lattice x -- serial, one call after the other
+        try:
+            del hb, hx, hout
+            nat_shape = (T, L, L, L, 4, 3)
+            h_b = torch.empty(nat_shape, dtype=torch.complex64).pin_memory()
+            h_x = torch.empty(nat_shape, dtype=torch.complex64).pin_memory()
+            h_b.copy_(ctx.unpack(pool_b[0][0], pool_b[0][1]))
+            d_nat = torch.empty(nat_shape, dtype=torch.complex64, device=dev)
+            bhat, xo_ = ctx.half_spinor(), ctx.half_spinor()
+
+            def natural_call(i):
+                d_nat.copy_(h_b, non_blocking=True)
+                be_, bo_ = ctx.pack(d_nat)
+                ctx.prepare_rhs(be_, bo_, bhat)
+                ctx.richardson(bhat, x_e, NU, c["omega"], zero_init=True)
+                ctx.reconstruct_odd(bo_, x_e, xo_)
+                h_x.copy_(ctx.unpack(x_e, xo_), non_blocking=True)
+            kn = 3
+            ms = timed(natural_call, kn, 1) / kn
+            rows["e2e_smoother_call_natural_layout"] = {
+                "ms": ms, "h2d_bytes": h_b.numel() * 8, "d2h_bytes": h_x.numel() * 8,
+                "note": "host natural layout -> H2D -> pack -> eq.-2 smoother call (nu=4, x0=0) -> unpack -> D2H, serial; "
+                        "PCIe-bound: 3.2 GB in + 3.2 GB out"}
+            flat["e2e_smoother_call_natural_ms"] = ms
+            del h_b, h_x, d_nat, bhat, xo_
+        except Exception as exc:                  # noqa: BLE001
+            rows["e2e_smoother_call_natural_layout"] = {"error": str(exc)[:200]}
 
     line = {
         "metric": "Richardson sites/s (odd-even Schur Wilson-clover, nu=4)",
