@@ -123,6 +123,28 @@ __device__ __forceinline__ void store_spinor(float* __restrict__ base, int Vs, i
     for (int h = 0; h < 12; ++h) p[(size_t)h * Vs] = make_float4(s[2 * h].v.x, s[2 * h].v.y, s[2 * h + 1].v.x, s[2 * h + 1].v.y);
 }
 
+// L1 prefetch of the 16-byte vectors of one site's spinor (experiment, DDAMG_PF_L1)
+template <typename T, typename S>
+__device__ __forceinline__ void prefetch_spinor(const T* __restrict__ base, int Vs, int idx)
+{
+    using V = typename VecOf<T>::type;
+    constexpr int NPL = (sizeof(S) / sizeof(T)) * 24 / VecOf<T>::N;
+    const V* p = reinterpret_cast<const V*>(base) + idx;
+#pragma unroll
+    for (int k = 0; k < NPL; ++k) asm volatile("prefetch.global.L1 [%0];" ::"l"(p + (size_t)k * Vs));
+}
+
+// L1 prefetch of the two clover blocks of a site; the `units` threads of a site share the 72/N vectors
+template <typename T>
+__device__ __forceinline__ void prefetch_clover(const T* __restrict__ base, int Vh, int cb, int r, int units)
+{
+    using V = typename VecOf<T>::type;
+    constexpr int NPL = 72 / VecOf<T>::N;
+    const V* p = reinterpret_cast<const V*>(base) + cb;
+    if (units < 1) units = 1;
+    for (int k = r; k < NPL; k += units) asm volatile("prefetch.global.L1 [%0];" ::"l"(p + (size_t)k * Vh));
+}
+
 // 18 reals of one link; blk = start of the (parity, mu) block
 __device__ __forceinline__ void load_link(const float* __restrict__ blk, int Vh, int cb, float (&u)[18])
 {

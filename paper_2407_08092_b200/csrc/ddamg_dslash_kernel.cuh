@@ -96,7 +96,20 @@ dslash_kernel(const DslashArgs<T> a)
     if (cb < a.g.Vh) {
         const Site s = site_of_cb(a.g, cb, a.parity);
         S acc[24];
+#ifdef DDAMG_PF_EPI
+        // L1 prefetch of the epilogue operands before the last direction pair (experiment)
+        auto mid = [&]() {
+            if (BATCH || DDAMG_PF_EPI > 1) {
+                if (EPI == EPI_CLOV_RHS_MINUS_HOP || EPI == EPI_RHS_MINUS_HOP) prefetch_spinor<T, S>(a.rhs, Vs, sv);
+                if (EPI > EPI_RHS_MINUS_HOP) prefetch_spinor<T, S>(a.own, Vs, sv);
+                if (EPI == EPI_RICHARDSON || EPI == EPI_RESIDUAL || EPI == EPI_FULL_RESIDUAL) prefetch_spinor<T, S>(a.rhs, Vs, sv);
+                if (EPI != EPI_RHS_MINUS_HOP) prefetch_clover<T>(a.clov, a.g.Vh, cb, rr, units);
+            }
+        };
+        hop_site<T, RECON, S>(a.g, cb, s, a.in, units, rr, a.gauge_own, a.gauge_opp, acc, a.apbc, mid);
+#else
         hop_site<T, RECON, S>(a.g, cb, s, a.in, units, rr, a.gauge_own, a.gauge_opp, acc, a.apbc);
+#endif
         S res[24];
         if (EPI == EPI_CLOV_HOP) {
 #pragma unroll
