@@ -16,13 +16,14 @@ value      = V * nu * N / t   [site-sweeps/s], inputs resident in HBM, CUDA even
 e2e        = same metric through the public API with HOST (pinned) buffers: H2D of b_e and
              x^(0), the call, D2H of x^(nu) inside the timed region
 roofline   = dominant kernel (B': A_ee x - H_eo t + Richardson update), algorithmic bytes
-             1248 B/even site / CUDA-event duration, against MEASURED_PEAKS.json
+             1184 B/even site (18-real links; 992 B with two-row links) / CUDA-event duration,
+             against MEASURED_PEAKS.json
 cpu_baseline = the fp64 oracle (oracle/, as it stands) timed on the host cores on a bounded
              sample (16^3 x 32 lattice, same recipe: `value`), plus SURVEY.md 8(d)'s table: Schur
              apply and one Richardson sweep at 16^4 and 32^3 x 64, all cores and 1 thread, with the
              CPU model string
 --rows     = 'all' (default), 'main' (the step only) or a comma list of side rows:
-             links18,schur,smoother,gmres,gcr,sap,multi_rhs,paper,f64,cfg3,cfg4
+             links18,schur,smoother,gmres,gcr,sap,multi_rhs,paper,f64,cfg2,cfg3,cfg4
 Multi-GPU: the path does not shard in this build ("replicas only"): --gpus N runs
 N independent replicas, one per rank, no data-path collective; scaling = "weak".
 """
@@ -48,15 +49,16 @@ CONFIGS = {
 }
 NU = 4
 # algorithmic bytes per EVEN site, fp32, 18-real links
+CLOV_A = 224            # A_ee in the compact 28-real form (2 x 28 x 4 B; SURVEY.md's model has the packed 288 B)
 BYTES_A = 1056          # kernel A : 8 links 576 + x_e neighbours 96 + A_oo^-1 288 + write 96
-BYTES_B = 1152          # kernel B : 8 links 576 + t_o 96 + x_e 96 + A_ee 288 + write 96
-BYTES_BR = 1248         # kernel B': kernel B + b_e 96
+BYTES_B = 864 + CLOV_A  # kernel B : 8 links 576 + t_o 96 + x_e 96 + A_ee 224 + write 96  (= 1088; 1152)
+BYTES_BR = BYTES_B + 96 # kernel B': kernel B + b_e 96                                     (= 1184; 1248)
 FLOP_PER_SITE = 1824    # 1320 (hop) + 504 (2 x 6x6 Hermitian mat-vec), per lattice site
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of kernel B' at config 5, from the
 # ncu --set full capture summarised in profiles/ (None until a capture exists)
 NCU_TRAFFIC_BYTES = {18: {5: 21.274e9}, 12: {5: 18.038e9}}     # profiles/r1b_ncu_full_dslash.md, profiles/r2_ncu_full_dslash12.md
 NOMINAL_HBM_GBS = 8000.0    # north_star's "~8 TB/s HBM peak" (DGX figure; HGX 7.7 TB/s), quoted beside the measured copy peak
-SIDE_ROWS = ("links18", "schur", "smoother", "gmres", "gcr", "sap", "multi_rhs", "paper", "f64", "cfg3", "cfg4")
+SIDE_ROWS = ("links18", "schur", "smoother", "gmres", "gcr", "sap", "multi_rhs", "paper", "f64", "cfg2", "cfg3", "cfg4")
 CPU_SAMPLE = dict(L=16, T=32)
 # SAP(n, m) row: the paper's smoother parameters (Tables 1, 2, 6) on 4^4 blocks
 SAP_N, SAP_M, SAP_BLOCK = 3, 4, (4, 4, 4, 4)
@@ -252,7 +254,7 @@ def run_reference(args):
 # --------------------------------------------------------------------------- our arm
 def f64_apply_row(torch, gen, Ddamg, dev):
     """fp64 Schur apply at 48^3 x 96 (config 4 recipe, 18-real links): the precision of BASELINE.json's
-    fp64 parity bar, timed against the two-pass byte model at 8 bytes per real (4416 B per even site)."""
+    fp64 parity bar, timed against the two-pass byte model at 8 bytes per real (2 x (1056 + 1088) = 4288 B per even site)."""
     from paper_2407_08092_b200 import F64
     c = CONFIGS[4]
     L, T = c["L"], c["T"]
@@ -276,7 +278,7 @@ def f64_apply_row(torch, gen, Ddamg, dev):
     ms = a.elapsed_time(b) / n
     V = L * L * L * T
     peak, _ = _peaks()
-    gbs = 2 * 2208 * (V // 2) / (ms * 1e-3) / 1e9
+    gbs = 2 * (1056 + 864 + CLOV_A) * (V // 2) / (ms * 1e-3) / 1e9     # 18-real links, whatever --gauge-recon says
     ctx.close()
     return {"lattice": "48^3x96, fp64, 18-real links", "ms": ms, "sites_per_s": V / (ms * 1e-3),
             "GBps_two_pass_model": gbs, "frac_of_peak": gbs / peak,
@@ -564,7 +566,7 @@ def main():
         return out
 
     if "links18" in sel and args.gauge_recon == 12:
-        # ---- the same step on full 18-real links (two-pass model 1056 + 1248 B per even site)
+        # ---- the same step on full 18-real links (two-pass model 1056 + 1184 B per even site)
         ctx.set_option("gauge_recon", 18)
         ks = max(3, min(K, 10))
         ms18 = timed(step, ks, 3, prep_x) / ks
@@ -673,7 +675,7 @@ def main():
                 ctx.kernel_timing(False)
                 lk = 384 if args.gauge_recon == 12 else 576          # 8 links per output site
                 bA = 192 + (lk + 288) / nrhs     # per (site, rhs): x_e neighbours 96 + write 96 + (links + clover 288) / nrhs
-                bB = 384 + (lk + 288) / nrhs     # t_o 96 + x_e 96 + b_e 96 + write 96 + (links + 288) / nrhs
+                bB = 384 + (lk + CLOV_A) / nrhs  # t_o 96 + x_e 96 + b_e 96 + write 96 + (links + compact A_ee 224) / nrhs
                 tA3, tB4 = ms3 / max(n3, 1) * 1e-3, ms4 / max(n4, 1) * 1e-3
                 rate = V * NU * nrhs / (ms * 1e-3)
                 rows["multi_rhs_richardson"][str(nrhs)] = {
@@ -689,6 +691,40 @@ def main():
                 torch.cuda.empty_cache()
             except Exception as e:
                 rows["multi_rhs_richardson"][str(nrhs)] = {"error": str(e)}
+
+    if "cfg2" in sel and rank == 0 and world == 1:
+        # ---- BASELINE.json configs[1] (SURVEY.md 8(d) cfg 2): 16^4, 8 sweeps omega=1.0.  Gauge + clover = 38 MB << L2:
+        # an L2-resident, launch-bound timing, NOT an HBM measurement; reported with and without the CUDA-graph
+        # replay of the 2 nu launches of a history-free call (option "cuda_graph")
+        try:
+            c2 = CONFIGS[2]
+            L2, T2 = c2["L"], c2["T"]
+            V2 = L2 ** 3 * T2
+            ctx2 = Ddamg(L2, T2, c2["csw"], c2["m0"], c2["bc"], F32, stream=None, device=dev)
+            ctx2.load_gauge(gen.gauge_field(L2, T2, 1002, c2["eps"], c2["reunit"], device=dev, dtype=torch.complex64))
+            ctx2.build_clover()
+            b2 = ctx2.pack(gen.spinor_field(L2, T2, 2002, device=dev, dtype=torch.complex64), want_odd=False)[0]
+            x2 = ctx2.half_spinor()
+            row2 = {"lattice": "16^4 (fp32, 18-real links)", "nu": 8,
+                    "note": "L2-resident (gauge + clover 38 MB): launch-bound, not an HBM measurement; 200 calls each, x0 = 0"}
+            for name, mode in (("launches", 0), ("cuda_graph", 1)):
+                ctx2.set_option("cuda_graph", mode)
+                timed(lambda i: ctx2.richardson(b2, x2, 8, c2["omega"], zero_init=True), 200, 20)
+                st2 = step_stats(last_per_step)
+                row2[name + "_us_per_call"] = {k: (v * 1e3 if k != "n" else v) for k, v in st2.items()}
+                torch.cuda.synchronize(dev)
+                w0 = time.perf_counter()
+                for _ in range(200):
+                    ctx2.richardson(b2, x2, 8, c2["omega"], zero_init=True)
+                torch.cuda.synchronize(dev)
+                row2[name + "_wall_us_per_call"] = (time.perf_counter() - w0) / 200 * 1e6
+                flat[f"cfg2_{name}_us_per_call_median"] = st2["median"] * 1e3
+            row2["site_sweeps_per_s_cuda_graph_median"] = V2 * 8 / (row2["cuda_graph_us_per_call"]["median"] * 1e-6)
+            rows["config2_richardson_8_sweeps"] = row2
+            ctx2.close()
+            del ctx2, b2, x2
+        except Exception as exc:                  # noqa: BLE001
+            rows["config2_richardson_8_sweeps"] = {"error": str(exc)[:200]}
 
     if "cfg3" in sel and rank == 0 and world == 1:
         # ---- BASELINE.json configs[2] as written (SURVEY.md 8(d) cfg 3): 32^3 x 64, 100 calls of Richardson nu=4

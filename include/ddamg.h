@@ -99,7 +99,10 @@ int ddamg_load_gauge(ddamg_ctx* ctx, const void* U, int u_prec, int on_device);
  * Build the clover term (step a1) from the loaded links: per site the two Hermitian 6x6
  * blocks of A(x), computed in fp64, stored in the context precision;
  * A itself is kept on even sites, its INVERSE on odd sites ("explicitly storing the data
- * for D_oo^-1 is cheap").  Synchronises.  ESTATE without a gauge field; ESINGULAR if an
+ * for D_oo^-1 is cheap").  Storage (internal): the inverses as packed Hermitian blocks (36
+ * reals each); the blocks themselves in a compact 28-real form that uses their structure
+ * A_+- = (m0+4) + sum_k sigma_k (x) G_k (the lower-right 3x3 sub-block is 2(m0+4) minus the
+ * upper-left one), 224 instead of 288 bytes per even site in fp32.  Synchronises.  ESTATE without a gauge field; ESINGULAR if an
  * odd-site block has a pivot below 1e-12 * (largest entry of the block).
  */
 int ddamg_build_clover(ddamg_ctx* ctx);

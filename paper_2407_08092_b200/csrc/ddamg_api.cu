@@ -29,12 +29,12 @@ struct ddamg_ctx {
     int recon;                  // 18 or 12: link format read by the fused hopping kernels
     unsigned int* recon_dev;    // device: largest |stored row 2 - rebuilt row 2| of the last compression
     double recon_deviation;     // host copy of it
-    void* clov[2];              // [0] = A_ee blocks, [1] = A_oo^-1 blocks
+    void* clov[2];              // [0] = A_ee blocks (compact 28-real form), [1] = A_oo^-1 blocks (packed 36-real form)
     void* tmp_o;                // t_o of eq. 3
     void* tmp_e;                // scratch half spinor (power iteration, final residual)
     void* krylov;               // (kcap + 1) half spinors
     int kcap;
-    void* clov_oo;              // A itself on odd sites (built lazily: only the full operator D needs it)
+    void* clov_oo;              // A itself on odd sites, compact form (built lazily: only the full operator D needs it)
     Scalars* sc2;               // device scalars of the outer FGMRES (the inner smoother uses sc)
     void* fgm_basis;            // outer FGMRES: (fgm_cap + 1) V + fgm_cap Z full-lattice vectors
     int fgm_cap;
@@ -240,7 +240,8 @@ extern "C" int ddamg_create(ddamg_ctx** out, int L, int T, double csw, double m0
     memset(&ctx->rich_key, 0, sizeof ctx->rich_key);
 
     const size_t gauge_bytes = (size_t)2 * 4 * 18 * ctx->g.Vh * ctx->real_bytes;
-    const size_t clov_bytes = (size_t)72 * ctx->g.Vh * ctx->real_bytes;
+    const size_t clov_bytes = (size_t)72 * ctx->g.Vh * ctx->real_bytes;                   // A_oo^-1: packed 36 reals per block
+    const size_t clovA_bytes = (size_t)2 * CLOVA_REALS * ctx->g.Vh * ctx->real_bytes;     // A_ee: compact 28 reals per block
     const int dgrid = dslash_grid(ctx->g);
     // reduction scratch: 2 * dgrid norm partials (both parities of the full operator), or the partials of the
     // widest BLAS-1 grid (every BLAS-1 grid is <= blas_grid_cap(), whatever the vector length)
@@ -248,7 +249,7 @@ extern "C" int ddamg_create(ddamg_ctx** out, int L, int T, double csw, double m0
     ctx->partials_len = (size_t)(2 * dgrid > bcap * 2 * MDOT_NB ? 2 * dgrid : bcap * 2 * MDOT_NB);
     cudaError_t e = cudaSuccess;
     if (e == cudaSuccess) e = cudaMalloc(&ctx->gauge, gauge_bytes);
-    if (e == cudaSuccess) e = cudaMalloc(&ctx->clov[0], clov_bytes);
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->clov[0], clovA_bytes);
     if (e == cudaSuccess) e = cudaMalloc(&ctx->clov[1], clov_bytes);
     if (e == cudaSuccess) e = cudaMalloc(&ctx->tmp_o, ctx->half_bytes);
     if (e == cudaSuccess) e = cudaMalloc(&ctx->tmp_e, ctx->half_bytes);
@@ -383,8 +384,8 @@ extern "C" int ddamg_get_clover(ddamg_ctx* ctx, void* A_nat, void* Ainv_nat)
     ENTER(ctx);
     if (!ctx->have_clover) return fail(ctx, DDAMG_ESTATE, "ddamg_get_clover: clover not built");
     if (!A_nat && !Ainv_nat) return fail(ctx, DDAMG_EINVAL, "ddamg_get_clover: both outputs NULL");
-    if (ctx->prec == DDAMG_F32) launch_get_clover<float>(ctx->g, ctx->clov[0], ctx->clov[1], A_nat, Ainv_nat, ctx->stream);
-    else launch_get_clover<double>(ctx->g, ctx->clov[0], ctx->clov[1], A_nat, Ainv_nat, ctx->stream);
+    if (ctx->prec == DDAMG_F32) launch_get_clover<float>(ctx->g, ctx->m0 + 4.0, ctx->clov[0], ctx->clov[1], A_nat, Ainv_nat, ctx->stream);
+    else launch_get_clover<double>(ctx->g, ctx->m0 + 4.0, ctx->clov[0], ctx->clov[1], A_nat, Ainv_nat, ctx->stream);
     return after_launch(ctx);
 }
 
@@ -400,10 +401,10 @@ static int dslash(ddamg_ctx* ctx, int epi, bool norm, int parity, const void* in
     KernelTimer kt(ctx, which);
     if (ctx->prec == DDAMG_F32)
         launch_dslash<float>(ctx->g, epi, norm, parity, in, hop_gauge_block(ctx, parity), hop_gauge_block(ctx, 1 - parity),
-                             clov, own, rhs, out, omega, partials, units, ctx->batch_l2_bytes, ctx->recon, ctx->bc == 1, ctx->stream);
+                             clov, own, rhs, out, omega, ctx->m0 + 4.0, partials, units, ctx->batch_l2_bytes, ctx->recon, ctx->bc == 1, ctx->stream);
     else
         launch_dslash<double>(ctx->g, epi, norm, parity, in, hop_gauge_block(ctx, parity), hop_gauge_block(ctx, 1 - parity),
-                              clov, own, rhs, out, omega, partials, units, ctx->batch_l2_bytes, ctx->recon, ctx->bc == 1, ctx->stream);
+                              clov, own, rhs, out, omega, ctx->m0 + 4.0, partials, units, ctx->batch_l2_bytes, ctx->recon, ctx->bc == 1, ctx->stream);
     return after_launch(ctx);
 }
 
@@ -486,7 +487,7 @@ static int richardson_enqueue(ddamg_ctx* ctx, const void* b_e, void* x_e, int nu
 }
 
 // "auto": replay through a CUDA graph where the kernels are short enough for launch gaps to show
-// (measured in bench.py rows.config2_cuda_graph): up to 2^19 sites per parity
+// (measured in bench.py rows.config2_richardson_8_sweeps): up to 2^19 sites per parity
 static bool use_graph(ddamg_ctx* ctx) { return ctx->graph_mode == 1 || (ctx->graph_mode < 0 && ctx->g.Vh <= (1 << 19)); }
 
 extern "C" int ddamg_richardson(ddamg_ctx* ctx, const void* b_e, void* x_e, int nu, double omega, int zero_init,
@@ -958,7 +959,7 @@ static int ensure_full(ddamg_ctx* ctx, const char* who)
     if (s != DDAMG_OK) return s;
     if (ctx->have_clov_oo) return DDAMG_OK;
     if (!ctx->clov_oo) {
-        cudaError_t e = cudaMalloc(&ctx->clov_oo, (size_t)72 * ctx->g.Vh * ctx->real_bytes);
+        cudaError_t e = cudaMalloc(&ctx->clov_oo, (size_t)2 * CLOVA_REALS * ctx->g.Vh * ctx->real_bytes);
         if (e != cudaSuccess) { cudaGetLastError(); ctx->clov_oo = nullptr; return fail(ctx, DDAMG_ENOMEM, std::string(who) + ": cannot allocate A_oo"); }
     }
     if (ctx->prec == DDAMG_F32)
@@ -1221,8 +1222,8 @@ extern "C" int ddamg_sap(ddamg_ctx* ctx, const void* b_e, const void* b_o, void*
                 return fail(ctx, DDAMG_ENOMEM, "ddamg_sap: cannot allocate the block-ordered operand copies");
             }
         }
-        if (f32) launch_sap_reorder<float>(ctx->g, sg, recon, ctx->gauge, ctx->clov[0], ctx->clov[1], ctx->sap_links, ctx->sap_clov, st);
-        else launch_sap_reorder<double>(ctx->g, sg, recon, ctx->gauge, ctx->clov[0], ctx->clov[1], ctx->sap_links, ctx->sap_clov, st);
+        if (f32) launch_sap_reorder<float>(ctx->g, sg, recon, ctx->m0 + 4.0, ctx->gauge, ctx->clov[0], ctx->clov[1], ctx->sap_links, ctx->sap_clov, st);
+        else launch_sap_reorder<double>(ctx->g, sg, recon, ctx->m0 + 4.0, ctx->gauge, ctx->clov[0], ctx->clov[1], ctx->sap_links, ctx->sap_clov, st);
         s = after_launch(ctx);
         if (s != DDAMG_OK) return s;
         memcpy(ctx->sap_built, sg.B, sizeof(int) * 4);

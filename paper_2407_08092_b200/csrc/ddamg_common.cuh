@@ -9,7 +9,8 @@
 //     fp64 = 9 planes of double2; reals are row-major (row, col, re/im)
 //   * clover: per parity 2 blocks/site, each block 36 reals = 6 real diagonal entries then
 //     the 15 complex strictly-lower entries (1,0),(2,0),(2,1),(3,0),...,(5,4); stored as
-//     72/NV planes of Vh vectors (block 0 first)
+//     72/NV planes of Vh vectors (block 0 first).  This is the format of the INVERSES (A_oo^-1);
+//     the blocks themselves (A_ee, A_oo) use the compact 28-real form of load_clover_A below
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -123,28 +124,6 @@ __device__ __forceinline__ void store_spinor(float* __restrict__ base, int Vs, i
     for (int h = 0; h < 12; ++h) p[(size_t)h * Vs] = make_float4(s[2 * h].v.x, s[2 * h].v.y, s[2 * h + 1].v.x, s[2 * h + 1].v.y);
 }
 
-// L1 prefetch of the 16-byte vectors of one site's spinor (experiment, DDAMG_PF_L1)
-template <typename T, typename S>
-__device__ __forceinline__ void prefetch_spinor(const T* __restrict__ base, int Vs, int idx)
-{
-    using V = typename VecOf<T>::type;
-    constexpr int NPL = (sizeof(S) / sizeof(T)) * 24 / VecOf<T>::N;
-    const V* p = reinterpret_cast<const V*>(base) + idx;
-#pragma unroll
-    for (int k = 0; k < NPL; ++k) asm volatile("prefetch.global.L1 [%0];" ::"l"(p + (size_t)k * Vs));
-}
-
-// L1 prefetch of the two clover blocks of a site; the `units` threads of a site share the 72/N vectors
-template <typename T>
-__device__ __forceinline__ void prefetch_clover(const T* __restrict__ base, int Vh, int cb, int r, int units)
-{
-    using V = typename VecOf<T>::type;
-    constexpr int NPL = 72 / VecOf<T>::N;
-    const V* p = reinterpret_cast<const V*>(base) + cb;
-    if (units < 1) units = 1;
-    for (int k = r; k < NPL; k += units) asm volatile("prefetch.global.L1 [%0];" ::"l"(p + (size_t)k * Vh));
-}
-
 // 18 reals of one link; blk = start of the (parity, mu) block
 __device__ __forceinline__ void load_link(const float* __restrict__ blk, int Vh, int cb, float (&u)[18])
 {
@@ -244,6 +223,64 @@ __device__ __forceinline__ void store_clover_block(T* __restrict__ base, int Vh,
     V* p = reinterpret_cast<V*>(base) + (size_t)b * (36 / N) * Vh + cb;
 #pragma unroll
     for (int k = 0; k < 36 / N; ++k) p[(size_t)k * Vh] = pack(&c[k * N]);
+}
+
+// Compact storage of the clover blocks THEMSELVES (A_ee, and A_oo for the full operator; never the
+// inverses).  In the chiral basis a block is  A_+- = c0 1_6 + sum_k sigma_k (x) G_k  with c0 = m0 + 4
+// and G_k Hermitian 3x3 (R4: the clover term is traceless in spin), i.e. with rows /
+// columns ordered (spin, colour)
+//        [ c0 + G_3      M    ]
+//        [   M^H      c0 - G_3 ]          M = G_1 - i G_2
+// so the lower-right 3x3 block is 2 c0 - (upper-left block) and need not be stored: 27 reals
+// instead of 36.  Stored per block (CLOVA_REALS = 28 with one pad real: 7 float4 / 14 double2
+// planes): delta_i = A_ii - c0 (i = 0..2), the lower entries (1,0) (2,0) (2,1) of the upper-left
+// block, the 9 complex entries (3+i, j) of M^H, pad.  224 instead of 288 bytes per site in fp32.
+// load_clover_A expands into the ordinary packed 36 (6 real diagonal + 15 complex lower entries):
+// 3 additions, 3 subtractions, sign flips folded into the consumers' operands.
+constexpr int CLOVA_REALS = 28;
+template <typename T, bool STREAM = true>
+__device__ __forceinline__ void load_clover_A(const T* __restrict__ base, int Vh, int cb, int b, T c0, T (&c)[36])
+{
+    using V = typename VecOf<T>::type;
+    constexpr int N = VecOf<T>::N;
+    const V* p = reinterpret_cast<const V*>(base) + (size_t)b * (CLOVA_REALS / N) * Vh + cb;
+    T a[CLOVA_REALS];
+#pragma unroll
+    for (int k = 0; k < CLOVA_REALS / N; ++k) unpack(STREAM ? ld_stream(p + (size_t)k * Vh) : ld_reuse(p + (size_t)k * Vh), &a[k * N]);
+#pragma unroll
+    for (int i = 0; i < 3; ++i) { c[i] = c0 + a[i]; c[3 + i] = c0 - a[i]; }
+#pragma unroll
+    for (int i = 0; i < 6; ++i) c[6 + i] = a[3 + i];                  // (1,0) (2,0) (2,1)
+#pragma unroll
+    for (int i = 0; i < 6; ++i) c[12 + i] = a[9 + i];                 // (3,0) (3,1) (3,2)
+#pragma unroll
+    for (int i = 0; i < 6; ++i) c[18 + i] = a[15 + i];                // (4,0) (4,1) (4,2)
+    c[24] = -a[3]; c[25] = -a[4];                                     // (4,3) = -(1,0)
+#pragma unroll
+    for (int i = 0; i < 6; ++i) c[26 + i] = a[21 + i];                // (5,0) (5,1) (5,2)
+    c[32] = -a[5]; c[33] = -a[6];                                     // (5,3) = -(2,0)
+    c[34] = -a[7]; c[35] = -a[8];                                     // (5,4) = -(2,1)
+}
+// a = the CLOVA_REALS compact reals of one block (delta_0..2, (1,0) (2,0) (2,1), rows 3..5 x columns 0..2, pad);
+// the builders form delta in fp64 before rounding
+template <typename T>
+__device__ __forceinline__ void store_clover_A(T* __restrict__ base, int Vh, int cb, int b, const T (&a)[CLOVA_REALS])
+{
+    using V = typename VecOf<T>::type;
+    constexpr int N = VecOf<T>::N;
+    V* p = reinterpret_cast<V*>(base) + (size_t)b * (CLOVA_REALS / N) * Vh + cb;
+#pragma unroll
+    for (int k = 0; k < CLOVA_REALS / N; ++k) p[(size_t)k * Vh] = pack(&a[k * N]);
+}
+// packed 36 (fp64, as the builders hold it) -> compact, delta passed separately
+template <typename T>
+__device__ __forceinline__ void compact_clover_A(const double (&p)[36], const double (&delta)[3], T (&a)[CLOVA_REALS])
+{
+#pragma unroll
+    for (int i = 0; i < 3; ++i) a[i] = (T)delta[i];
+#pragma unroll
+    for (int i = 0; i < 6; ++i) { a[3 + i] = (T)p[6 + i]; a[9 + i] = (T)p[12 + i]; a[15 + i] = (T)p[18 + i]; a[21 + i] = (T)p[26 + i]; }
+    a[27] = 0;
 }
 
 // ------------------------------------------------------------------------- geometry

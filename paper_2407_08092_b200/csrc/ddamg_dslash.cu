@@ -16,36 +16,36 @@
 namespace ddamg {
 
 template void launch_dslash_recon<float, 18>(const Geom&, int, bool, int, const void*, const void*, const void*, const void*,
-                                             const void*, const void*, void*, double, double*, int, double, int, cudaStream_t);
+                                             const void*, const void*, void*, double, double, double*, int, double, int, cudaStream_t);
 template void launch_dslash_recon<double, 18>(const Geom&, int, bool, int, const void*, const void*, const void*, const void*,
-                                              const void*, const void*, void*, double, double*, int, double, int, cudaStream_t);
+                                              const void*, const void*, void*, double, double, double*, int, double, int, cudaStream_t);
 
 // instantiated in ddamg_dslash12.cu
 extern template void launch_dslash_recon<float, 12>(const Geom&, int, bool, int, const void*, const void*, const void*,
-                                                    const void*, const void*, const void*, void*, double, double*, int,
-                                                    double, int, cudaStream_t);
+                                                    const void*, const void*, const void*, void*, double, double, double*,
+                                                    int, double, int, cudaStream_t);
 extern template void launch_dslash_recon<double, 12>(const Geom&, int, bool, int, const void*, const void*, const void*,
-                                                     const void*, const void*, const void*, void*, double, double*, int,
-                                                     double, int, cudaStream_t);
+                                                     const void*, const void*, const void*, void*, double, double, double*,
+                                                     int, double, int, cudaStream_t);
 
 // recon = 18: gauge_* point into the full link blocks; recon = 12: into the two-row blocks
 template <typename T>
 void launch_dslash(const Geom& g, int epi, bool norm, int parity, const void* in, const void* gauge_own,
                    const void* gauge_opp, const void* clov, const void* own, const void* rhs, void* out,
-                   double omega, double* partials, int units, double batch_l2_bytes, int recon, int apbc,
+                   double omega, double c0, double* partials, int units, double batch_l2_bytes, int recon, int apbc,
                    cudaStream_t st)
 {
     if (recon == 12)
-        launch_dslash_recon<T, 12>(g, epi, norm, parity, in, gauge_own, gauge_opp, clov, own, rhs, out, omega, partials,
+        launch_dslash_recon<T, 12>(g, epi, norm, parity, in, gauge_own, gauge_opp, clov, own, rhs, out, omega, c0, partials,
                                    units, batch_l2_bytes, apbc, st);
     else
-        launch_dslash_recon<T, 18>(g, epi, norm, parity, in, gauge_own, gauge_opp, clov, own, rhs, out, omega, partials,
+        launch_dslash_recon<T, 18>(g, epi, norm, parity, in, gauge_own, gauge_opp, clov, own, rhs, out, omega, c0, partials,
                                    units, batch_l2_bytes, apbc, st);
 }
 template void launch_dslash<float>(const Geom&, int, bool, int, const void*, const void*, const void*, const void*,
-                                   const void*, const void*, void*, double, double*, int, double, int, int, cudaStream_t);
+                                   const void*, const void*, void*, double, double, double*, int, double, int, int, cudaStream_t);
 template void launch_dslash<double>(const Geom&, int, bool, int, const void*, const void*, const void*, const void*,
-                                    const void*, const void*, void*, double, double*, int, double, int, int, cudaStream_t);
+                                    const void*, const void*, void*, double, double, double*, int, double, int, int, cudaStream_t);
 
 // out = Cl in on one parity (right factor of eq. 2: t_o = A_oo^-1 b_o); units as in launch_dslash
 template <typename T, bool BATCH>

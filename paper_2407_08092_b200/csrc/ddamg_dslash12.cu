@@ -7,8 +7,8 @@
 namespace ddamg {
 
 template void launch_dslash_recon<float, 12>(const Geom&, int, bool, int, const void*, const void*, const void*, const void*,
-                                             const void*, const void*, void*, double, double*, int, double, int, cudaStream_t);
+                                             const void*, const void*, void*, double, double, double*, int, double, int, cudaStream_t);
 template void launch_dslash_recon<double, 12>(const Geom&, int, bool, int, const void*, const void*, const void*, const void*,
-                                              const void*, const void*, void*, double, double*, int, double, int, cudaStream_t);
+                                              const void*, const void*, void*, double, double, double*, int, double, int, cudaStream_t);
 
 }  // namespace ddamg

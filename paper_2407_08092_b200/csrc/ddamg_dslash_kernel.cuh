@@ -14,7 +14,9 @@ struct DslashArgs {
     const T* in;             // opposite-parity spinor (the 8 neighbours)
     const T* gauge_own;      // 4 link blocks of the output parity
     const T* gauge_opp;      // 4 link blocks of the opposite parity
-    const T* clov;           // clover blocks stored for the output parity
+    const T* clov;           // clover blocks of the output parity: the inverses (packed 36 reals per block) for
+                             // EPI_CLOV_*, the blocks themselves (compact 28 reals per block) for EPI >= EPI_SCHUR
+    T c0;                    // m0 + 4, the constant part of the compact blocks
     const T* own;            // own-site spinor (EPI_SCHUR / RICHARDSON / RESIDUAL)
     const T* rhs;            // b (EPI_RICHARDSON / RESIDUAL / *_RHS_*)
     T* out;
@@ -96,20 +98,7 @@ dslash_kernel(const DslashArgs<T> a)
     if (cb < a.g.Vh) {
         const Site s = site_of_cb(a.g, cb, a.parity);
         S acc[24];
-#ifdef DDAMG_PF_EPI
-        // L1 prefetch of the epilogue operands before the last direction pair (experiment)
-        auto mid = [&]() {
-            if (BATCH || DDAMG_PF_EPI > 1) {
-                if (EPI == EPI_CLOV_RHS_MINUS_HOP || EPI == EPI_RHS_MINUS_HOP) prefetch_spinor<T, S>(a.rhs, Vs, sv);
-                if (EPI > EPI_RHS_MINUS_HOP) prefetch_spinor<T, S>(a.own, Vs, sv);
-                if (EPI == EPI_RICHARDSON || EPI == EPI_RESIDUAL || EPI == EPI_FULL_RESIDUAL) prefetch_spinor<T, S>(a.rhs, Vs, sv);
-                if (EPI != EPI_RHS_MINUS_HOP) prefetch_clover<T>(a.clov, a.g.Vh, cb, rr, units);
-            }
-        };
-        hop_site<T, RECON, S>(a.g, cb, s, a.in, units, rr, a.gauge_own, a.gauge_opp, acc, a.apbc, mid);
-#else
         hop_site<T, RECON, S>(a.g, cb, s, a.in, units, rr, a.gauge_own, a.gauge_opp, acc, a.apbc);
-#endif
         S res[24];
         if (EPI == EPI_CLOV_HOP) {
 #pragma unroll
@@ -129,7 +118,7 @@ dslash_kernel(const DslashArgs<T> a)
         } else {
             S x[24], ax[24];
             load_spinor<T, true>(a.own, Vs, sv, x);
-            clover_site_mul<T>(a.clov, a.g.Vh, cb, x, ax);
+            clover_site_mul<T, true, true>(a.clov, a.g.Vh, cb, x, ax, a.c0);
             // H = -1/2 acc:  Schur forms subtract H t (+1/2 acc), the full operator adds H x (-1/2 acc)
             constexpr bool FULL = (EPI == EPI_FULL || EPI == EPI_FULL_RESIDUAL);
             const T hs = FULL ? (T)(-0.5) : (T)0.5;
@@ -183,7 +172,7 @@ static void launch(const DslashArgs<T>& a, cudaStream_t st)
 template <typename T, int RECON>
 void launch_dslash_recon(const Geom& g, int epi, bool norm, int parity, const void* in, const void* gauge_own,
                          const void* gauge_opp, const void* clov, const void* own, const void* rhs, void* out,
-                         double omega, double* partials, int units, double batch_l2_bytes, int apbc, cudaStream_t st)
+                         double omega, double c0, double* partials, int units, double batch_l2_bytes, int apbc, cudaStream_t st)
 {
     // units = 0: one right-hand side in the native half-spinor layout; units >= 1: multi-rhs batch with
     // that many threads per site (fp32: rhs pairs, fp64: rhs)
@@ -216,6 +205,7 @@ void launch_dslash_recon(const Geom& g, int epi, bool norm, int parity, const vo
     a.rhs = (const T*)rhs;
     a.out = (T*)out;
     a.omega = (T)omega;
+    a.c0 = (T)c0;
     a.partials = partials;
     switch (epi) {
     case EPI_CLOV_HOP: launch<T, EPI_CLOV_HOP, false, RECON>(a, st); break;

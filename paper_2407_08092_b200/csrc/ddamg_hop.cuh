@@ -152,13 +152,11 @@ __device__ __forceinline__ void hop_dir(const S (&psi)[24], const T (&u)[18], S 
 // one site read the same link vectors (one DRAM fetch, L1 broadcast).
 // RECON = 18: full links.  RECON = 12: two-row storage, third row rebuilt in registers
 // (load_link12); apbc != 0 then restores the antiperiodic sign of the links U_t(t = T-1).
-struct NoMid { __device__ __forceinline__ void operator()() const {} };
-template <typename T, int RECON, typename S, typename MID = NoMid>
+template <typename T, int RECON, typename S>
 __device__ __forceinline__ void hop_site(const Geom& g, int cb, const Site& s,
                                          const T* __restrict__ in, const int units, const int r,
                                          const T* __restrict__ gauge_own,
-                                         const T* __restrict__ gauge_opp, S (&acc)[24], const int apbc = 0,
-                                         const MID& mid = MID())
+                                         const T* __restrict__ gauge_opp, S (&acc)[24], const int apbc = 0)
 {
     const int Vs = g.Vh * units;                // vectors per spinor plane
     const size_t lblk = (size_t)RECON * g.Vh;   // reals per (parity, mu) link block
@@ -174,29 +172,20 @@ __device__ __forceinline__ void hop_site(const Geom& g, int cb, const Site& s,
     nbs[2] = neighbour_cb<1, +1>(g, cb, s); nbs[3] = neighbour_cb<1, -1>(g, cb, s);
     nbs[4] = neighbour_cb<2, +1>(g, cb, s); nbs[5] = neighbour_cb<2, -1>(g, cb, s);
     nbs[6] = neighbour_cb<3, +1>(g, cb, s); nbs[7] = neighbour_cb<3, -1>(g, cb, s);
-#ifdef DDAMG_PF_L1
-#define DDAMG_PF(nb) prefetch_spinor<T, S>(in, Vs, (nb) * units + r);
-#else
-#define DDAMG_PF(nb)
-#endif
 #define DDAMG_HOP(MU)                                                        \
     load_spinor<T>(in, Vs, nbs[2 * MU] * units + r, psi);                    \
-    DDAMG_PF(nbs[2 * MU + 1])                                                \
     if (RECON == 12) load_link12(gauge_own + MU * lblk, g.Vh, cb, MU == 3 ? sgn_f3 : (T)1, u); \
     else load_link(gauge_own + MU * lblk, g.Vh, cb, u);                      \
     hop_dir<MU, true, T, S>(psi, u, acc);                                    \
     load_spinor<T>(in, Vs, nbs[2 * MU + 1] * units + r, psi);                \
-    if (MU < 3) { DDAMG_PF(nbs[(2 * MU + 2) & 7]) }                          \
     if (RECON == 12) load_link12(gauge_opp + MU * lblk, g.Vh, nbs[2 * MU + 1], MU == 3 ? sgn_b3 : (T)1, u); \
     else load_link(gauge_opp + MU * lblk, g.Vh, nbs[2 * MU + 1], u);         \
     hop_dir<MU, false, T, S>(psi, u, acc);
     DDAMG_HOP(0)
     DDAMG_HOP(1)
     DDAMG_HOP(2)
-    mid();
     DDAMG_HOP(3)
 #undef DDAMG_HOP
-#undef DDAMG_PF
 }
 
 // y (6 complex) = M v for a packed Hermitian 6x6 block c (6 real diag, 15 complex lower)
@@ -256,15 +245,19 @@ __device__ __forceinline__ void clover_block_mul(const float (&c)[36], const flo
     }
 }
 
-// out = Cl(x) v for the two blocks of one site (upper: reals 0..11, lower: 12..23)
-template <typename T, bool STREAM = true, typename S>
+// out = Cl(x) v for the two blocks of one site (upper: reals 0..11, lower: 12..23).
+// AFMT = false: `clov` holds general Hermitian blocks (the inverses) in the packed 36-real form;
+// AFMT = true: it holds the clover blocks themselves in the compact 28-real form (c0 = m0 + 4).
+template <typename T, bool STREAM = true, bool AFMT = false, typename S>
 __device__ __forceinline__ void clover_site_mul(const T* __restrict__ clov, int Vh, int cb,
-                                                const S (&v)[24], S (&out)[24])
+                                                const S (&v)[24], S (&out)[24], T c0 = 0)
 {
     T c[36];
-    load_clover_block<T, STREAM>(clov, Vh, cb, 0, c);
+    if (AFMT) load_clover_A<T, STREAM>(clov, Vh, cb, 0, c0, c);
+    else load_clover_block<T, STREAM>(clov, Vh, cb, 0, c);
     clover_block_mul(c, &v[0], &out[0]);
-    load_clover_block<T, STREAM>(clov, Vh, cb, 1, c);
+    if (AFMT) load_clover_A<T, STREAM>(clov, Vh, cb, 1, c0, c);
+    else load_clover_block<T, STREAM>(clov, Vh, cb, 1, c);
     clover_block_mul(c, &v[12], &out[12]);
 }
 

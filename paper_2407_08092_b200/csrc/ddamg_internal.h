@@ -32,8 +32,10 @@ enum {
 template <typename T>
 void launch_dslash(const Geom& g, int epi, bool norm, int parity, const void* in, const void* gauge_own,
                    const void* gauge_opp, const void* clov, const void* own, const void* rhs, void* out,
-                   double omega, double* partials, int units, double batch_l2_bytes, int recon, int apbc,
+                   double omega, double c0, double* partials, int units, double batch_l2_bytes, int recon, int apbc,
                    cudaStream_t st);
+// clov: for EPI_CLOV_* the INVERSE blocks (packed 36 reals per block), for EPI >= EPI_SCHUR the blocks themselves in
+// the compact form of load_clover_A (CLOVA_REALS per block; c0 = m0 + 4)
 // `units`: 0 = one right-hand side in the native half-spinor layout; >= 1 = multi-rhs batch processed by that
 // many threads per site: fp32 -> pairs of right-hand sides (pair layout, batch_units()), fp64 -> right-hand sides
 inline int batch_units(int nrhs, size_t real_bytes) { return real_bytes == 4 ? (nrhs + 1) / 2 : nrhs; }
@@ -58,9 +60,10 @@ struct SapGeom {
 };
 size_t sap_smem_bytes(const SapGeom& sg, size_t real_bytes, int recon);
 // block-ordered copies of the links (2 * 4 * recon reals per site pair; recon = 18, or 12: rows 0 and 1) and of
-// A_ee / A_oo^-1 (2 * 72 reals per site pair), V/2 site pairs each, for one block geometry
+// A_ee / A_oo^-1 (2 * 72 reals per site pair, both expanded to the packed 36-real form), V/2 site pairs each, for
+// one block geometry; clov_e is the context's compact A_ee (c0 = m0 + 4)
 template <typename T>
-void launch_sap_reorder(const Geom& g, const SapGeom& sg, int recon, const void* gauge, const void* clov_e,
+void launch_sap_reorder(const Geom& g, const SapGeom& sg, int recon, double c0, const void* gauge, const void* clov_e,
                         const void* clov_oinv, void* blk_links, void* blk_clov, cudaStream_t st);
 // block solves of one colour: x += e, e -> (e_e, e_o), residual (rho, 0) -> (rn_e, rn_o) on those blocks
 template <typename T>
@@ -92,7 +95,7 @@ template <typename T>
 void launch_build_clover_pivoted(const Geom& g, double csw, double m0, const void* gauge, void* clov_e, void* clov_o,
                                  void* clov_o_plain, int* singular_flag, cudaStream_t st);
 template <typename T>
-void launch_get_clover(const Geom& g, const void* clov_e, const void* clov_o, void* A_nat, void* Ainv_nat,
+void launch_get_clover(const Geom& g, double c0, const void* clov_e, const void* clov_o, void* A_nat, void* Ainv_nat,
                        cudaStream_t st);
 
 // ---- BLAS-1 and the small dense part of GMRES (ddamg_blas.cu)

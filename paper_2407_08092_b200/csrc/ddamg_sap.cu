@@ -344,7 +344,7 @@ sap_block_kernel(const SapArgs<T> a)
 // the block's own SoA order (plane-major, n = V_b/2 sites per plane), block id = cx + nbx (cy +
 // nby (cz + nbz ct)) over the blocks of BOTH colours.
 template <typename T, int RECON>
-__global__ void sap_reorder_kernel(Geom g, SapGeom sg, const T* __restrict__ gauge, const T* __restrict__ clov_e,
+__global__ void sap_reorder_kernel(Geom g, SapGeom sg, T c0, const T* __restrict__ gauge, const T* __restrict__ clov_e,
                                    const T* __restrict__ clov_oinv, T* __restrict__ blk_links, T* __restrict__ blk_clov)
 {
     const int n = sg.Vbh, i = threadIdx.x;
@@ -372,27 +372,28 @@ __global__ void sap_reorder_kernel(Geom g, SapGeom sg, const T* __restrict__ gau
 #pragma unroll 1
         for (int b = 0; b < 2; ++b) {
             T c[36];
-            load_clover_block<T, true>(src, g.Vh, cbg, b, c);
+            if (p) load_clover_block<T, true>(src, g.Vh, cbg, b, c);
+            else load_clover_A<T, true>(src, g.Vh, cbg, b, c0, c);        // compact A_ee -> packed 36
             store_clover_block<T>(blk_clov + (bid * 2 + p) * 72 * n, n, i, b, c);
         }
     }
 }
 
 template <typename T>
-void launch_sap_reorder(const Geom& g, const SapGeom& sg, int recon, const void* gauge, const void* clov_e,
+void launch_sap_reorder(const Geom& g, const SapGeom& sg, int recon, double c0, const void* gauge, const void* clov_e,
                         const void* clov_oinv, void* blk_links, void* blk_clov, cudaStream_t st)
 {
     const int threads = (sg.Vbh + 31) / 32 * 32;
     const int grid = sg.nb[0] * sg.nb[1] * sg.nb[2] * sg.nb[3];
     if (recon == 12)
-        sap_reorder_kernel<T, 12><<<grid, threads, 0, st>>>(g, sg, (const T*)gauge, (const T*)clov_e, (const T*)clov_oinv,
+        sap_reorder_kernel<T, 12><<<grid, threads, 0, st>>>(g, sg, (T)c0, (const T*)gauge, (const T*)clov_e, (const T*)clov_oinv,
                                                             (T*)blk_links, (T*)blk_clov);
     else
-        sap_reorder_kernel<T, 18><<<grid, threads, 0, st>>>(g, sg, (const T*)gauge, (const T*)clov_e, (const T*)clov_oinv,
+        sap_reorder_kernel<T, 18><<<grid, threads, 0, st>>>(g, sg, (T)c0, (const T*)gauge, (const T*)clov_e, (const T*)clov_oinv,
                                                             (T*)blk_links, (T*)blk_clov);
 }
-template void launch_sap_reorder<float>(const Geom&, const SapGeom&, int, const void*, const void*, const void*, void*, void*, cudaStream_t);
-template void launch_sap_reorder<double>(const Geom&, const SapGeom&, int, const void*, const void*, const void*, void*, void*, cudaStream_t);
+template void launch_sap_reorder<float>(const Geom&, const SapGeom&, int, double, const void*, const void*, const void*, void*, void*, cudaStream_t);
+template void launch_sap_reorder<double>(const Geom&, const SapGeom&, int, double, const void*, const void*, const void*, void*, void*, cudaStream_t);
 
 size_t sap_smem_bytes(const SapGeom& sg, size_t real_bytes, int recon)
 {

@@ -412,15 +412,25 @@ __global__ void build_clover_pivoted_kernel(Geom g, double csw, double m0, const
       for (int blk = 0; blk < 2; ++blk) {
         double (&mr)[6][6] = blk ? lr : ur;
         double (&mi)[6][6] = blk ? li : ui;
-        for (int i = 0; i < 6; ++i) c[i] = (T)mr[i][i];
+        double pd[36];
+        for (int i = 0; i < 6; ++i) pd[i] = mr[i][i];
         for (int i = 1; i < 6; ++i)
             for (int j = 0; j < i; ++j) {
                 // Hermitian part of the lower triangle (rounding-level symmetrisation)
                 const int k = 6 + 2 * (i * (i - 1) / 2 + j);
-                c[k] = (T)(0.5 * (mr[i][j] + mr[j][i]));
-                c[k + 1] = (T)(0.5 * (mi[i][j] - mi[j][i]));
+                pd[k] = 0.5 * (mr[i][j] + mr[j][i]);
+                pd[k + 1] = 0.5 * (mi[i][j] - mi[j][i]);
             }
-        store_clover_block<T>(dst, g.Vh, cb, blk, c);
+        if (pass == 0) {
+            // the block itself: compact form (ddamg_common.cuh)
+            const double delta[3] = { mr[0][0] - (m0 + 4.0), mr[1][1] - (m0 + 4.0), mr[2][2] - (m0 + 4.0) };
+            T a[CLOVA_REALS];
+            compact_clover_A<T>(pd, delta, a);
+            store_clover_A<T>(dst, g.Vh, cb, blk, a);
+        } else {
+            for (int q = 0; q < 36; ++q) c[q] = (T)pd[q];
+            store_clover_block<T>(dst, g.Vh, cb, blk, c);
+        }
       }
     }
 }
@@ -704,9 +714,11 @@ build_clover_kernel(Geom g, double csw, double m0, const T* __restrict__ gauge,
     T c[36];
     T* plain = parity ? clov_o_plain : clov_e;
     if (plain) {
-#pragma unroll
-        for (int q = 0; q < 36; ++q) c[q] = (T)p[q];
-        store_clover_block<T>(plain, g.Vh, cb, h, c);
+        // the block itself: compact form (ddamg_common.cuh), delta_a = A_aa - c0 formed before rounding
+        const double delta[3] = { -kap * gz[0], -kap * gz[1], -kap * gz[2] };
+        T a[CLOVA_REALS];
+        compact_clover_A<T>(p, delta, a);
+        store_clover_A<T>(plain, g.Vh, cb, h, a);
     }
     if (parity == 1 && clov_o) {
         if (!invert6_ldl(p)) atomicOr(need_pivot, 1);
@@ -740,7 +752,7 @@ template void launch_build_clover_pivoted<double>(const Geom&, double, double, c
 
 // ------------------------------------------------------------------ debug: dense clover out
 template <typename T>
-__global__ void get_clover_kernel(Geom g, const T* __restrict__ clov_e, const T* __restrict__ clov_o,
+__global__ void get_clover_kernel(Geom g, T c0, const T* __restrict__ clov_e, const T* __restrict__ clov_o,
                                   T* __restrict__ A_nat, T* __restrict__ Ainv_nat)
 {
     const int idx = blockIdx.x * blockDim.x + threadIdx.x;
@@ -755,7 +767,8 @@ __global__ void get_clover_kernel(Geom g, const T* __restrict__ clov_e, const T*
     const T* src = parity ? clov_o : clov_e;
     for (int blk = 0; blk < 2; ++blk) {
         T c[36];
-        load_clover_block<T>(src, g.Vh, cb, blk, c);
+        if (parity) load_clover_block<T>(src, g.Vh, cb, blk, c);      // A_oo^-1: packed
+        else load_clover_A<T>(src, g.Vh, cb, blk, c0, c);             // A_ee: compact
         T* out = mine + n * 144 + blk * 72;
         for (int i = 0; i < 6; ++i)
             for (int j = 0; j < 6; ++j) {
@@ -770,14 +783,14 @@ __global__ void get_clover_kernel(Geom g, const T* __restrict__ clov_e, const T*
 }
 
 template <typename T>
-void launch_get_clover(const Geom& g, const void* clov_e, const void* clov_o, void* A_nat, void* Ainv_nat,
+void launch_get_clover(const Geom& g, double c0, const void* clov_e, const void* clov_o, void* A_nat, void* Ainv_nat,
                        cudaStream_t st)
 {
     const int n = 2 * g.Vh;
-    get_clover_kernel<T><<<(n + 127) / 128, 128, 0, st>>>(g, (const T*)clov_e, (const T*)clov_o, (T*)A_nat,
+    get_clover_kernel<T><<<(n + 127) / 128, 128, 0, st>>>(g, (T)c0, (const T*)clov_e, (const T*)clov_o, (T*)A_nat,
                                                            (T*)Ainv_nat);
 }
-template void launch_get_clover<float>(const Geom&, const void*, const void*, void*, void*, cudaStream_t);
-template void launch_get_clover<double>(const Geom&, const void*, const void*, void*, void*, cudaStream_t);
+template void launch_get_clover<float>(const Geom&, double, const void*, const void*, void*, void*, cudaStream_t);
+template void launch_get_clover<double>(const Geom&, double, const void*, const void*, void*, void*, cudaStream_t);
 
 }  // namespace ddamg

@@ -243,6 +243,25 @@ def test_clover_chiral_block_form_and_6x6_structure():
     assert np.abs(A[..., 6:, 6:] - lo).max() < 1e-13
 
 
+@pytest.mark.parametrize("cfg", [1, 3])
+def test_clover_blocks_are_constant_plus_spin_traceless(cfg):
+    """The property the CUDA path's compact storage of A_ee / A_oo relies on: each
+    6x6 block is (m0+4) 1 + sum_k sigma_k (x) G_k, so with rows ordered (spin, colour) its lower-right 3x3
+    sub-block equals 2(m0+4) - (upper-left sub-block) and its off-diagonal sub-blocks are each other's
+    adjoint.  Checked on the oracle's own A (which is built entry by entry from gamma_mu gamma_nu (x) F'),
+    so the statement does not depend on the chiral-block restatement above.  The INVERSE has no such
+    structure (it is stored in full)."""
+    op = make(cfg, 4, 4)
+    c0 = CONFIGS[cfg]["m0"] + 4.0
+    for b in (0, 1):
+        B = op.A[..., 6 * b:6 * b + 6, 6 * b:6 * b + 6]
+        ul, lr, ll, ur = B[..., :3, :3], B[..., 3:, 3:], B[..., 3:, :3], B[..., :3, 3:]
+        assert np.abs(lr - (2.0 * c0 * np.eye(3) - ul)).max() < 1e-14
+        assert np.abs(ll - np.conj(np.swapaxes(ur, -1, -2))).max() < 1e-14
+        Bi = op.Ainv[..., 6 * b:6 * b + 6, 6 * b:6 * b + 6]
+        assert np.abs(Bi[..., 3:, 3:] + Bi[..., :3, :3] - 2.0 / c0 * np.eye(3)).max() > 1e-3
+
+
 def test_clover_independent_of_time_boundary_sign():
     """Every leaf crosses the t boundary an even number of times (reading R2)."""
     U = _np(config_gauge(1))
