@@ -56,7 +56,7 @@ BYTES_BR = BYTES_B + 96 # kernel B': kernel B + b_e 96                          
 FLOP_PER_SITE = 1824    # 1320 (hop) + 504 (2 x 6x6 Hermitian mat-vec), per lattice site
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of kernel B' at config 5, from the
 # ncu --set full capture summarised in profiles/ (None until a capture exists)
-NCU_TRAFFIC_BYTES = {18: {5: 21.274e9}, 12: {5: 18.038e9}}     # profiles/r1b_ncu_full_dslash.md, profiles/r2_ncu_full_dslash12.md
+NCU_TRAFFIC_BYTES = {18: {}, 12: {5: 16.956e9}}     # profiles/r2b_ncu_full_dslash12.md (kernel B' with the compact A_ee)
 NOMINAL_HBM_GBS = 8000.0    # north_star's "~8 TB/s HBM peak" (DGX figure; HGX 7.7 TB/s), quoted beside the measured copy peak
 SIDE_ROWS = ("links18", "schur", "smoother", "gmres", "gcr", "sap", "multi_rhs", "paper", "f64", "cfg2", "cfg3", "cfg4")
 CPU_SAMPLE = dict(L=16, T=32)
@@ -706,18 +706,12 @@ def main():
             b2 = ctx2.pack(gen.spinor_field(L2, T2, 2002, device=dev, dtype=torch.complex64), want_odd=False)[0]
             x2 = ctx2.half_spinor()
             row2 = {"lattice": "16^4 (fp32, 18-real links)", "nu": 8,
-                    "note": "L2-resident (gauge + clover 38 MB): launch-bound, not an HBM measurement; 200 calls each, x0 = 0"}
+                    "note": "L2-resident (gauge + clover 38 MB): launch-bound, not an HBM measurement; 40 calls each (CUDA events per call), x0 = 0"}
             for name, mode in (("launches", 0), ("cuda_graph", 1)):
                 ctx2.set_option("cuda_graph", mode)
-                timed(lambda i: ctx2.richardson(b2, x2, 8, c2["omega"], zero_init=True), 200, 20)
+                timed(lambda i: ctx2.richardson(b2, x2, 8, c2["omega"], zero_init=True), 40, 5)
                 st2 = step_stats(last_per_step)
                 row2[name + "_us_per_call"] = {k: (v * 1e3 if k != "n" else v) for k, v in st2.items()}
-                torch.cuda.synchronize(dev)
-                w0 = time.perf_counter()
-                for _ in range(200):
-                    ctx2.richardson(b2, x2, 8, c2["omega"], zero_init=True)
-                torch.cuda.synchronize(dev)
-                row2[name + "_wall_us_per_call"] = (time.perf_counter() - w0) / 200 * 1e6
                 flat[f"cfg2_{name}_us_per_call_median"] = st2["median"] * 1e3
             row2["site_sweeps_per_s_cuda_graph_median"] = V2 * 8 / (row2["cuda_graph_us_per_call"]["median"] * 1e-6)
             rows["config2_richardson_8_sweeps"] = row2
