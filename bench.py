@@ -56,7 +56,7 @@ BYTES_BR = BYTES_B + 96 # kernel B': kernel B + b_e 96                          
 FLOP_PER_SITE = 1824    # 1320 (hop) + 504 (2 x 6x6 Hermitian mat-vec), per lattice site
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of kernel B' at config 5, from the
 # ncu --set full capture summarised in profiles/ (None until a capture exists)
-NCU_TRAFFIC_BYTES = {18: {}, 12: {5: 16.956e9}}     # profiles/r2b_ncu_full_dslash12.md (kernel B' with the compact A_ee)
+NCU_TRAFFIC_BYTES = {18: {5: 20.194e9}, 12: {5: 16.956e9}}     # profiles/r2b_ncu_full_dslash18.md, profiles/r2b_ncu_full_dslash12.md
 NOMINAL_HBM_GBS = 8000.0    # north_star's "~8 TB/s HBM peak" (DGX figure; HGX 7.7 TB/s), quoted beside the measured copy peak
 SIDE_ROWS = ("links18", "schur", "smoother", "gmres", "gcr", "sap", "multi_rhs", "paper", "f64", "cfg2", "cfg3", "cfg4")
 CPU_SAMPLE = dict(L=16, T=32)
