@@ -1222,8 +1222,8 @@ extern "C" int ddamg_sap(ddamg_ctx* ctx, const void* b_e, const void* b_o, void*
                 return fail(ctx, DDAMG_ENOMEM, "ddamg_sap: cannot allocate the block-ordered operand copies");
             }
         }
-        if (f32) launch_sap_reorder<float>(ctx->g, sg, recon, ctx->m0 + 4.0, ctx->gauge, ctx->clov[0], ctx->clov[1], ctx->sap_links, ctx->sap_clov, st);
-        else launch_sap_reorder<double>(ctx->g, sg, recon, ctx->m0 + 4.0, ctx->gauge, ctx->clov[0], ctx->clov[1], ctx->sap_links, ctx->sap_clov, st);
+        if (f32) launch_sap_reorder<float>(ctx->g, sg, recon, ctx->gauge, ctx->clov[0], ctx->clov[1], ctx->sap_links, ctx->sap_clov, st);
+        else launch_sap_reorder<double>(ctx->g, sg, recon, ctx->gauge, ctx->clov[0], ctx->clov[1], ctx->sap_links, ctx->sap_clov, st);
         s = after_launch(ctx);
         if (s != DDAMG_OK) return s;
         memcpy(ctx->sap_built, sg.B, sizeof(int) * 4);
@@ -1252,8 +1252,8 @@ extern "C" int ddamg_sap(ddamg_ctx* ctx, const void* b_e, const void* b_o, void*
         {
             KernelTimer kt(ctx, KT_SAP);
             cudaError_t e = f32
-                ? launch_sap_blocks<float>(ctx->g, sg, recon, colour, m, ctx->sap_links, ctx->sap_clov, rin_e, rin_o, r_e, r_o, e_e, e_o, x_e, x_o, st)
-                : launch_sap_blocks<double>(ctx->g, sg, recon, colour, m, ctx->sap_links, ctx->sap_clov, rin_e, rin_o, r_e, r_o, e_e, e_o, x_e, x_o, st);
+                ? launch_sap_blocks<float>(ctx->g, sg, recon, ctx->m0 + 4.0, colour, m, ctx->sap_links, ctx->sap_clov, rin_e, rin_o, r_e, r_o, e_e, e_o, x_e, x_o, st)
+                : launch_sap_blocks<double>(ctx->g, sg, recon, ctx->m0 + 4.0, colour, m, ctx->sap_links, ctx->sap_clov, rin_e, rin_o, r_e, r_o, e_e, e_o, x_e, x_o, st);
             if (e != cudaSuccess) return check_cuda(ctx, e, "sap_block_kernel attributes");
         }
         int q = after_launch(ctx);

@@ -60,14 +60,14 @@ struct SapGeom {
 };
 size_t sap_smem_bytes(const SapGeom& sg, size_t real_bytes, int recon);
 // block-ordered copies of the links (2 * 4 * recon reals per site pair; recon = 18, or 12: rows 0 and 1) and of
-// A_ee / A_oo^-1 (2 * 72 reals per site pair, both expanded to the packed 36-real form), V/2 site pairs each, for
-// one block geometry; clov_e is the context's compact A_ee (c0 = m0 + 4)
+// A_ee / A_oo^-1 (slots of 72 reals per site; A_ee keeps its compact form and uses 2 * CLOVA_REALS of its slot),
+// V/2 site pairs each, for one block geometry; clov_e is the context's compact A_ee
 template <typename T>
-void launch_sap_reorder(const Geom& g, const SapGeom& sg, int recon, double c0, const void* gauge, const void* clov_e,
+void launch_sap_reorder(const Geom& g, const SapGeom& sg, int recon, const void* gauge, const void* clov_e,
                         const void* clov_oinv, void* blk_links, void* blk_clov, cudaStream_t st);
 // block solves of one colour: x += e, e -> (e_e, e_o), residual (rho, 0) -> (rn_e, rn_o) on those blocks
 template <typename T>
-cudaError_t launch_sap_blocks(const Geom& g, const SapGeom& sg, int recon, int colour, int m, const void* blk_links,
+cudaError_t launch_sap_blocks(const Geom& g, const SapGeom& sg, int recon, double c0, int colour, int m, const void* blk_links,
                               const void* blk_clov, const void* r_e, const void* r_o, void* rn_e, void* rn_o,
                               void* e_e, void* e_o, void* x_e, void* x_o, cudaStream_t st);
 // rn = r - (hops across block faces) e on the sites of colour `target`; gauge: the hopping kernels' link blocks

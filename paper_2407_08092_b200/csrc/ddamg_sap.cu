@@ -17,7 +17,7 @@
 // and odd site i of the block (all lanes busy in both half steps); the block's links (the only
 // operand re-used by all 2m+3 hopping applications) are staged ONCE in shared memory, the two
 // exchanged half-block spinors live in shared memory, e and rho stay in registers, the 6x6
-// clover blocks are re-read through L1/L2 (73 KB per 4^4 block: L2-resident).  All dot
+// clover blocks are re-read through L1/L2 (65 KB per 4^4 block with A_ee in its compact form: L2-resident).  All dot
 // products are block-local: one CTA-wide fp64 reduction per MR iteration, no
 // global reduction, no host involvement.
 //
@@ -41,7 +41,8 @@ struct SapArgs {
     int colour;              // colour of the blocks this launch solves (0 = red)
     int m;                   // Minimal Residual iterations (>= 1)
     const T* blk_links;      // block-ordered links:  [block][parity][mu][RECON * n]   (sap_reorder_kernel)
-    const T* blk_clov;       // block-ordered A_ee / A_oo^-1 blocks:  [block][parity][72 * n]
+    const T* blk_clov;       // block-ordered A_ee (compact form, 2 * CLOVA_REALS * n of the slot used) / A_oo^-1 blocks (packed):  [block][parity][72 * n]
+    T c0;                    // m0 + 4, the constant part of the compact A_ee blocks
     const T* r_e;            // global residual r = b - D x (read on the blocks of this colour)
     const T* r_o;
     T* rn_e;                 // residual after the update, written on the blocks of this colour: (rho, 0)
@@ -293,7 +294,7 @@ sap_block_kernel(const SapArgs<T> a)
             T q[24];
             double nr = 0.0, ni = 0.0, dd = 0.0;
             if (active) {
-                clover_site_mul<T, false>(clov_e, n, tid, rho, q);
+                clover_site_mul<T, false, true>(clov_e, n, tid, rho, q, a.c0);
 #pragma unroll
                 for (int i = 0; i < 24; ++i) q[i] = q[i] + (T)0.5 * acc[i];
                 // <q, rho> = q^H rho and <q, q>, this site's share: the 12 complex products of the site in the
@@ -344,7 +345,7 @@ sap_block_kernel(const SapArgs<T> a)
 // the block's own SoA order (plane-major, n = V_b/2 sites per plane), block id = cx + nbx (cy +
 // nby (cz + nbz ct)) over the blocks of BOTH colours.
 template <typename T, int RECON>
-__global__ void sap_reorder_kernel(Geom g, SapGeom sg, T c0, const T* __restrict__ gauge, const T* __restrict__ clov_e,
+__global__ void sap_reorder_kernel(Geom g, SapGeom sg, const T* __restrict__ gauge, const T* __restrict__ clov_e,
                                    const T* __restrict__ clov_oinv, T* __restrict__ blk_links, T* __restrict__ blk_clov)
 {
     const int n = sg.Vbh, i = threadIdx.x;
@@ -372,28 +373,37 @@ __global__ void sap_reorder_kernel(Geom g, SapGeom sg, T c0, const T* __restrict
 #pragma unroll 1
         for (int b = 0; b < 2; ++b) {
             T c[36];
-            if (p) load_clover_block<T, true>(src, g.Vh, cbg, b, c);
-            else load_clover_A<T, true>(src, g.Vh, cbg, b, c0, c);        // compact A_ee -> packed 36
-            store_clover_block<T>(blk_clov + (bid * 2 + p) * 72 * n, n, i, b, c);
+            if (p) {
+                load_clover_block<T, true>(src, g.Vh, cbg, b, c);
+                store_clover_block<T>(blk_clov + (bid * 2 + p) * 72 * n, n, i, b, c);
+            } else {
+                // A_ee stays in the compact form (CLOVA_REALS per block): a plain copy of its vectors
+                using V = typename VecOf<T>::type;
+                constexpr int NV = CLOVA_REALS / VecOf<T>::N;
+                const V* sv = reinterpret_cast<const V*>(src) + (size_t)b * NV * g.Vh + cbg;
+                V* dv = reinterpret_cast<V*>(blk_clov + (bid * 2 + p) * 72 * n) + (size_t)b * NV * n + i;
+#pragma unroll
+                for (int k = 0; k < NV; ++k) dv[(size_t)k * n] = ld_stream(sv + (size_t)k * g.Vh);
+            }
         }
     }
 }
 
 template <typename T>
-void launch_sap_reorder(const Geom& g, const SapGeom& sg, int recon, double c0, const void* gauge, const void* clov_e,
+void launch_sap_reorder(const Geom& g, const SapGeom& sg, int recon, const void* gauge, const void* clov_e,
                         const void* clov_oinv, void* blk_links, void* blk_clov, cudaStream_t st)
 {
     const int threads = (sg.Vbh + 31) / 32 * 32;
     const int grid = sg.nb[0] * sg.nb[1] * sg.nb[2] * sg.nb[3];
     if (recon == 12)
-        sap_reorder_kernel<T, 12><<<grid, threads, 0, st>>>(g, sg, (T)c0, (const T*)gauge, (const T*)clov_e, (const T*)clov_oinv,
+        sap_reorder_kernel<T, 12><<<grid, threads, 0, st>>>(g, sg, (const T*)gauge, (const T*)clov_e, (const T*)clov_oinv,
                                                             (T*)blk_links, (T*)blk_clov);
     else
-        sap_reorder_kernel<T, 18><<<grid, threads, 0, st>>>(g, sg, (T)c0, (const T*)gauge, (const T*)clov_e, (const T*)clov_oinv,
+        sap_reorder_kernel<T, 18><<<grid, threads, 0, st>>>(g, sg, (const T*)gauge, (const T*)clov_e, (const T*)clov_oinv,
                                                             (T*)blk_links, (T*)blk_clov);
 }
-template void launch_sap_reorder<float>(const Geom&, const SapGeom&, int, double, const void*, const void*, const void*, void*, void*, cudaStream_t);
-template void launch_sap_reorder<double>(const Geom&, const SapGeom&, int, double, const void*, const void*, const void*, void*, void*, cudaStream_t);
+template void launch_sap_reorder<float>(const Geom&, const SapGeom&, int, const void*, const void*, const void*, void*, void*, cudaStream_t);
+template void launch_sap_reorder<double>(const Geom&, const SapGeom&, int, const void*, const void*, const void*, void*, void*, cudaStream_t);
 
 size_t sap_smem_bytes(const SapGeom& sg, size_t real_bytes, int recon)
 {
@@ -410,12 +420,12 @@ static cudaError_t launch_blocks_as(const SapArgs<T>& a, int threads, int grid, 
 }
 
 template <typename T>
-cudaError_t launch_sap_blocks(const Geom& g, const SapGeom& sg, int recon, int colour, int m, const void* blk_links,
+cudaError_t launch_sap_blocks(const Geom& g, const SapGeom& sg, int recon, double c0, int colour, int m, const void* blk_links,
                               const void* blk_clov, const void* r_e, const void* r_o, void* rn_e, void* rn_o,
                               void* e_e, void* e_o, void* x_e, void* x_o, cudaStream_t st)
 {
     SapArgs<T> a;
-    a.g = g; a.sg = sg; a.colour = colour; a.m = m;
+    a.g = g; a.sg = sg; a.colour = colour; a.m = m; a.c0 = (T)c0;
     a.blk_links = (const T*)blk_links; a.blk_clov = (const T*)blk_clov;
     a.r_e = (const T*)r_e; a.r_o = (const T*)r_o; a.rn_e = (T*)rn_e; a.rn_o = (T*)rn_o;
     a.e_e = (T*)e_e; a.e_o = (T*)e_o; a.x_e = (T*)x_e; a.x_o = (T*)x_o;
@@ -432,9 +442,9 @@ cudaError_t launch_sap_blocks(const Geom& g, const SapGeom& sg, int recon, int c
     return recon == 12 ? launch_blocks_as<T, 12, SAP_MAX_THREADS, false>(a, threads, grid, smem, st)
                        : launch_blocks_as<T, 18, SAP_MAX_THREADS, false>(a, threads, grid, smem, st);
 }
-template cudaError_t launch_sap_blocks<float>(const Geom&, const SapGeom&, int, int, int, const void*, const void*,
+template cudaError_t launch_sap_blocks<float>(const Geom&, const SapGeom&, int, double, int, int, const void*, const void*,
                                               const void*, const void*, void*, void*, void*, void*, void*, void*, cudaStream_t);
-template cudaError_t launch_sap_blocks<double>(const Geom&, const SapGeom&, int, int, int, const void*, const void*,
+template cudaError_t launch_sap_blocks<double>(const Geom&, const SapGeom&, int, double, int, int, const void*, const void*,
                                                const void*, const void*, void*, void*, void*, void*, void*, void*, cudaStream_t);
 
 // ---- incremental residual (Alg. 1 lines 2 / 7 after the first evaluation): for every site of colour `target`
