@@ -15,7 +15,7 @@
 // with D^k_S = A_ee - H^k_eo A_oo^-1 H^k_oe and H^k the hopping term with every hop that leaves
 // the block dropped (D_k = P_k D P_k^T, R21).  B200 mapping: thread i owns even site i
 // and odd site i of the block (all lanes busy in both half steps); the block's links (the only
-// operand re-used by all 2m+3 hopping applications) are staged ONCE in shared memory, the two
+// operand re-used by all 2m+3 hopping applications) are staged ONCE in shared memory (one TMA bulk copy), the two
 // exchanged half-block spinors live in shared memory, e and rho stay in registers, the 6x6
 // clover blocks are re-read through L1/L2 (65 KB per 4^4 block with A_ee in its compact form: L2-resident).  All dot
 // products are block-local: one CTA-wide fp64 reduction per MR iteration, no
@@ -218,14 +218,21 @@ sap_block_kernel(const SapArgs<T> a)
         }
     }
     const int sblk = 4 * RECON * n;                            // one parity's four link blocks in shared memory
-    {
-        // ---- stage the block's links (read once from HBM per launch): the block-ordered copy has
-        // the shared-memory layout, so this is one contiguous, fully coalesced 16-byte-vector copy
-        using V = typename VecOf<T>::type;
-        const V* src = reinterpret_cast<const V*>(a.blk_links + bid * 2 * sblk);
-        V* dst = reinterpret_cast<V*>(links);
-        const int nv = 2 * sblk / VecOf<T>::N;
-        for (int i = tid; i < nv; i += blockDim.x) dst[i] = ld_stream(src + i);
+    // ---- stage the block's links (read once from HBM per launch): the block-ordered copy has the
+    // shared-memory layout, so this is ONE contiguous bulk copy (TMA engine, `cp.async.bulk`, SASS UBLKCP)
+    // issued by one thread and tracked by an mbarrier; it runs behind the prologue's own global loads
+    // instead of in front of them, and no thread spends instructions or registers on it.
+    unsigned long long* bar = reinterpret_cast<unsigned long long*>(red + 3 * 32);
+    const unsigned bar_s = (unsigned)__cvta_generic_to_shared(bar);
+    if (tid == 0) {
+        const unsigned bytes = (unsigned)(2 * sblk * sizeof(T));
+        const unsigned dst_s = (unsigned)__cvta_generic_to_shared(links);
+        const T* src = a.blk_links + bid * 2 * sblk;
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar_s));
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar_s), "r"(bytes) : "memory");
+        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                     ::"r"(dst_s), "l"(src), "r"(bytes), "r"(bar_s) : "memory");
     }
     if (active) {
         // ---- eq. 2 right factor, odd half: t_o = A_oo^-1 r_o;  rho starts as r_e
@@ -235,7 +242,14 @@ sap_block_kernel(const SapArgs<T> a)
         sts_spinor<T>(S_o, n, tid, t);
         load_spinor<T, true>(a.r_e, a.g.Vh, cbg[0], rho);
     }
-    __syncthreads();
+    __syncthreads();                                           // S_o complete; the barrier's init is visible
+    {
+        // wait for the links (phase 0 of the mbarrier)
+        unsigned done = 0;
+        while (!done)
+            asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], 0; selp.u32 %0, 1, 0, p; }"
+                         : "=r"(done) : "r"(bar_s) : "memory");
+    }
 
     // ---- the block solve as 2m+2 half steps, one copy of the block hopping code:
     //   hs = 0        even:  rho = rhat_e = r_e - H^k_eo t_o;  e = 0
@@ -407,7 +421,7 @@ template void launch_sap_reorder<double>(const Geom&, const SapGeom&, int, const
 
 size_t sap_smem_bytes(const SapGeom& sg, size_t real_bytes, int recon)
 {
-    return (size_t)(2 * 4 * recon + 48) * sg.Vbh * real_bytes + (size_t)32 * 3 * sizeof(double);
+    return (size_t)(2 * 4 * recon + 48) * sg.Vbh * real_bytes + (size_t)32 * 3 * sizeof(double) + 16;    // + the mbarrier of the link copy
 }
 
 template <typename T, int RECON, int MAXT, bool B4>
