@@ -204,16 +204,26 @@ __device__ __forceinline__ void store_link12(double* __restrict__ blk, int Vh, i
     for (int k = 0; k < 6; ++k) p[(size_t)k * Vh] = pack(&u[2 * k]);
 }
 
-// 36 reals of clover block b (0/1) of one site.  STREAM: read once per kernel (evict-first);
-// !STREAM: re-read by the same CTA (SAP block solves), keep it cacheable.
-template <typename T, bool STREAM = true>
+// load modes of the clover accessors: LD_REUSE = global, read-only path, cacheable (re-read by the same CTA);
+// LD_STREAM = global, read once per kernel (evict-first); LD_PLAIN = ordinary load (shared memory: the SAP
+// block kernel's staged blocks).  (false / true convert to LD_REUSE / LD_STREAM.)
+enum { LD_REUSE = 0, LD_STREAM = 1, LD_PLAIN = 2 };
+template <int MODE, typename V>
+__device__ __forceinline__ V ld_mode(const V* p)
+{
+    if (MODE == LD_STREAM) return ld_stream(p);
+    if (MODE == LD_REUSE) return ld_reuse(p);
+    return *p;
+}
+// 36 reals of clover block b (0/1) of one site
+template <typename T, int MODE = LD_STREAM>
 __device__ __forceinline__ void load_clover_block(const T* __restrict__ base, int Vh, int cb, int b, T (&c)[36])
 {
     using V = typename VecOf<T>::type;
     constexpr int N = VecOf<T>::N;
     const V* p = reinterpret_cast<const V*>(base) + (size_t)b * (36 / N) * Vh + cb;
 #pragma unroll
-    for (int k = 0; k < 36 / N; ++k) unpack(STREAM ? ld_stream(p + (size_t)k * Vh) : ld_reuse(p + (size_t)k * Vh), &c[k * N]);
+    for (int k = 0; k < 36 / N; ++k) unpack(ld_mode<MODE>(p + (size_t)k * Vh), &c[k * N]);
 }
 template <typename T>
 __device__ __forceinline__ void store_clover_block(T* __restrict__ base, int Vh, int cb, int b, const T (&c)[36])
@@ -238,7 +248,7 @@ __device__ __forceinline__ void store_clover_block(T* __restrict__ base, int Vh,
 // load_clover_A expands into the ordinary packed 36 (6 real diagonal + 15 complex lower entries):
 // 3 additions, 3 subtractions, sign flips folded into the consumers' operands.
 constexpr int CLOVA_REALS = 28;
-template <typename T, bool STREAM = true>
+template <typename T, int MODE = LD_STREAM>
 __device__ __forceinline__ void load_clover_A(const T* __restrict__ base, int Vh, int cb, int b, T c0, T (&c)[36])
 {
     using V = typename VecOf<T>::type;
@@ -246,7 +256,7 @@ __device__ __forceinline__ void load_clover_A(const T* __restrict__ base, int Vh
     const V* p = reinterpret_cast<const V*>(base) + (size_t)b * (CLOVA_REALS / N) * Vh + cb;
     T a[CLOVA_REALS];
 #pragma unroll
-    for (int k = 0; k < CLOVA_REALS / N; ++k) unpack(STREAM ? ld_stream(p + (size_t)k * Vh) : ld_reuse(p + (size_t)k * Vh), &a[k * N]);
+    for (int k = 0; k < CLOVA_REALS / N; ++k) unpack(ld_mode<MODE>(p + (size_t)k * Vh), &a[k * N]);
 #pragma unroll
     for (int i = 0; i < 3; ++i) { c[i] = c0 + a[i]; c[3 + i] = c0 - a[i]; }
 #pragma unroll

@@ -248,16 +248,17 @@ __device__ __forceinline__ void clover_block_mul(const float (&c)[36], const flo
 // out = Cl(x) v for the two blocks of one site (upper: reals 0..11, lower: 12..23).
 // AFMT = false: `clov` holds general Hermitian blocks (the inverses) in the packed 36-real form;
 // AFMT = true: it holds the clover blocks themselves in the compact 28-real form (c0 = m0 + 4).
-template <typename T, bool STREAM = true, bool AFMT = false, typename S>
+// MODE: LD_STREAM / LD_REUSE (global) or LD_PLAIN (`clov` in shared memory), ddamg_common.cuh.
+template <typename T, int MODE = LD_STREAM, bool AFMT = false, typename S>
 __device__ __forceinline__ void clover_site_mul(const T* __restrict__ clov, int Vh, int cb,
                                                 const S (&v)[24], S (&out)[24], T c0 = 0)
 {
     T c[36];
-    if (AFMT) load_clover_A<T, STREAM>(clov, Vh, cb, 0, c0, c);
-    else load_clover_block<T, STREAM>(clov, Vh, cb, 0, c);
+    if (AFMT) load_clover_A<T, MODE>(clov, Vh, cb, 0, c0, c);
+    else load_clover_block<T, MODE>(clov, Vh, cb, 0, c);
     clover_block_mul(c, &v[0], &out[0]);
-    if (AFMT) load_clover_A<T, STREAM>(clov, Vh, cb, 1, c0, c);
-    else load_clover_block<T, STREAM>(clov, Vh, cb, 1, c);
+    if (AFMT) load_clover_A<T, MODE>(clov, Vh, cb, 1, c0, c);
+    else load_clover_block<T, MODE>(clov, Vh, cb, 1, c);
     clover_block_mul(c, &v[12], &out[12]);
 }
 

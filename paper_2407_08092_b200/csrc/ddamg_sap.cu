@@ -175,8 +175,16 @@ __device__ __forceinline__ void hop_block(const SapGeom& sg, int lcb, const LSit
 #ifndef DDAMG_SAP_B4_SPECIALISE
 #define DDAMG_SAP_B4_SPECIALISE 1
 #endif
-template <typename T, int RECON, int MAXT, bool B4>
-__global__ void __launch_bounds__(MAXT, MAXT == 128 ? (RECON == 12 && sizeof(T) == 4 ? 3 : 2) : 1)
+#ifndef DDAMG_SAP_STAGE_CLOVER
+#define DDAMG_SAP_STAGE_CLOVER 1
+#endif
+// CS (fp32, two-row links, 4^4 blocks: the default case): the 6x6 blocks of the coming half step are staged in
+// shared memory as well -- one TMA bulk copy (A_oo^-1: 36.9 KB, compact A_ee: 28.7 KB) issued at the start of the
+// half step by one thread, which completes behind the hopping sum; the half step's 6x6 multiplies then read
+// shared memory instead of waiting for L2 / HBM (the dominant stall of the kernel without it).  111.5 KB per CTA:
+// 2 CTAs per SM instead of 3.
+template <typename T, int RECON, int MAXT, bool B4, bool CS>
+__global__ void __launch_bounds__(MAXT, MAXT == 128 ? (RECON == 12 && sizeof(T) == 4 && !CS ? 3 : 2) : 1)
 sap_block_kernel(const SapArgs<T> a)
 {
     extern __shared__ __align__(16) unsigned char sap_smem[];
@@ -190,7 +198,8 @@ sap_block_kernel(const SapArgs<T> a)
     T* links = reinterpret_cast<T*>(sap_smem);                 // [parity][mu][RECON * n]
     T* S_e = links + 2 * 4 * RECON * n;                        // even-site half-block spinor
     T* S_o = S_e + 24 * n;                                     // odd-site half-block spinor
-    double* red = reinterpret_cast<double*>(S_o + 24 * n);     // [warp][3]
+    T* C = S_o + 24 * n;                                       // CS: the staged 6x6 blocks of one parity (72 n reals)
+    double* red = reinterpret_cast<double*>(C + (CS ? 72 * n : 0));    // [warp][3]
     const int tid = threadIdx.x;
     const bool active = tid < n;
     const int lane = tid & 31, warp = tid >> 5, nwarps = (blockDim.x + 31) >> 5;
@@ -222,33 +231,52 @@ sap_block_kernel(const SapArgs<T> a)
     // shared-memory layout, so this is ONE contiguous bulk copy (TMA engine, `cp.async.bulk`, SASS UBLKCP)
     // issued by one thread and tracked by an mbarrier; it runs behind the prologue's own global loads
     // instead of in front of them, and no thread spends instructions or registers on it.
-    unsigned long long* bar = reinterpret_cast<unsigned long long*>(red + 3 * 32);
+    unsigned long long* bar = reinterpret_cast<unsigned long long*>(red + 3 * 32);     // [0]: links (+ first blocks), [1]: 6x6 blocks
     const unsigned bar_s = (unsigned)__cvta_generic_to_shared(bar);
+    const unsigned C_s = (unsigned)__cvta_generic_to_shared(C);
     if (tid == 0) {
         const unsigned bytes = (unsigned)(2 * sblk * sizeof(T));
+        const unsigned cbytes = CS ? (unsigned)(72 * n * sizeof(T)) : 0u;
         const unsigned dst_s = (unsigned)__cvta_generic_to_shared(links);
         const T* src = a.blk_links + bid * 2 * sblk;
         asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar_s));
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar_s + 8));
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar_s), "r"(bytes) : "memory");
+        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar_s), "r"(bytes + cbytes) : "memory");
+        if (CS)                                                // A_oo^-1 first: the prologue needs it before the links
+            asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                         ::"r"(C_s), "l"(clov_oinv), "r"(cbytes), "r"(bar_s) : "memory");
         asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                      ::"r"(dst_s), "l"(src), "r"(bytes), "r"(bar_s) : "memory");
     }
-    if (active) {
-        // ---- eq. 2 right factor, odd half: t_o = A_oo^-1 r_o;  rho starts as r_e
-        T v[24], t[24];
-        load_spinor<T, false>(a.r_o, a.g.Vh, cbg[1], v);
-        clover_site_mul<T, false>(clov_oinv, n, tid, v, t);
-        sts_spinor<T>(S_o, n, tid, t);
-        load_spinor<T, true>(a.r_e, a.g.Vh, cbg[0], rho);
-    }
-    __syncthreads();                                           // S_o complete; the barrier's init is visible
-    {
-        // wait for the links (phase 0 of the mbarrier)
+    auto wait_bar = [&](unsigned addr, unsigned parity) {
         unsigned done = 0;
         while (!done)
-            asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], 0; selp.u32 %0, 1, 0, p; }"
-                         : "=r"(done) : "r"(bar_s) : "memory");
+            asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+                         : "=r"(done) : "r"(addr), "r"(parity) : "memory");
+    };
+    if (CS) {
+        __syncthreads();                                       // the barriers' init is visible
+        T v[24], t[24];
+        if (active) load_spinor<T, false>(a.r_o, a.g.Vh, cbg[1], v);
+        wait_bar(bar_s, 0);                                    // links and A_oo^-1 have landed
+        if (active) {
+            clover_site_mul<T, LD_PLAIN>(C, n, tid, v, t);
+            sts_spinor<T>(S_o, n, tid, t);
+            load_spinor<T, true>(a.r_e, a.g.Vh, cbg[0], rho);
+        }
+        __syncthreads();
+    } else {
+        if (active) {
+            // ---- eq. 2 right factor, odd half: t_o = A_oo^-1 r_o;  rho starts as r_e
+            T v[24], t[24];
+            load_spinor<T, false>(a.r_o, a.g.Vh, cbg[1], v);
+            clover_site_mul<T, false>(clov_oinv, n, tid, v, t);
+            sts_spinor<T>(S_o, n, tid, t);
+            load_spinor<T, true>(a.r_e, a.g.Vh, cbg[0], rho);
+        }
+        __syncthreads();                                       // S_o complete; the barrier's init is visible
+        wait_bar(bar_s, 0);                                    // wait for the links (phase 0 of the mbarrier)
     }
 
     // ---- the block solve as 2m+2 half steps, one copy of the block hopping code:
@@ -260,9 +288,19 @@ sap_block_kernel(const SapArgs<T> a)
 #pragma unroll 1
     for (int hs = 0; hs <= last; ++hs) {
         const int par = hs & 1;
+        if (CS && hs >= 2 && tid == 0) {
+            // the 6x6 blocks of this half step (hs = 1 still finds the prologue's A_oo^-1): every thread has passed
+            // the barrier that ended the previous half step, so the buffer is free; completion k = hs - 2 of bar[1]
+            const unsigned cbytes = (unsigned)((par ? 72 : 2 * CLOVA_REALS) * n * sizeof(T));
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar_s + 8), "r"(cbytes) : "memory");
+            asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                         ::"r"(C_s), "l"(par ? clov_oinv : clov_e), "r"(cbytes), "r"(bar_s + 8) : "memory");
+        }
         T acc[24];
         if (active)
             hop_block<T, RECON>(sg, tid, ls[par], par ? S_e : S_o, links + par * sblk, links + (1 - par) * sblk, acc);
+        if (CS && hs >= 2) wait_bar(bar_s + 8, (unsigned)par);
         if (par) {
             if (active) {
                 T v[24], t[24];
@@ -274,7 +312,8 @@ sap_block_kernel(const SapArgs<T> a)
 #pragma unroll
                     for (int i = 0; i < 24; ++i) v[i] = (T)(-0.5) * acc[i];              // H rho
                 }
-                clover_site_mul<T, false>(clov_oinv, n, tid, v, t);
+                if (CS) clover_site_mul<T, LD_PLAIN>(C, n, tid, v, t);
+                else clover_site_mul<T, false>(clov_oinv, n, tid, v, t);
                 if (hs == last) {
                     load_spinor<T, true>(a.x_o, a.g.Vh, cbg[1], v);
 #pragma unroll
@@ -308,7 +347,8 @@ sap_block_kernel(const SapArgs<T> a)
             T q[24];
             double nr = 0.0, ni = 0.0, dd = 0.0;
             if (active) {
-                clover_site_mul<T, false, true>(clov_e, n, tid, rho, q, a.c0);
+                if (CS) clover_site_mul<T, LD_PLAIN, true>(C, n, tid, rho, q, a.c0);
+                else clover_site_mul<T, false, true>(clov_e, n, tid, rho, q, a.c0);
 #pragma unroll
                 for (int i = 0; i < 24; ++i) q[i] = q[i] + (T)0.5 * acc[i];
                 // <q, rho> = q^H rho and <q, q>, this site's share: the 12 complex products of the site in the
@@ -419,17 +459,23 @@ void launch_sap_reorder(const Geom& g, const SapGeom& sg, int recon, const void*
 template void launch_sap_reorder<float>(const Geom&, const SapGeom&, int, const void*, const void*, const void*, void*, void*, cudaStream_t);
 template void launch_sap_reorder<double>(const Geom&, const SapGeom&, int, const void*, const void*, const void*, void*, void*, cudaStream_t);
 
+// fp32 blocks of 4^4 sites with two-row links also stage the 6x6 blocks of one parity (sap_block_kernel<.., CS>)
+static bool sap_stages_clover(const SapGeom& sg, size_t real_bytes, int recon)
+{
+    return DDAMG_SAP_STAGE_CLOVER && real_bytes == 4 && recon == 12 && sg.B[0] == 4 && sg.B[1] == 4 && sg.B[2] == 4 && sg.B[3] == 4;
+}
 size_t sap_smem_bytes(const SapGeom& sg, size_t real_bytes, int recon)
 {
-    return (size_t)(2 * 4 * recon + 48) * sg.Vbh * real_bytes + (size_t)32 * 3 * sizeof(double) + 16;    // + the mbarrier of the link copy
+    return (size_t)(2 * 4 * recon + 48 + (sap_stages_clover(sg, real_bytes, recon) ? 72 : 0)) * sg.Vbh * real_bytes +
+           (size_t)32 * 3 * sizeof(double) + 16;               // + the two mbarriers of the bulk copies
 }
 
-template <typename T, int RECON, int MAXT, bool B4>
+template <typename T, int RECON, int MAXT, bool B4, bool CS = false>
 static cudaError_t launch_blocks_as(const SapArgs<T>& a, int threads, int grid, size_t smem, cudaStream_t st)
 {
-    cudaError_t e = cudaFuncSetAttribute(sap_block_kernel<T, RECON, MAXT, B4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = cudaFuncSetAttribute(sap_block_kernel<T, RECON, MAXT, B4, CS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    sap_block_kernel<T, RECON, MAXT, B4><<<grid, threads, smem, st>>>(a);
+    sap_block_kernel<T, RECON, MAXT, B4, CS><<<grid, threads, smem, st>>>(a);
     return cudaSuccess;
 }
 
@@ -447,6 +493,9 @@ cudaError_t launch_sap_blocks(const Geom& g, const SapGeom& sg, int recon, doubl
     const int threads = (sg.Vbh + 31) / 32 * 32;
     const int grid = sg.nbxh * sg.nb[1] * sg.nb[2] * sg.nb[3];
     const bool b4 = DDAMG_SAP_B4_SPECIALISE && sg.B[0] == 4 && sg.B[1] == 4 && sg.B[2] == 4 && sg.B[3] == 4;
+    if constexpr (sizeof(T) == 4) {
+        if (b4 && sap_stages_clover(sg, sizeof(T), recon)) return launch_blocks_as<T, 12, 128, true, true>(a, threads, grid, smem, st);
+    }
     if (b4)
         return recon == 12 ? launch_blocks_as<T, 12, 128, true>(a, threads, grid, smem, st)
                            : launch_blocks_as<T, 18, 128, true>(a, threads, grid, smem, st);
