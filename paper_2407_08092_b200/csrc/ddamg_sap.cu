@@ -17,7 +17,9 @@
 // and odd site i of the block (all lanes busy in both half steps); the block's links (the only
 // operand re-used by all 2m+3 hopping applications) are staged ONCE in shared memory (one TMA bulk copy), the two
 // exchanged half-block spinors live in shared memory, e and rho stay in registers, the 6x6
-// clover blocks are re-read through L1/L2 (65 KB per 4^4 block with A_ee in its compact form: L2-resident).  All dot
+// clover blocks are re-read through L1/L2 (65 KB per 4^4 block with A_ee in its compact form: L2-resident) or,
+// in the default case (fp32, two-row links, 4^4 blocks: template flag CS), staged in shared memory by one TMA
+// bulk copy per half step that lands behind the hopping sum.  All dot
 // products are block-local: one CTA-wide fp64 reduction per MR iteration, no
 // global reduction, no host involvement.
 //
