@@ -54,9 +54,6 @@ __device__ __forceinline__ double block_sum(double v)
 #ifndef DDAMG_MAXREG_B
 #define DDAMG_MAXREG_B 128
 #endif
-#ifndef DDAMG_TMA_CLOVER
-#define DDAMG_TMA_CLOVER 0
-#endif
 #ifndef DDAMG_MAXREG_BATCH
 #define DDAMG_MAXREG_BATCH 128     // multi-rhs kernels
 #endif
@@ -98,52 +95,6 @@ dslash_kernel(const DslashArgs<T> a)
     const int Vs = a.g.Vh * units;         // vectors per spinor plane
     const int sv = cb * units + rr;        // this thread's vector index in a spinor plane (== tid)
     double nrm[2] = { 0.0, 0.0 };
-#if DDAMG_TMA_CLOVER
-    // single rhs, fp32: the CTA's 6x6 blocks (the epilogue's operand, 36.9 KB packed inverses / 28.7 KB compact
-    // blocks) are brought into shared memory by TMA bulk copies issued at kernel entry, one per 16-byte plane
-    // (2 KB runs), and land behind the hopping sum: no registers wait for them during the hops
-    constexpr bool TMA_CLOV = !BATCH && sizeof(T) == 4 && EPI != EPI_RHS_MINUS_HOP;
-    constexpr bool AF = EPI >= EPI_SCHUR;
-    constexpr int NPL = AF ? 2 * CLOVA_REALS / 4 : 18;
-    __shared__ __align__(128) float clov_s[TMA_CLOV ? NPL * 4 * DSLASH_THREADS : 4];
-    __shared__ unsigned long long clov_bar;
-    if (TMA_CLOV) {
-        if (threadIdx.x == 0) {
-            const int cb0 = blk * DSLASH_THREADS;
-            const int ns = a.g.Vh - cb0 < DSLASH_THREADS ? a.g.Vh - cb0 : DSLASH_THREADS;
-            const unsigned bar_s = (unsigned)__cvta_generic_to_shared(&clov_bar);
-            const unsigned dst0 = (unsigned)__cvta_generic_to_shared(clov_s);
-            const unsigned bytes = (unsigned)ns * 16u;
-            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar_s));
-            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-            asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar_s), "r"(bytes * NPL) : "memory");
-            const float4* src = reinterpret_cast<const float4*>(a.clov) + cb0;
-#pragma unroll 1
-            for (int k = 0; k < NPL; ++k)
-                asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                             ::"r"(dst0 + (unsigned)k * 16u * DSLASH_THREADS), "l"(src + (size_t)k * a.g.Vh), "r"(bytes), "r"(bar_s) : "memory");
-        }
-        __syncthreads();                   // the barrier's init is visible to the threads that will wait on it
-    }
-    auto clover_mul = [&](const S (&v)[24], S (&out)[24]) {
-        if (TMA_CLOV) {
-            const unsigned bar_s = (unsigned)__cvta_generic_to_shared(&clov_bar);
-            unsigned done = 0;
-            while (!done)
-                asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], 0; selp.u32 %0, 1, 0, p; }"
-                             : "=r"(done) : "r"(bar_s) : "memory");
-            clover_site_mul<T, LD_PLAIN, AF>(reinterpret_cast<const T*>(clov_s), DSLASH_THREADS, (int)threadIdx.x, v, out, a.c0);
-        } else {
-            if (AF) clover_site_mul<T, LD_STREAM, true>(a.clov, a.g.Vh, cb, v, out, a.c0);
-            else clover_site_mul<T>(a.clov, a.g.Vh, cb, v, out);
-        }
-    };
-#else
-    auto clover_mul = [&](const S (&v)[24], S (&out)[24]) {
-        if (EPI >= EPI_SCHUR) clover_site_mul<T, LD_STREAM, true>(a.clov, a.g.Vh, cb, v, out, a.c0);
-        else clover_site_mul<T>(a.clov, a.g.Vh, cb, v, out);
-    };
-#endif
     if (cb < a.g.Vh) {
         const Site s = site_of_cb(a.g, cb, a.parity);
         S acc[24];
@@ -152,13 +103,13 @@ dslash_kernel(const DslashArgs<T> a)
         if (EPI == EPI_CLOV_HOP) {
 #pragma unroll
             for (int i = 0; i < 24; ++i) acc[i] = vmul((T)(-0.5), acc[i]);
-            clover_mul(acc, res);
+            clover_site_mul<T>(a.clov, a.g.Vh, cb, acc, res);
         } else if (EPI == EPI_CLOV_RHS_MINUS_HOP) {
             S b[24];
             load_spinor<T, true>(a.rhs, Vs, sv, b);
 #pragma unroll
             for (int i = 0; i < 24; ++i) acc[i] = vfma((T)0.5, acc[i], b[i]);
-            clover_mul(acc, res);
+            clover_site_mul<T>(a.clov, a.g.Vh, cb, acc, res);
         } else if (EPI == EPI_RHS_MINUS_HOP) {
             S b[24];
             load_spinor<T, true>(a.rhs, Vs, sv, b);
@@ -167,7 +118,7 @@ dslash_kernel(const DslashArgs<T> a)
         } else {
             S x[24], ax[24];
             load_spinor<T, true>(a.own, Vs, sv, x);
-            clover_mul(x, ax);
+            clover_site_mul<T, LD_STREAM, true>(a.clov, a.g.Vh, cb, x, ax, a.c0);
             // H = -1/2 acc:  Schur forms subtract H t (+1/2 acc), the full operator adds H x (-1/2 acc)
             constexpr bool FULL = (EPI == EPI_FULL || EPI == EPI_FULL_RESIDUAL);
             const T hs = FULL ? (T)(-0.5) : (T)0.5;

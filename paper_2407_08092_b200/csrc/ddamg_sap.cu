@@ -273,7 +273,7 @@ sap_block_kernel(const SapArgs<T> a)
             // ---- eq. 2 right factor, odd half: t_o = A_oo^-1 r_o;  rho starts as r_e
             T v[24], t[24];
             load_spinor<T, false>(a.r_o, a.g.Vh, cbg[1], v);
-            clover_site_mul<T, false>(clov_oinv, n, tid, v, t);
+            clover_site_mul<T, LD_REUSE>(clov_oinv, n, tid, v, t);
             sts_spinor<T>(S_o, n, tid, t);
             load_spinor<T, true>(a.r_e, a.g.Vh, cbg[0], rho);
         }
@@ -315,7 +315,7 @@ sap_block_kernel(const SapArgs<T> a)
                     for (int i = 0; i < 24; ++i) v[i] = (T)(-0.5) * acc[i];              // H rho
                 }
                 if (CS) clover_site_mul<T, LD_PLAIN>(C, n, tid, v, t);
-                else clover_site_mul<T, false>(clov_oinv, n, tid, v, t);
+                else clover_site_mul<T, LD_REUSE>(clov_oinv, n, tid, v, t);
                 if (hs == last) {
                     load_spinor<T, true>(a.x_o, a.g.Vh, cbg[1], v);
 #pragma unroll
@@ -350,7 +350,7 @@ sap_block_kernel(const SapArgs<T> a)
             double nr = 0.0, ni = 0.0, dd = 0.0;
             if (active) {
                 if (CS) clover_site_mul<T, LD_PLAIN, true>(C, n, tid, rho, q, a.c0);
-                else clover_site_mul<T, false, true>(clov_e, n, tid, rho, q, a.c0);
+                else clover_site_mul<T, LD_REUSE, true>(clov_e, n, tid, rho, q, a.c0);
 #pragma unroll
                 for (int i = 0; i < 24; ++i) q[i] = q[i] + (T)0.5 * acc[i];
                 // <q, rho> = q^H rho and <q, q>, this site's share: the 12 complex products of the site in the
@@ -430,7 +430,7 @@ __global__ void sap_reorder_kernel(Geom g, SapGeom sg, const T* __restrict__ gau
         for (int b = 0; b < 2; ++b) {
             T c[36];
             if (p) {
-                load_clover_block<T, true>(src, g.Vh, cbg, b, c);
+                load_clover_block<T, LD_STREAM>(src, g.Vh, cbg, b, c);
                 store_clover_block<T>(blk_clov + (bid * 2 + p) * 72 * n, n, i, b, c);
             } else {
                 // A_ee stays in the compact form (CLOVA_REALS per block): a plain copy of its vectors
