@@ -218,7 +218,8 @@ int ddamg_prepare_rhs(ddamg_ctx* ctx, const void* b_e, const void* b_o, void* bh
  */
 int ddamg_power_iteration(ddamg_ctx* ctx, void* v_e, int iters, double* lambda_max);
 
-/* natural (DEVICE, context precision, full lattice) -> native halves.  x_e or x_o may be NULL. */
+/* natural (DEVICE, context precision, full lattice, 16-byte aligned: EINVAL otherwise) -> native halves.
+ * x_e or x_o may be NULL. */
 int ddamg_pack_spinor(ddamg_ctx* ctx, const void* nat, void* x_e, void* x_o);
 /* native halves -> natural (DEVICE).  A NULL half writes zeros on that parity. */
 int ddamg_unpack_spinor(ddamg_ctx* ctx, const void* x_e, const void* x_o, void* nat);

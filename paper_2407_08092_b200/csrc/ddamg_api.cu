@@ -3,6 +3,7 @@
 // Host orchestration only: every arithmetic step of the path runs in the kernels of
 // ddamg_dslash.cu / ddamg_setup.cu / ddamg_blas.cu.  Nothing here touches spinor data on the
 // host, and there is no CPU fallback.
+#include <cstdint>
 #include <cstdio>
 #include <cstring>
 #include <new>
@@ -365,6 +366,7 @@ extern "C" int ddamg_pack_spinor(ddamg_ctx* ctx, const void* nat, void* x_e, voi
 {
     ENTER(ctx);
     if (!nat || (!x_e && !x_o)) return fail(ctx, DDAMG_EINVAL, "ddamg_pack_spinor: NULL argument");
+    if (((uintptr_t)nat & 15) != 0) return fail(ctx, DDAMG_EINVAL, "ddamg_pack_spinor: nat must be 16-byte aligned");
     if (ctx->prec == DDAMG_F32) launch_pack_spinor<float>(ctx->g, nat, x_e, x_o, ctx->stream);
     else launch_pack_spinor<double>(ctx->g, nat, x_e, x_o, ctx->stream);
     return after_launch(ctx);
@@ -374,6 +376,7 @@ extern "C" int ddamg_unpack_spinor(ddamg_ctx* ctx, const void* x_e, const void* 
 {
     ENTER(ctx);
     if (!nat) return fail(ctx, DDAMG_EINVAL, "ddamg_unpack_spinor: nat is NULL");
+    if (((uintptr_t)nat & 15) != 0) return fail(ctx, DDAMG_EINVAL, "ddamg_unpack_spinor: nat must be 16-byte aligned");
     if (ctx->prec == DDAMG_F32) launch_unpack_spinor<float>(ctx->g, x_e, x_o, nat, ctx->stream);
     else launch_unpack_spinor<double>(ctx->g, x_e, x_o, nat, ctx->stream);
     return after_launch(ctx);

@@ -8,6 +8,7 @@
 //   A_lower = (m0+4) - (csw/16) sum_k sigma_k (x) i (F'_ij + F'_kt),  (i,j,k) cyclic,
 // with F' = Q - Q^H and Q the sum of the four plaquette leaves.  All arithmetic in fp64;
 // the result is rounded once to the context precision.
+#include <cstdint>
 #include "ddamg_internal.h"
 
 namespace ddamg {
@@ -39,7 +40,9 @@ __device__ __forceinline__ Coord shift(const Geom& g, Coord c, int mu, int d)
 }
 
 // ------------------------------------------------------------------ a0: gauge repack
-template <typename Tin, typename T>
+// VEC: the natural field is 16-byte aligned, so a site's 72 input reals are read as whole 16-byte vectors
+// (18 float4 / 36 double2 / ...) instead of 72 scalars.
+template <typename Tin, typename T, bool VEC>
 __global__ void pack_gauge_kernel(Geom g, int bc, const Tin* __restrict__ U, T* __restrict__ gauge)
 {
     const int idx = blockIdx.x * blockDim.x + threadIdx.x;
@@ -48,12 +51,23 @@ __global__ void pack_gauge_kernel(Geom g, int bc, const Tin* __restrict__ U, T* 
     const Coord c = coord_of(g, cb, parity);
     const size_t n = nat_of(g, c);
     const size_t lblk = (size_t)18 * g.Vh;
+    Tin r[72];
+    if (VEC) {
+        using Vin = typename VecOf<Tin>::type;
+        constexpr int NI = VecOf<Tin>::N;
+        const Vin* src = reinterpret_cast<const Vin*>(U) + n * (72 / NI);
+#pragma unroll
+        for (int k = 0; k < 72 / NI; ++k) unpack(ld_stream(src + k), &r[k * NI]);
+    } else {
+#pragma unroll
+        for (int k = 0; k < 72; ++k) r[k] = U[n * 72 + k];
+    }
 #pragma unroll
     for (int mu = 0; mu < 4; ++mu) {
         T u[18];
         const T sgn = (bc == 1 && mu == 3 && c.x[3] == g.T - 1) ? (T)-1 : (T)1;
 #pragma unroll
-        for (int k = 0; k < 18; ++k) u[k] = sgn * (T)U[(n * 4 + mu) * 18 + k];
+        for (int k = 0; k < 18; ++k) u[k] = sgn * (T)r[18 * mu + k];
         store_link(gauge + ((size_t)parity * 4 + mu) * lblk, g.Vh, cb, u);
     }
 }
@@ -62,7 +76,10 @@ template <typename Tin, typename T>
 void launch_pack_gauge(const Geom& g, int bc, const void* U_nat, void* gauge, cudaStream_t st)
 {
     const int n = 2 * g.Vh;
-    pack_gauge_kernel<Tin, T><<<(n + 255) / 256, 256, 0, st>>>(g, bc, (const Tin*)U_nat, (T*)gauge);
+    if (((uintptr_t)U_nat & 15) == 0)
+        pack_gauge_kernel<Tin, T, true><<<(n + 127) / 128, 128, 0, st>>>(g, bc, (const Tin*)U_nat, (T*)gauge);
+    else
+        pack_gauge_kernel<Tin, T, false><<<(n + 127) / 128, 128, 0, st>>>(g, bc, (const Tin*)U_nat, (T*)gauge);
 }
 template void launch_pack_gauge<float, float>(const Geom&, int, const void*, void*, cudaStream_t);
 template void launch_pack_gauge<double, float>(const Geom&, int, const void*, void*, cudaStream_t);
@@ -117,38 +134,52 @@ template void launch_compress_gauge<float>(const Geom&, int, const void*, void*,
 template void launch_compress_gauge<double>(const Geom&, int, const void*, void*, unsigned int*, cudaStream_t);
 
 // ------------------------------------------------------------------ spinor layout converters
+// A site's 24 reals are 24/N 16-byte vectors in the natural layout as well, and vector k of the site IS plane k of
+// the native layout: both converters move whole vectors (natural side: 6 / 12 accesses of 16 bytes per thread at
+// a 96 / 192-byte stride, all sectors fully used between them; native side: one contiguous run per plane and warp).
 template <typename T>
 __global__ void pack_spinor_kernel(Geom g, const T* __restrict__ nat, T* __restrict__ xe, T* __restrict__ xo)
 {
+    using V = typename VecOf<T>::type;
+    constexpr int NV = 24 / VecOf<T>::N;
     const int idx = blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= 2 * g.Vh) return;
     const int parity = idx / g.Vh, cb = idx % g.Vh;
     T* dst = parity ? xo : xe;
     if (!dst) return;
     const size_t n = nat_of(g, coord_of(g, cb, parity));
-    T s[24];
+    const V* src = reinterpret_cast<const V*>(nat) + n * NV;
+    V v[NV];
 #pragma unroll
-    for (int k = 0; k < 24; ++k) s[k] = nat[n * 24 + k];
-    store_spinor<T>(dst, g.Vh, cb, s);
+    for (int k = 0; k < NV; ++k) v[k] = ld_stream(src + k);
+    V* d = reinterpret_cast<V*>(dst) + cb;
+#pragma unroll
+    for (int k = 0; k < NV; ++k) d[(size_t)k * g.Vh] = v[k];
 }
 
 template <typename T>
 __global__ void unpack_spinor_kernel(Geom g, const T* __restrict__ xe, const T* __restrict__ xo, T* __restrict__ nat)
 {
+    using V = typename VecOf<T>::type;
+    constexpr int NV = 24 / VecOf<T>::N;
     const int idx = blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= 2 * g.Vh) return;
     const int parity = idx / g.Vh, cb = idx % g.Vh;
     const T* src = parity ? xo : xe;
     const size_t n = nat_of(g, coord_of(g, cb, parity));
-    T s[24];
+    V v[NV];
     if (src) {
-        load_spinor<T>(src, g.Vh, cb, s);
+        const V* sp = reinterpret_cast<const V*>(src) + cb;
+#pragma unroll
+        for (int k = 0; k < NV; ++k) v[k] = ld_stream(sp + (size_t)k * g.Vh);
     } else {
+        T z[VecOf<T>::N] = {};
 #pragma unroll
-        for (int k = 0; k < 24; ++k) s[k] = 0;
+        for (int k = 0; k < NV; ++k) v[k] = pack(z);
     }
+    V* d = reinterpret_cast<V*>(nat) + n * NV;
 #pragma unroll
-    for (int k = 0; k < 24; ++k) nat[n * 24 + k] = s[k];
+    for (int k = 0; k < NV; ++k) d[k] = v[k];
 }
 
 template <typename T>
