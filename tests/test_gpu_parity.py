@@ -383,6 +383,11 @@ def test_error_codes():
     with pytest.raises(dd.DdamgError) as e:
         ctx.gmres_oe(x, y, 0, 1)
     assert e.value.status == dd.EINVAL
+    # the layout converters move 16-byte vectors: a natural buffer that is only 8-byte aligned is refused
+    buf = torch.zeros(12 * 256 + 1, dtype=torch.complex64, device="cuda")
+    with pytest.raises(dd.DdamgError) as e:
+        ctx.pack(buf[1:])
+    assert e.value.status == dd.EINVAL
 
 
 def test_host_and_device_gauge_paths_agree():
