@@ -302,6 +302,10 @@ int ddamg_get_clover(ddamg_ctx* ctx, void* A_nat, void* Ainv_nat);
  *                     link format change).  Auto = on for lattices up to 2^19 sites per parity,
  *                     where the kernels are short enough for launch gaps to show.  Same kernels,
  *                     same order: bit-identical results.  Off while ddamg_kernel_timing is on.
+ *   "sap_blocked"     1 (default) or 0.  ddamg_sap keeps its residual and update vectors block-ordered
+ *                     (contiguous per domain-decomposition block) instead of in the native half-spinor
+ *                     layout; same arithmetic per site, results identical up to the summation order of
+ *                     the residual-history norms.
  * EINVAL for an unknown name or a bad value.
  */
 int ddamg_set_option(ddamg_ctx* ctx, const char* name, double value);

@@ -48,6 +48,7 @@ struct ddamg_ctx {
     int sap_built[4];           // block extents the two copies were built for ({0,..} = stale)
     int sap_built_recon;        // link format (18 / 12 reals) of the block-ordered link copy
     void* sap_e;                // SAP: the update e of the last solved colour, even half then odd half
+    int sap_blocked;            // SAP keeps r and e block-ordered (option "sap_blocked", default 1)
     int sap_block[4];           // SAP block extents used when SAP is the FGMRES smoother (options "sap_block_x".."_t")
     // CUDA-graph replay of a history-free Richardson call (option "cuda_graph"): the 2 nu launches are captured
     // once on cap_stream (nothing ever executes there) and replayed on the context's stream
@@ -232,6 +233,7 @@ extern "C" int ddamg_create(ddamg_ctx** out, int L, int T, double csw, double m0
     ctx->clov_oo = nullptr; ctx->sc2 = nullptr; ctx->fgm_basis = nullptr; ctx->fgm_cap = 0;
     ctx->tmp_batch = nullptr; ctx->partials_batch = nullptr; ctx->batch_cap = 0; ctx->batch_l2_bytes = 40e6;
     for (int mu = 0; mu < 4; ++mu) ctx->sap_block[mu] = 4;
+    ctx->sap_blocked = 1;
     ctx->sap_links = ctx->sap_clov = ctx->sap_e = nullptr; ctx->sap_built_recon = 0;
     for (int mu = 0; mu < 4; ++mu) ctx->sap_built[mu] = 0;
     ctx->partials = nullptr; ctx->sc = nullptr; ctx->host_hist = nullptr; ctx->singular = nullptr;
@@ -1241,6 +1243,9 @@ extern "C" int ddamg_sap(ddamg_ctx* ctx, const void* b_e, const void* b_o, void*
     void* r_o = ctx->tmp_o;
     void* e_e = ctx->sap_e;
     void* e_o = ctx->sap_e ? (char*)ctx->sap_e + ctx->half_bytes : nullptr;
+    // r and e are BLOCK-ORDERED (ddamg_sap.cu): every launch touches the blocks of one colour, which in the native
+    // layout are every other 32-byte sector.  (Option "sap_blocked" = 0 keeps them native.)
+    const int blocked = ctx->sap_blocked;
     // ||r|| of the maintained residual -> history
     auto append_norm = [&]() -> int {
         const int n1 = f32 ? launch_copy_norm<float>(ctx->nreal, r_e, r_e, ctx->partials, st)
@@ -1255,17 +1260,27 @@ extern "C" int ddamg_sap(ddamg_ctx* ctx, const void* b_e, const void* b_o, void*
         {
             KernelTimer kt(ctx, KT_SAP);
             cudaError_t e = f32
-                ? launch_sap_blocks<float>(ctx->g, sg, recon, ctx->m0 + 4.0, colour, m, ctx->sap_links, ctx->sap_clov, rin_e, rin_o, r_e, r_o, e_e, e_o, x_e, x_o, st)
-                : launch_sap_blocks<double>(ctx->g, sg, recon, ctx->m0 + 4.0, colour, m, ctx->sap_links, ctx->sap_clov, rin_e, rin_o, r_e, r_o, e_e, e_o, x_e, x_o, st);
+                ? launch_sap_blocks<float>(ctx->g, sg, recon, ctx->m0 + 4.0, colour, m, ctx->sap_links, ctx->sap_clov, rin_e, rin_o, r_e, r_o, e_e, e_o, x_e, x_o, blocked, st)
+                : launch_sap_blocks<double>(ctx->g, sg, recon, ctx->m0 + 4.0, colour, m, ctx->sap_links, ctx->sap_clov, rin_e, rin_o, r_e, r_o, e_e, e_o, x_e, x_o, blocked, st);
             if (e != cudaSuccess) return check_cuda(ctx, e, "sap_block_kernel attributes");
         }
         int q = after_launch(ctx);
         if (q != DDAMG_OK || !update_other) return q;
         {
             KernelTimer kt(ctx, KT_FULL);
-            if (f32) launch_sap_boundary<float>(ctx->g, sg, recon, 1 - colour, ctx->bc == 1, hop_gauge_block(ctx, 0), e_e, e_o, rin_e, rin_o, r_e, r_o, st);
-            else launch_sap_boundary<double>(ctx->g, sg, recon, 1 - colour, ctx->bc == 1, hop_gauge_block(ctx, 0), e_e, e_o, rin_e, rin_o, r_e, r_o, st);
+            if (blocked) {
+                if (f32) launch_sap_boundary_blocked<float>(ctx->g, sg, recon, 1 - colour, ctx->bc == 1, ctx->sap_links, e_e, e_o, r_e, r_o, st);
+                else launch_sap_boundary_blocked<double>(ctx->g, sg, recon, 1 - colour, ctx->bc == 1, ctx->sap_links, e_e, e_o, r_e, r_o, st);
+            } else {
+                if (f32) launch_sap_boundary<float>(ctx->g, sg, recon, 1 - colour, ctx->bc == 1, hop_gauge_block(ctx, 0), e_e, e_o, rin_e, rin_o, r_e, r_o, st);
+                else launch_sap_boundary<double>(ctx->g, sg, recon, 1 - colour, ctx->bc == 1, hop_gauge_block(ctx, 0), e_e, e_o, rin_e, rin_o, r_e, r_o, st);
+            }
         }
+        return after_launch(ctx);
+    };
+    auto to_blocked = [&](const void* s_e, const void* s_o) -> int {
+        if (f32) launch_sap_spinor_to_blocked<float>(ctx->g, sg, s_e, s_o, r_e, r_o, st);
+        else launch_sap_spinor_to_blocked<double>(ctx->g, sg, s_e, s_o, r_e, r_o, st);
         return after_launch(ctx);
     };
     if (m == 0 || n == 0) {
@@ -1280,16 +1295,25 @@ extern "C" int ddamg_sap(ddamg_ctx* ctx, const void* b_e, const void* b_o, void*
         }
         return DDAMG_OK;
     }
-    // Alg. 1 line 2, first iteration: r = b - D x, evaluated in full once (x = 0: r = b itself, read in place --
-    // the smoother use); afterwards every block solve and boundary pass keeps r current
+    // Alg. 1 line 2, first iteration: r = b - D x, evaluated in full once (x = 0: r = b itself -- the smoother use,
+    // PAPER.md:55); afterwards every block solve and boundary pass keeps r current
     const void* rin_e = b_e;
     const void* rin_o = b_o;
     if (!zero_init) {
-        s = dslash(ctx, EPI_FULL_RESIDUAL, hist, 0, x_o, x_e, b_e, r_e, 0.0, 5);
+        // blocked: the residual is formed in the (still unused) e arrays and re-ordered into r
+        void* t_e = blocked ? e_e : r_e;
+        void* t_o = blocked ? e_o : r_o;
+        s = dslash(ctx, EPI_FULL_RESIDUAL, hist, 0, x_o, x_e, b_e, t_e, 0.0, 5);
         if (s != DDAMG_OK) return s;
-        s = dslash(ctx, EPI_FULL_RESIDUAL, hist, 1, x_e, x_o, b_o, r_o, 0.0, 5, 0, (size_t)dgrid, ctx->clov_oo);
+        s = dslash(ctx, EPI_FULL_RESIDUAL, hist, 1, x_e, x_o, b_o, t_o, 0.0, 5, 0, (size_t)dgrid, ctx->clov_oo);
         if (s != DDAMG_OK) return s;
         if (hist) { launch_finalize_norm(ctx->partials, 2 * dgrid, ctx->sc, 1, st); s = after_launch(ctx); if (s != DDAMG_OK) return s; }
+        if (blocked) { s = to_blocked(t_e, t_o); if (s != DDAMG_OK) return s; }
+        rin_e = r_e; rin_o = r_o;
+    } else if (blocked) {
+        s = to_blocked(b_e, b_o);                                                      // r = b, block-ordered
+        if (s != DDAMG_OK) return s;
+        if (hist) { s = append_norm(); if (s != DDAMG_OK) return s; }                  // ||b||
         rin_e = r_e; rin_o = r_o;
     } else if (hist) {
         // ||b||: reduce b without touching it
@@ -1360,6 +1384,11 @@ extern "C" int ddamg_set_option(ddamg_ctx* ctx, const char* name, double value)
     if (strcmp(name, "cuda_graph") == 0) {
         if (value != 0.0 && value != 1.0 && value != -1.0) return fail(ctx, DDAMG_EINVAL, "ddamg_set_option: cuda_graph must be 0, 1 or -1 (auto)");
         ctx->graph_mode = (int)value;
+        return DDAMG_OK;
+    }
+    if (strcmp(name, "sap_blocked") == 0) {
+        if (value != 0.0 && value != 1.0) return fail(ctx, DDAMG_EINVAL, "ddamg_set_option: sap_blocked must be 0 or 1");
+        ctx->sap_blocked = (int)value;
         return DDAMG_OK;
     }
     if (strcmp(name, "gauge_recon") == 0) {

@@ -53,6 +53,8 @@ struct SapArgs {
     T* e_o;
     T* x_e;                  // iterate, updated in place on the blocks of this colour
     T* x_o;
+    int blocked;             // r, rn, e are BLOCK-ORDERED arrays ([block][plane][n], one array per parity) instead of
+                             // native half spinors: every access of a block is then a contiguous run per plane
 };
 
 // ---- shared-memory access (plain loads/stores: the read-only global path does not apply)
@@ -228,6 +230,11 @@ sap_block_kernel(const SapArgs<T> a)
             cbg[p] = ((ox + ls[p].lx) >> 1) + a.g.Lh * ((oy + ls[p].ly) + a.g.L * ((oz + ls[p].lz) + a.g.L * (ot + ls[p].lt)));
         }
     }
+    // where this thread's even / odd site lives in r, rn, e: native (checkerboard index, plane stride V/2) or
+    // block-ordered (local index, plane stride n, block offset 24 n reals)
+    const int rstr = a.blocked ? n : a.g.Vh;
+    const int ri[2] = { a.blocked ? tid : cbg[0], a.blocked ? tid : cbg[1] };
+    const size_t roff = a.blocked ? bid * 24 * n : 0;
     const int sblk = 4 * RECON * n;                            // one parity's four link blocks in shared memory
     // ---- stage the block's links (read once from HBM per launch): the block-ordered copy has the
     // shared-memory layout, so this is ONE contiguous bulk copy (TMA engine, `cp.async.bulk`, SASS UBLKCP)
@@ -260,22 +267,22 @@ sap_block_kernel(const SapArgs<T> a)
     if (CS) {
         __syncthreads();                                       // the barriers' init is visible
         T v[24], t[24];
-        if (active) load_spinor<T, false>(a.r_o, a.g.Vh, cbg[1], v);
+        if (active) load_spinor<T, false>(a.r_o + roff, rstr, ri[1], v);
         wait_bar(bar_s, 0);                                    // links and A_oo^-1 have landed
         if (active) {
             clover_site_mul<T, LD_PLAIN>(C, n, tid, v, t);
             sts_spinor<T>(S_o, n, tid, t);
-            load_spinor<T, true>(a.r_e, a.g.Vh, cbg[0], rho);
+            load_spinor<T, true>(a.r_e + roff, rstr, ri[0], rho);
         }
         __syncthreads();
     } else {
         if (active) {
             // ---- eq. 2 right factor, odd half: t_o = A_oo^-1 r_o;  rho starts as r_e
             T v[24], t[24];
-            load_spinor<T, false>(a.r_o, a.g.Vh, cbg[1], v);
+            load_spinor<T, false>(a.r_o + roff, rstr, ri[1], v);
             clover_site_mul<T, LD_REUSE>(clov_oinv, n, tid, v, t);
             sts_spinor<T>(S_o, n, tid, t);
-            load_spinor<T, true>(a.r_e, a.g.Vh, cbg[0], rho);
+            load_spinor<T, true>(a.r_e + roff, rstr, ri[0], rho);
         }
         __syncthreads();                                       // S_o complete; the barrier's init is visible
         wait_bar(bar_s, 0);                                    // wait for the links (phase 0 of the mbarrier)
@@ -307,7 +314,7 @@ sap_block_kernel(const SapArgs<T> a)
             if (active) {
                 T v[24], t[24];
                 if (hs == last) {
-                    load_spinor<T, false>(a.r_o, a.g.Vh, cbg[1], v);
+                    load_spinor<T, false>(a.r_o + roff, rstr, ri[1], v);
 #pragma unroll
                     for (int i = 0; i < 24; ++i) v[i] = v[i] + (T)0.5 * acc[i];          // r_o - H e
                 } else {
@@ -326,12 +333,12 @@ sap_block_kernel(const SapArgs<T> a)
                     for (int i = 0; i < 24; ++i) v[i] += e[i];
                     store_spinor<T>(a.x_e, a.g.Vh, cbg[0], v);
                     // the update and the residual it leaves on this block: r_k - D_k e_k = (rho, 0)
-                    store_spinor<T>(a.e_o, a.g.Vh, cbg[1], t);
-                    store_spinor<T>(a.e_e, a.g.Vh, cbg[0], e);
-                    store_spinor<T>(a.rn_e, a.g.Vh, cbg[0], rho);
+                    store_spinor<T>(a.e_o + roff, rstr, ri[1], t);
+                    store_spinor<T>(a.e_e + roff, rstr, ri[0], e);
+                    store_spinor<T>(a.rn_e + roff, rstr, ri[0], rho);
 #pragma unroll
                     for (int i = 0; i < 24; ++i) v[i] = 0;
-                    store_spinor<T>(a.rn_o, a.g.Vh, cbg[1], v);
+                    store_spinor<T>(a.rn_o + roff, rstr, ri[1], v);
                 } else {
                     sts_spinor<T>(S_o, n, tid, t);
                 }
@@ -484,9 +491,10 @@ static cudaError_t launch_blocks_as(const SapArgs<T>& a, int threads, int grid, 
 template <typename T>
 cudaError_t launch_sap_blocks(const Geom& g, const SapGeom& sg, int recon, double c0, int colour, int m, const void* blk_links,
                               const void* blk_clov, const void* r_e, const void* r_o, void* rn_e, void* rn_o,
-                              void* e_e, void* e_o, void* x_e, void* x_o, cudaStream_t st)
+                              void* e_e, void* e_o, void* x_e, void* x_o, int blocked, cudaStream_t st)
 {
     SapArgs<T> a;
+    a.blocked = blocked;
     a.g = g; a.sg = sg; a.colour = colour; a.m = m; a.c0 = (T)c0;
     a.blk_links = (const T*)blk_links; a.blk_clov = (const T*)blk_clov;
     a.r_e = (const T*)r_e; a.r_o = (const T*)r_o; a.rn_e = (T*)rn_e; a.rn_o = (T*)rn_o;
@@ -508,9 +516,141 @@ cudaError_t launch_sap_blocks(const Geom& g, const SapGeom& sg, int recon, doubl
                        : launch_blocks_as<T, 18, SAP_MAX_THREADS, false>(a, threads, grid, smem, st);
 }
 template cudaError_t launch_sap_blocks<float>(const Geom&, const SapGeom&, int, double, int, int, const void*, const void*,
-                                              const void*, const void*, void*, void*, void*, void*, void*, void*, cudaStream_t);
+                                              const void*, const void*, void*, void*, void*, void*, void*, void*, int, cudaStream_t);
 template cudaError_t launch_sap_blocks<double>(const Geom&, const SapGeom&, int, double, int, int, const void*, const void*,
-                                               const void*, const void*, void*, void*, void*, void*, void*, void*, cudaStream_t);
+                                               const void*, const void*, void*, void*, void*, void*, void*, void*, int, cudaStream_t);
+
+// ---- block-ordered residual and update arrays.  In the checkerboard layout a block owns 2-site (32-byte) x-runs,
+// alternating with the other colour's: a launch that touches the sites of ONE colour uses every other 32-byte
+// sector, i.e. half of each 64-byte DRAM access, and a warp's access to a block is 16 different lines.  r, rn and e
+// are internal to SAP, so they are kept block-ordered instead -- per parity an array [block][24/N planes][n sites]
+// of 16-byte vectors, block = cx + nbx (cy + nby (cz + nbz ct)) -- and every access of a block is one contiguous
+// run per plane.  native -> block-ordered, both parities (Alg. 1 line 2: the first residual):
+template <typename T>
+__global__ void sap_spinor_to_blocked_kernel(Geom g, SapGeom sg, const T* __restrict__ s_e, const T* __restrict__ s_o,
+                                             T* __restrict__ b_e, T* __restrict__ b_o)
+{
+    const int n = sg.Vbh, i = threadIdx.x;
+    if (i >= n) return;
+    int r = blockIdx.x;
+    const int cx = r % sg.nb[0]; r /= sg.nb[0];
+    const int cy = r % sg.nb[1]; r /= sg.nb[1];
+    const int cz = r % sg.nb[2];
+    const int ct = r / sg.nb[2];
+    const size_t off = (size_t)blockIdx.x * 24 * n;
+#pragma unroll 1
+    for (int p = 0; p < 2; ++p) {
+        const LSite ls = lsite_of(sg, i, p);
+        const int cbg = ((cx * sg.B[0] + ls.lx) >> 1) +
+                        g.Lh * ((cy * sg.B[1] + ls.ly) + g.L * ((cz * sg.B[2] + ls.lz) + g.L * (ct * sg.B[3] + ls.lt)));
+        T v[24];
+        load_spinor<T, true>(p ? s_o : s_e, g.Vh, cbg, v);
+        store_spinor<T>((p ? b_o : b_e) + off, n, i, v);
+    }
+}
+template <typename T>
+void launch_sap_spinor_to_blocked(const Geom& g, const SapGeom& sg, const void* s_e, const void* s_o, void* b_e, void* b_o,
+                                  cudaStream_t st)
+{
+    const int threads = (sg.Vbh + 31) / 32 * 32;
+    const int grid = sg.nb[0] * sg.nb[1] * sg.nb[2] * sg.nb[3];
+    sap_spinor_to_blocked_kernel<T><<<grid, threads, 0, st>>>(g, sg, (const T*)s_e, (const T*)s_o, (T*)b_e, (T*)b_o);
+}
+template void launch_sap_spinor_to_blocked<float>(const Geom&, const SapGeom&, const void*, const void*, void*, void*, cudaStream_t);
+template void launch_sap_spinor_to_blocked<double>(const Geom&, const SapGeom&, const void*, const void*, void*, void*, cudaStream_t);
+
+// Incremental residual on block-ordered arrays, in place: for every site x of the blocks of colour `target`
+//   r(x) -= sum over the neighbours y of x in OTHER blocks of H_xy e(y)
+// One CTA per target block, one thread per site (even sites first); sites none of whose hops leaves the block have
+// nothing to do.  Links come from the block-ordered link copy: U_mu(x) is the block's own forward link, U_mu(x - mu)
+// the forward link of the neighbour block's far face.
+template <typename T, int RECON>
+__global__ void __launch_bounds__(2 * SAP_MAX_THREADS)
+sap_boundary_blocked_kernel(Geom g, SapGeom sg, int target, int apbc, const T* __restrict__ blk_links,
+                            const T* __restrict__ e_e, const T* __restrict__ e_o, T* r_e, T* r_o)
+{
+    const int n = sg.Vbh;
+    if ((int)threadIdx.x >= 2 * n) return;
+    int b = blockIdx.x;
+    const int cxh = b % sg.nbxh; b /= sg.nbxh;
+    const int cy = b % sg.nb[1]; b /= sg.nb[1];
+    const int cz = b % sg.nb[2];
+    const int ct = b / sg.nb[2];
+    const int cx = 2 * cxh + ((cy + cz + ct + target) & 1);
+    const int c[4] = { cx, cy, cz, ct };
+    const int parity = (int)threadIdx.x >= n ? 1 : 0;
+    const int lcb = (int)threadIdx.x - parity * n;
+    const LSite ls = lsite_of(sg, lcb, parity);
+    const int l[4] = { ls.lx, ls.ly, ls.lz, ls.lt };
+    bool any = false;
+#pragma unroll
+    for (int mu = 0; mu < 4; ++mu) any = any || l[mu] == 0 || l[mu] == sg.B[mu] - 1;
+    if (!any) return;
+    const size_t bid = (size_t)cx + (size_t)sg.nb[0] * (cy + (size_t)sg.nb[1] * (cz + (size_t)sg.nb[2] * ct));
+    const T* e_in = parity ? e_e : e_o;                        // neighbours have the opposite parity
+    T acc[24], psi[24], u[18];
+#pragma unroll
+    for (int i = 0; i < 24; ++i) acc[i] = 0;
+    // neighbour across the face in direction mu (dir = +1 / -1): its block id and local index
+#define DDAMG_BXHOP(MU)                                                                              \
+    {                                                                                                \
+        const bool t_edge_f = MU == 3 && apbc && ct == sg.nb[3] - 1;                                 \
+        const bool t_edge_b = MU == 3 && apbc && ct == 0;                                            \
+        if (l[MU] == sg.B[MU] - 1) {                                                                 \
+            int cn[4] = { c[0], c[1], c[2], c[3] }, ln[4] = { l[0], l[1], l[2], l[3] };              \
+            cn[MU] = c[MU] + 1 == sg.nb[MU] ? 0 : c[MU] + 1;                                         \
+            ln[MU] = 0;                                                                              \
+            const size_t nbid = (size_t)cn[0] + (size_t)sg.nb[0] * (cn[1] + (size_t)sg.nb[1] * (cn[2] + (size_t)sg.nb[2] * cn[3])); \
+            const int nlcb = (ln[0] >> 1) + sg.Bxh * (ln[1] + sg.B[1] * (ln[2] + sg.B[2] * ln[3]));  \
+            load_spinor<T>(e_in + nbid * 24 * n, n, nlcb, psi);                                      \
+            const T* lk = blk_links + (bid * 8 + parity * 4 + MU) * RECON * n;                       \
+            if (RECON == 12) load_link12(lk, n, lcb, t_edge_f ? (T)-1 : (T)1, u);                    \
+            else load_link(lk, n, lcb, u);                                                           \
+            hop_dir<MU, true>(psi, u, acc);                                                          \
+        }                                                                                            \
+        if (l[MU] == 0) {                                                                            \
+            int cn[4] = { c[0], c[1], c[2], c[3] }, ln[4] = { l[0], l[1], l[2], l[3] };              \
+            cn[MU] = c[MU] == 0 ? sg.nb[MU] - 1 : c[MU] - 1;                                         \
+            ln[MU] = sg.B[MU] - 1;                                                                   \
+            const size_t nbid = (size_t)cn[0] + (size_t)sg.nb[0] * (cn[1] + (size_t)sg.nb[1] * (cn[2] + (size_t)sg.nb[2] * cn[3])); \
+            const int nlcb = (ln[0] >> 1) + sg.Bxh * (ln[1] + sg.B[1] * (ln[2] + sg.B[2] * ln[3]));  \
+            load_spinor<T>(e_in + nbid * 24 * n, n, nlcb, psi);                                      \
+            const T* lk = blk_links + (nbid * 8 + (1 - parity) * 4 + MU) * RECON * n;                \
+            if (RECON == 12) load_link12(lk, n, nlcb, t_edge_b ? (T)-1 : (T)1, u);                   \
+            else load_link(lk, n, nlcb, u);                                                          \
+            hop_dir<MU, false>(psi, u, acc);                                                         \
+        }                                                                                            \
+    }
+    DDAMG_BXHOP(0)
+    DDAMG_BXHOP(1)
+    DDAMG_BXHOP(2)
+    DDAMG_BXHOP(3)
+#undef DDAMG_BXHOP
+    T* r = (parity ? r_o : r_e) + bid * 24 * n;
+    T v[24];
+    load_spinor<T, true>(r, n, lcb, v);
+#pragma unroll
+    for (int i = 0; i < 24; ++i) v[i] = vfma((T)0.5, acc[i], v[i]);          // r - H e,  H = -1/2 acc
+    store_spinor<T>(r, n, lcb, v);
+}
+
+template <typename T>
+void launch_sap_boundary_blocked(const Geom& g, const SapGeom& sg, int recon, int target, int apbc, const void* blk_links,
+                                 const void* e_e, const void* e_o, void* r_e, void* r_o, cudaStream_t st)
+{
+    const int grid = sg.nbxh * sg.nb[1] * sg.nb[2] * sg.nb[3];          // blocks of one colour
+    const int threads = (2 * sg.Vbh + 31) / 32 * 32;
+    if (recon == 12)
+        sap_boundary_blocked_kernel<T, 12><<<grid, threads, 0, st>>>(g, sg, target, apbc, (const T*)blk_links, (const T*)e_e,
+                                                                     (const T*)e_o, (T*)r_e, (T*)r_o);
+    else
+        sap_boundary_blocked_kernel<T, 18><<<grid, threads, 0, st>>>(g, sg, target, apbc, (const T*)blk_links, (const T*)e_e,
+                                                                     (const T*)e_o, (T*)r_e, (T*)r_o);
+}
+template void launch_sap_boundary_blocked<float>(const Geom&, const SapGeom&, int, int, int, const void*, const void*, const void*,
+                                                 void*, void*, cudaStream_t);
+template void launch_sap_boundary_blocked<double>(const Geom&, const SapGeom&, int, int, int, const void*, const void*, const void*,
+                                                  void*, void*, cudaStream_t);
 
 // ---- incremental residual (Alg. 1 lines 2 / 7 after the first evaluation): for every site of colour `target`
 //   rn(x) = r(x) - sum over the neighbours y of x in OTHER blocks of H_xy e(y)

@@ -54,6 +54,32 @@ def test_sap_matches_oracle(cfg, prec, L, T, block, n, m):
     assert all(abs(a - r) <= tol_h * r for a, r in zip(h0, h0_ref))
 
 
+@pytest.mark.parametrize("cfg,prec,L,T,block", [
+    (4, "f32", 8, 8, (4, 4, 4, 4)),
+    (3, "f32", 8, 16, (4, 2, 4, 4)),
+    (1, "f64", 4, 8, (2, 2, 2, 4)),
+])
+def test_sap_block_ordered_and_native_residual_storage_agree(cfg, prec, L, T, block):
+    """Option "sap_blocked": r and e kept block-ordered (default) or as native half spinors.  Same arithmetic per
+    site, so the iterate is bit-identical; only the summation order of the history norms differs."""
+    p = make_pair(cfg, prec, L, T)
+    _, b_d = p.spinor(9100 + cfg)
+    _, x_d = p.spinor(9150 + cfg)
+    b_e, b_o = p.ctx.pack(b_d)
+    out = {}
+    for mode in (1, 0):
+        p.ctx.set_option("sap_blocked", mode)
+        for zero_init in (False, True):
+            x_e, x_o = p.ctx.pack(x_d)
+            hist = p.ctx.sap(b_e, b_o, x_e, x_o, 2, 3, block, zero_init=zero_init, history=True)
+            out[(mode, zero_init)] = (x_e, x_o, hist)
+    p.ctx.set_option("sap_blocked", 1)
+    for zero_init in (False, True):
+        a, b = out[(1, zero_init)], out[(0, zero_init)]
+        assert torch.equal(a[0], b[0]) and torch.equal(a[1], b[1])
+        assert all(abs(u - v) <= (1e-13 if p.f64 else 1e-6) * v for u, v in zip(a[2], b[2]))
+
+
 def test_sap_smooths_and_m0_is_identity():
     """SAP(n, 4) reduces the residual every iteration; SAP(n, 0) leaves x untouched."""
     p = make_pair(4, "f32", 8, 8)
