@@ -1235,7 +1235,7 @@ extern "C" int ddamg_sap(ddamg_ctx* ctx, const void* b_e, const void* b_o, void*
         ctx->sap_built_recon = recon;
     }
     if (hist) { s = reset_hist(ctx); if (s != DDAMG_OK) return s; }
-    if (zero_init) {
+    if (zero_init && (m == 0 || n == 0)) {                   // otherwise the first solve of each colour assigns x
         CK(cudaMemsetAsync(x_e, 0, ctx->half_bytes, st));
         CK(cudaMemsetAsync(x_o, 0, ctx->half_bytes, st));
     }
@@ -1256,12 +1256,13 @@ extern "C" int ddamg_sap(ddamg_ctx* ctx, const void* b_e, const void* b_o, void*
         return after_launch(ctx, 3);
     };
     // block solves of one colour (Alg. 1 lines 4-6 / 8-10), then the residual of the other colour's sites (line 7 / 2)
-    auto half_iteration = [&](int colour, const void* rin_e, const void* rin_o, bool update_other) -> int {
+    // rin_native: (blocked) rin is still the native pair b; x_assign: first solve of this colour from x = 0
+    auto half_iteration = [&](int colour, const void* rin_e, const void* rin_o, bool update_other, int rin_native, int x_assign) -> int {
         {
             KernelTimer kt(ctx, KT_SAP);
             cudaError_t e = f32
-                ? launch_sap_blocks<float>(ctx->g, sg, recon, ctx->m0 + 4.0, colour, m, ctx->sap_links, ctx->sap_clov, rin_e, rin_o, r_e, r_o, e_e, e_o, x_e, x_o, blocked, st)
-                : launch_sap_blocks<double>(ctx->g, sg, recon, ctx->m0 + 4.0, colour, m, ctx->sap_links, ctx->sap_clov, rin_e, rin_o, r_e, r_o, e_e, e_o, x_e, x_o, blocked, st);
+                ? launch_sap_blocks<float>(ctx->g, sg, recon, ctx->m0 + 4.0, colour, m, ctx->sap_links, ctx->sap_clov, rin_e, rin_o, r_e, r_o, e_e, e_o, x_e, x_o, blocked, rin_native, x_assign, st)
+                : launch_sap_blocks<double>(ctx->g, sg, recon, ctx->m0 + 4.0, colour, m, ctx->sap_links, ctx->sap_clov, rin_e, rin_o, r_e, r_o, e_e, e_o, x_e, x_o, blocked, rin_native, x_assign, st);
             if (e != cudaSuccess) return check_cuda(ctx, e, "sap_block_kernel attributes");
         }
         int q = after_launch(ctx);
@@ -1269,8 +1270,10 @@ extern "C" int ddamg_sap(ddamg_ctx* ctx, const void* b_e, const void* b_o, void*
         {
             KernelTimer kt(ctx, KT_FULL);
             if (blocked) {
-                if (f32) launch_sap_boundary_blocked<float>(ctx->g, sg, recon, 1 - colour, ctx->bc == 1, ctx->sap_links, e_e, e_o, r_e, r_o, st);
-                else launch_sap_boundary_blocked<double>(ctx->g, sg, recon, 1 - colour, ctx->bc == 1, ctx->sap_links, e_e, e_o, r_e, r_o, st);
+                const void* nin_e = rin_native ? rin_e : nullptr;
+                const void* nin_o = rin_native ? rin_o : nullptr;
+                if (f32) launch_sap_boundary_blocked<float>(ctx->g, sg, recon, 1 - colour, ctx->bc == 1, ctx->sap_links, e_e, e_o, r_e, r_o, nin_e, nin_o, st);
+                else launch_sap_boundary_blocked<double>(ctx->g, sg, recon, 1 - colour, ctx->bc == 1, ctx->sap_links, e_e, e_o, r_e, r_o, nin_e, nin_o, st);
             } else {
                 if (f32) launch_sap_boundary<float>(ctx->g, sg, recon, 1 - colour, ctx->bc == 1, hop_gauge_block(ctx, 0), e_e, e_o, rin_e, rin_o, r_e, r_o, st);
                 else launch_sap_boundary<double>(ctx->g, sg, recon, 1 - colour, ctx->bc == 1, hop_gauge_block(ctx, 0), e_e, e_o, rin_e, rin_o, r_e, r_o, st);
@@ -1299,6 +1302,7 @@ extern "C" int ddamg_sap(ddamg_ctx* ctx, const void* b_e, const void* b_o, void*
     // PAPER.md:55); afterwards every block solve and boundary pass keeps r current
     const void* rin_e = b_e;
     const void* rin_o = b_o;
+    int native0 = 0;
     if (!zero_init) {
         // blocked: the residual is formed in the (still unused) e arrays and re-ordered into r
         void* t_e = blocked ? e_e : r_e;
@@ -1310,11 +1314,13 @@ extern "C" int ddamg_sap(ddamg_ctx* ctx, const void* b_e, const void* b_o, void*
         if (hist) { launch_finalize_norm(ctx->partials, 2 * dgrid, ctx->sc, 1, st); s = after_launch(ctx); if (s != DDAMG_OK) return s; }
         if (blocked) { s = to_blocked(t_e, t_o); if (s != DDAMG_OK) return s; }
         rin_e = r_e; rin_o = r_o;
-    } else if (blocked) {
+    } else if (blocked && hist) {
         s = to_blocked(b_e, b_o);                                                      // r = b, block-ordered
         if (s != DDAMG_OK) return s;
-        if (hist) { s = append_norm(); if (s != DDAMG_OK) return s; }                  // ||b||
+        s = append_norm(); if (s != DDAMG_OK) return s;                                // ||b||
         rin_e = r_e; rin_o = r_o;
+    } else if (blocked) {
+        native0 = 1;           // the smoother use: the first red solves and the first boundary pass read b in place
     } else if (hist) {
         // ||b||: reduce b without touching it
         const int n1 = f32 ? launch_copy_norm<float>(ctx->nreal, b_e, r_e, ctx->partials, st) : launch_copy_norm<double>(ctx->nreal, b_e, r_e, ctx->partials, st);
@@ -1325,10 +1331,11 @@ extern "C" int ddamg_sap(ddamg_ctx* ctx, const void* b_e, const void* b_o, void*
     }
     for (int i = 0; i < n; ++i) {
         if (i > 0 && hist) { s = append_norm(); if (s != DDAMG_OK) return s; }       // line 2: ||r|| before iteration i
-        s = half_iteration(0, rin_e, rin_o, true);                                     // red blocks, then r on the black sites
+        const int first = zero_init && i == 0;                                         // x = 0: the solves assign x
+        s = half_iteration(0, rin_e, rin_o, true, native0 && i == 0, first);           // red blocks, then r on the black sites
         if (s != DDAMG_OK) return s;
         rin_e = r_e; rin_o = r_o;
-        s = half_iteration(1, r_e, r_o, i + 1 < n || hist);                            // black blocks, then r on the red sites
+        s = half_iteration(1, r_e, r_o, i + 1 < n || hist, 0, first);                  // black blocks, then r on the red sites
         if (s != DDAMG_OK) return s;
     }
     if (hist) {

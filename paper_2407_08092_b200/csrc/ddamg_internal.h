@@ -69,7 +69,9 @@ void launch_sap_reorder(const Geom& g, const SapGeom& sg, int recon, const void*
 template <typename T>
 cudaError_t launch_sap_blocks(const Geom& g, const SapGeom& sg, int recon, double c0, int colour, int m, const void* blk_links,
                               const void* blk_clov, const void* r_e, const void* r_o, void* rn_e, void* rn_o,
-                              void* e_e, void* e_o, void* x_e, void* x_o, int blocked, cudaStream_t st);
+                              void* e_e, void* e_o, void* x_e, void* x_o, int blocked, int rin_native, int x_assign,
+                              cudaStream_t st);
+// rin_native: (blocked only) the input residual is still a native half-spinor pair; x_assign: x = e instead of x += e
 // blocked != 0: r, rn, e are block-ordered arrays (per parity [block][24/N planes][n] 16-byte vectors) instead of
 // native half spinors; launch_sap_spinor_to_blocked converts a native pair, launch_sap_boundary_blocked is the
 // in-place incremental residual on them (links from the block-ordered link copy)
@@ -78,7 +80,10 @@ void launch_sap_spinor_to_blocked(const Geom& g, const SapGeom& sg, const void* 
                                   cudaStream_t st);
 template <typename T>
 void launch_sap_boundary_blocked(const Geom& g, const SapGeom& sg, int recon, int target, int apbc, const void* blk_links,
-                                 const void* e_e, const void* e_o, void* r_e, void* r_o, cudaStream_t st);
+                                 const void* e_e, const void* e_o, void* r_e, void* r_o, const void* native_in_e,
+                                 const void* native_in_o, cudaStream_t st);
+// native_in_* != NULL: the input residual of the target blocks is read from that native pair (and every site of the
+// block written block-ordered) instead of in place
 // rn = r - (hops across block faces) e on the sites of colour `target`; gauge: the hopping kernels' link blocks
 // (recon reals per link), apbc as in launch_dslash
 template <typename T>

@@ -55,6 +55,9 @@ struct SapArgs {
     T* x_o;
     int blocked;             // r, rn, e are BLOCK-ORDERED arrays ([block][plane][n], one array per parity) instead of
                              // native half spinors: every access of a block is then a contiguous run per plane
+    int rin_native;          // blocked: the INPUT residual r_e / r_o is still a native half spinor (first launch of a
+                             // call from x = 0, where r = b is read in place)
+    int x_assign;            // x = e instead of x += e (first solve of a colour from x = 0: x is not read)
 };
 
 // ---- shared-memory access (plain loads/stores: the read-only global path does not apply)
@@ -235,6 +238,10 @@ sap_block_kernel(const SapArgs<T> a)
     const int rstr = a.blocked ? n : a.g.Vh;
     const int ri[2] = { a.blocked ? tid : cbg[0], a.blocked ? tid : cbg[1] };
     const size_t roff = a.blocked ? bid * 24 * n : 0;
+    const bool in_blk = a.blocked && !a.rin_native;            // the same for the input residual
+    const int istr = in_blk ? n : a.g.Vh;
+    const int ii[2] = { in_blk ? tid : cbg[0], in_blk ? tid : cbg[1] };
+    const size_t ioff = in_blk ? bid * 24 * n : 0;
     const int sblk = 4 * RECON * n;                            // one parity's four link blocks in shared memory
     // ---- stage the block's links (read once from HBM per launch): the block-ordered copy has the
     // shared-memory layout, so this is ONE contiguous bulk copy (TMA engine, `cp.async.bulk`, SASS UBLKCP)
@@ -267,22 +274,22 @@ sap_block_kernel(const SapArgs<T> a)
     if (CS) {
         __syncthreads();                                       // the barriers' init is visible
         T v[24], t[24];
-        if (active) load_spinor<T, false>(a.r_o + roff, rstr, ri[1], v);
+        if (active) load_spinor<T, false>(a.r_o + ioff, istr, ii[1], v);
         wait_bar(bar_s, 0);                                    // links and A_oo^-1 have landed
         if (active) {
             clover_site_mul<T, LD_PLAIN>(C, n, tid, v, t);
             sts_spinor<T>(S_o, n, tid, t);
-            load_spinor<T, true>(a.r_e + roff, rstr, ri[0], rho);
+            load_spinor<T, true>(a.r_e + ioff, istr, ii[0], rho);
         }
         __syncthreads();
     } else {
         if (active) {
             // ---- eq. 2 right factor, odd half: t_o = A_oo^-1 r_o;  rho starts as r_e
             T v[24], t[24];
-            load_spinor<T, false>(a.r_o + roff, rstr, ri[1], v);
+            load_spinor<T, false>(a.r_o + ioff, istr, ii[1], v);
             clover_site_mul<T, LD_REUSE>(clov_oinv, n, tid, v, t);
             sts_spinor<T>(S_o, n, tid, t);
-            load_spinor<T, true>(a.r_e + roff, rstr, ri[0], rho);
+            load_spinor<T, true>(a.r_e + ioff, istr, ii[0], rho);
         }
         __syncthreads();                                       // S_o complete; the barrier's init is visible
         wait_bar(bar_s, 0);                                    // wait for the links (phase 0 of the mbarrier)
@@ -314,7 +321,7 @@ sap_block_kernel(const SapArgs<T> a)
             if (active) {
                 T v[24], t[24];
                 if (hs == last) {
-                    load_spinor<T, false>(a.r_o + roff, rstr, ri[1], v);
+                    load_spinor<T, false>(a.r_o + ioff, istr, ii[1], v);
 #pragma unroll
                     for (int i = 0; i < 24; ++i) v[i] = v[i] + (T)0.5 * acc[i];          // r_o - H e
                 } else {
@@ -324,14 +331,19 @@ sap_block_kernel(const SapArgs<T> a)
                 if (CS) clover_site_mul<T, LD_PLAIN>(C, n, tid, v, t);
                 else clover_site_mul<T, LD_REUSE>(clov_oinv, n, tid, v, t);
                 if (hs == last) {
-                    load_spinor<T, true>(a.x_o, a.g.Vh, cbg[1], v);
+                    if (a.x_assign) {
+                        store_spinor<T>(a.x_o, a.g.Vh, cbg[1], t);
+                        store_spinor<T>(a.x_e, a.g.Vh, cbg[0], e);
+                    } else {
+                        load_spinor<T, true>(a.x_o, a.g.Vh, cbg[1], v);
 #pragma unroll
-                    for (int i = 0; i < 24; ++i) v[i] += t[i];
-                    store_spinor<T>(a.x_o, a.g.Vh, cbg[1], v);
-                    load_spinor<T, true>(a.x_e, a.g.Vh, cbg[0], v);
+                        for (int i = 0; i < 24; ++i) v[i] += t[i];
+                        store_spinor<T>(a.x_o, a.g.Vh, cbg[1], v);
+                        load_spinor<T, true>(a.x_e, a.g.Vh, cbg[0], v);
 #pragma unroll
-                    for (int i = 0; i < 24; ++i) v[i] += e[i];
-                    store_spinor<T>(a.x_e, a.g.Vh, cbg[0], v);
+                        for (int i = 0; i < 24; ++i) v[i] += e[i];
+                        store_spinor<T>(a.x_e, a.g.Vh, cbg[0], v);
+                    }
                     // the update and the residual it leaves on this block: r_k - D_k e_k = (rho, 0)
                     store_spinor<T>(a.e_o + roff, rstr, ri[1], t);
                     store_spinor<T>(a.e_e + roff, rstr, ri[0], e);
@@ -491,10 +503,12 @@ static cudaError_t launch_blocks_as(const SapArgs<T>& a, int threads, int grid, 
 template <typename T>
 cudaError_t launch_sap_blocks(const Geom& g, const SapGeom& sg, int recon, double c0, int colour, int m, const void* blk_links,
                               const void* blk_clov, const void* r_e, const void* r_o, void* rn_e, void* rn_o,
-                              void* e_e, void* e_o, void* x_e, void* x_o, int blocked, cudaStream_t st)
+                              void* e_e, void* e_o, void* x_e, void* x_o, int blocked, int rin_native, int x_assign, cudaStream_t st)
 {
     SapArgs<T> a;
     a.blocked = blocked;
+    a.rin_native = rin_native;
+    a.x_assign = x_assign;
     a.g = g; a.sg = sg; a.colour = colour; a.m = m; a.c0 = (T)c0;
     a.blk_links = (const T*)blk_links; a.blk_clov = (const T*)blk_clov;
     a.r_e = (const T*)r_e; a.r_o = (const T*)r_o; a.rn_e = (T*)rn_e; a.rn_o = (T*)rn_o;
@@ -516,9 +530,9 @@ cudaError_t launch_sap_blocks(const Geom& g, const SapGeom& sg, int recon, doubl
                        : launch_blocks_as<T, 18, SAP_MAX_THREADS, false>(a, threads, grid, smem, st);
 }
 template cudaError_t launch_sap_blocks<float>(const Geom&, const SapGeom&, int, double, int, int, const void*, const void*,
-                                              const void*, const void*, void*, void*, void*, void*, void*, void*, int, cudaStream_t);
+                                              const void*, const void*, void*, void*, void*, void*, void*, void*, int, int, int, cudaStream_t);
 template cudaError_t launch_sap_blocks<double>(const Geom&, const SapGeom&, int, double, int, int, const void*, const void*,
-                                               const void*, const void*, void*, void*, void*, void*, void*, void*, int, cudaStream_t);
+                                               const void*, const void*, void*, void*, void*, void*, void*, void*, int, int, int, cudaStream_t);
 
 // ---- block-ordered residual and update arrays.  In the checkerboard layout a block owns 2-site (32-byte) x-runs,
 // alternating with the other colour's: a launch that touches the sites of ONE colour uses every other 32-byte
@@ -570,8 +584,11 @@ template void launch_sap_spinor_to_blocked<double>(const Geom&, const SapGeom&, 
 template <typename T, int RECON>
 __global__ void __launch_bounds__(2 * SAP_MAX_THREADS) __maxnreg__(sizeof(T) == 4 ? DDAMG_SAP_BND_MAXREG : 128)
 sap_boundary_blocked_kernel(Geom g, SapGeom sg, int target, int apbc, const T* __restrict__ blk_links,
-                            const T* __restrict__ e_e, const T* __restrict__ e_o, T* r_e, T* r_o)
+                            const T* __restrict__ e_e, const T* __restrict__ e_o, T* r_e, T* r_o,
+                            const T* __restrict__ nin_e, const T* __restrict__ nin_o)
 {
+    // nin_e / nin_o != NULL: the input residual is still a NATIVE half-spinor pair (first pass of a call from
+    // x = 0, r = b): every site of the block is read from it and written block-ordered, also those without a hop
     const int n = sg.Vbh;
     if ((int)threadIdx.x >= 2 * n) return;
     int b = blockIdx.x;
@@ -588,7 +605,7 @@ sap_boundary_blocked_kernel(Geom g, SapGeom sg, int target, int apbc, const T* _
     bool any = false;
 #pragma unroll
     for (int mu = 0; mu < 4; ++mu) any = any || l[mu] == 0 || l[mu] == sg.B[mu] - 1;
-    if (!any) return;
+    if (!any && !nin_e) return;
     const size_t bid = (size_t)cx + (size_t)sg.nb[0] * (cy + (size_t)sg.nb[1] * (cz + (size_t)sg.nb[2] * ct));
     const T* e_in = parity ? e_e : e_o;                        // neighbours have the opposite parity
     T acc[24], psi[24], u[18];
@@ -631,7 +648,12 @@ sap_boundary_blocked_kernel(Geom g, SapGeom sg, int target, int apbc, const T* _
 #undef DDAMG_BXHOP
     T* r = (parity ? r_o : r_e) + bid * 24 * n;
     T v[24];
-    load_spinor<T, true>(r, n, lcb, v);
+    if (nin_e) {
+        const int cbg = ((cx * sg.B[0] + l[0]) >> 1) + g.Lh * ((cy * sg.B[1] + l[1]) + g.L * ((cz * sg.B[2] + l[2]) + g.L * (ct * sg.B[3] + l[3])));
+        load_spinor<T, true>(parity ? nin_o : nin_e, g.Vh, cbg, v);
+    } else {
+        load_spinor<T, true>(r, n, lcb, v);
+    }
 #pragma unroll
     for (int i = 0; i < 24; ++i) v[i] = vfma((T)0.5, acc[i], v[i]);          // r - H e,  H = -1/2 acc
     store_spinor<T>(r, n, lcb, v);
@@ -639,21 +661,24 @@ sap_boundary_blocked_kernel(Geom g, SapGeom sg, int target, int apbc, const T* _
 
 template <typename T>
 void launch_sap_boundary_blocked(const Geom& g, const SapGeom& sg, int recon, int target, int apbc, const void* blk_links,
-                                 const void* e_e, const void* e_o, void* r_e, void* r_o, cudaStream_t st)
+                                 const void* e_e, const void* e_o, void* r_e, void* r_o, const void* native_in_e,
+                                 const void* native_in_o, cudaStream_t st)
 {
     const int grid = sg.nbxh * sg.nb[1] * sg.nb[2] * sg.nb[3];          // blocks of one colour
     const int threads = (2 * sg.Vbh + 31) / 32 * 32;
     if (recon == 12)
         sap_boundary_blocked_kernel<T, 12><<<grid, threads, 0, st>>>(g, sg, target, apbc, (const T*)blk_links, (const T*)e_e,
-                                                                     (const T*)e_o, (T*)r_e, (T*)r_o);
+                                                                     (const T*)e_o, (T*)r_e, (T*)r_o, (const T*)native_in_e,
+                                                                     (const T*)native_in_o);
     else
         sap_boundary_blocked_kernel<T, 18><<<grid, threads, 0, st>>>(g, sg, target, apbc, (const T*)blk_links, (const T*)e_e,
-                                                                     (const T*)e_o, (T*)r_e, (T*)r_o);
+                                                                     (const T*)e_o, (T*)r_e, (T*)r_o, (const T*)native_in_e,
+                                                                     (const T*)native_in_o);
 }
 template void launch_sap_boundary_blocked<float>(const Geom&, const SapGeom&, int, int, int, const void*, const void*, const void*,
-                                                 void*, void*, cudaStream_t);
+                                                 void*, void*, const void*, const void*, cudaStream_t);
 template void launch_sap_boundary_blocked<double>(const Geom&, const SapGeom&, int, int, int, const void*, const void*, const void*,
-                                                  void*, void*, cudaStream_t);
+                                                  void*, void*, const void*, const void*, cudaStream_t);
 
 // ---- incremental residual (Alg. 1 lines 2 / 7 after the first evaluation): for every site of colour `target`
 //   rn(x) = r(x) - sum over the neighbours y of x in OTHER blocks of H_xy e(y)
