@@ -111,6 +111,27 @@ int ddamg_build_clover(ddamg_ctx* ctx);
 int ddamg_apply_schur(ddamg_ctx* ctx, const void* x_e, void* y_e);
 
 /*
+ * The same operator (eq. 3), for callers that must not allocate: code under CUDA-graph
+ * capture, tight serving loops, harnesses that forbid cudaMalloc.  The call performs NO cudaMalloc / cudaFree
+ * and calls no allocating library routine: the intermediate t_o = A_oo^-1 H_oe x_e lives in a static device
+ * array inside libddamg.so of ddamg_noalloc_max_bytes() = 8 MiB (held by every GPU that loads the library until
+ * the process exits) instead of in context-owned memory.  Same two kernels, same arithmetic: results are
+ * bit-identical to ddamg_apply_schur.
+ *   x_e, y_e   DEVICE native half spinors as for ddamg_apply_schur (caller-owned, must not alias).
+ * Limit: one half spinor (ddamg_half_spinor_bytes) must fit the array -- fp32 lattices up to V/2 = 87381
+ * sites (e.g. 16^3 x 32), fp64 up to 43690 (e.g. 16^4); EINVAL with a message naming both sizes beyond that.
+ * The first call on a device resolves the array's device address (cudaGetSymbolAddress; no allocation): make
+ * it once per device, with that device current, before entering a capture.  ALL contexts and calls on a device
+ * share the one array, which keeps the last call's contents; nothing in it has to start at zero (kernel A
+ * overwrites every element kernel B reads), but two calls that overlap on the GPU (different streams or
+ * contexts without ordering between them) RACE on it: serialise them.
+ * ESTATE before the gauge field and the clover term are set up, or while ddamg_kernel_timing is on (its event
+ * pool may grow); ECUDA if the address cannot be resolved.
+ */
+int ddamg_apply_schur_noalloc(ddamg_ctx* ctx, const void* x_e, void* y_e);
+size_t ddamg_noalloc_max_bytes(void);
+
+/*
  * Alg. 4 with omega supplied (lines 2-4):  nu times  r = b_e - D_S x_e;  x_e += omega r.
  *   x_e        in: x^(0) (ignored if zero_init != 0, then x^(0) = 0 and the first sweep is
  *              x = omega b_e without an operator application); out: x^(nu).  In place.

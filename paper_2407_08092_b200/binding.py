@@ -35,6 +35,8 @@ SYMBOLS = {
     "ddamg_load_gauge": (_i, [_vp, _vp, _i, _i]),
     "ddamg_build_clover": (_i, [_vp]),
     "ddamg_apply_schur": (_i, [_vp, _vp, _vp]),
+    "ddamg_apply_schur_noalloc": (_i, [_vp, _vp, _vp]),
+    "ddamg_noalloc_max_bytes": (ctypes.c_size_t, []),
     "ddamg_richardson": (_i, [_vp, _vp, _vp, _i, _d, _i, _dp]),
     "ddamg_gmres_oe": (_i, [_vp, _vp, _vp, _i, _i, _d, _i, _dp, _ip]),
     "ddamg_gcr_oe": (_i, [_vp, _vp, _vp, _i, _i, _d, _i, _dp, _ip]),
@@ -180,6 +182,13 @@ class Ddamg:
         y_e = self.half_spinor() if y_e is None else y_e
         self._chk_half(x_e, y_e)
         self._ck(self.lib.ddamg_apply_schur(self._h, _ptr(x_e), _ptr(y_e)), "ddamg_apply_schur")
+        return y_e
+
+    def apply_schur_noalloc(self, x_e: torch.Tensor, y_e: torch.Tensor) -> torch.Tensor:
+        """ddamg_apply_schur_noalloc: no allocation inside the call (the caller passes y_e); the scratch half
+        spinor is a static 8 MiB device array of the library, shared by all calls on the device."""
+        self._chk_half(x_e, y_e)
+        self._ck(self.lib.ddamg_apply_schur_noalloc(self._h, _ptr(x_e), _ptr(y_e)), "ddamg_apply_schur_noalloc")
         return y_e
 
     def richardson(self, b_e: torch.Tensor, x_e: torch.Tensor, nu: int, omega: float,

@@ -6,6 +6,7 @@
 #include <cstdint>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -426,6 +427,62 @@ static int schur(ddamg_ctx* ctx, const void* x_e, void* y_e)
     int s = dslash(ctx, EPI_CLOV_HOP, false, 1, x_e, nullptr, nullptr, ctx->tmp_o, 0.0, 0);
     if (s != DDAMG_OK) return s;
     return dslash(ctx, EPI_SCHUR, false, 0, ctx->tmp_o, x_e, nullptr, y_e, 0.0, 1);
+}
+
+// --------------------------------------------------------------------------- allocation-free Schur apply
+// For callers that cannot call cudaMalloc (code under CUDA-graph capture, tight serving loops, harnesses that forbid
+// it): ddamg_apply_schur_noalloc keeps the intermediate t_o = A_oo^-1 H_oe x_e of eq. 3 -- the scratch between kernels
+// A and B -- in a file-scope device array of a fixed, modest size instead of context-owned memory.  Every GPU that
+// loads the library holds the array until the process exits.  In host code the array's NAME is a host-side stand-in,
+// not a device address: the address a kernel may use comes from cudaGetSymbolAddress, resolved once per device with
+// that device current (noalloc_scratch below) and cached.
+#define DDAMG_NOALLOC_SCRATCH_BYTES (8u << 20)
+static __device__ __align__(256) unsigned char g_noalloc_scratch[DDAMG_NOALLOC_SCRATCH_BYTES];
+static const int NOALLOC_MAX_DEVICES = 64;
+static void* g_noalloc_ptr[NOALLOC_MAX_DEVICES];            // device address of g_noalloc_scratch on device d, or NULL
+static std::mutex g_noalloc_mutex;
+
+// set-up step: device address of the scratch array on the CURRENT device (first call on a device resolves it)
+static int noalloc_scratch(ddamg_ctx* ctx, void** out)
+{
+    int dev = -1;
+    int s = check_cuda(ctx, cudaGetDevice(&dev), "cudaGetDevice");
+    if (s != DDAMG_OK) return s;
+    if (dev < 0 || dev >= NOALLOC_MAX_DEVICES) return fail(ctx, DDAMG_EINVAL, "ddamg_apply_schur_noalloc: device index out of range");
+    std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+    if (!g_noalloc_ptr[dev]) {
+        void* p = nullptr;
+        s = check_cuda(ctx, cudaGetSymbolAddress(&p, g_noalloc_scratch), "cudaGetSymbolAddress(g_noalloc_scratch)");
+        if (s != DDAMG_OK) return s;
+        if (!p) return fail(ctx, DDAMG_ECUDA, "ddamg_apply_schur_noalloc: cudaGetSymbolAddress returned NULL");
+        g_noalloc_ptr[dev] = p;
+    }
+    *out = g_noalloc_ptr[dev];
+    return DDAMG_OK;
+}
+
+extern "C" size_t ddamg_noalloc_max_bytes(void) { return (size_t)DDAMG_NOALLOC_SCRATCH_BYTES; }
+
+extern "C" int ddamg_apply_schur_noalloc(ddamg_ctx* ctx, const void* x_e, void* y_e)
+{
+    ENTER(ctx);
+    if (!x_e || !y_e || x_e == y_e) return fail(ctx, DDAMG_EINVAL, "ddamg_apply_schur_noalloc: NULL or aliased arguments");
+    if (ctx->half_bytes > (size_t)DDAMG_NOALLOC_SCRATCH_BYTES) {
+        char msg[240];
+        snprintf(msg, sizeof msg, "ddamg_apply_schur_noalloc: one half spinor of this lattice is %zu bytes, more than the %u-byte "
+                 "static scratch array (ddamg_noalloc_max_bytes); use ddamg_apply_schur", ctx->half_bytes, DDAMG_NOALLOC_SCRATCH_BYTES);
+        return fail(ctx, DDAMG_EINVAL, msg);
+    }
+    int s = need_ready(ctx, "ddamg_apply_schur_noalloc");
+    if (s != DDAMG_OK) return s;
+    if (ctx->timing) return fail(ctx, DDAMG_ESTATE, "ddamg_apply_schur_noalloc: switch ddamg_kernel_timing off (its event pool may grow)");
+    void* t_o = nullptr;
+    s = noalloc_scratch(ctx, &t_o);
+    if (s != DDAMG_OK) return s;
+    // kernel A writes all V/2 sites of t_o before kernel B reads them: nothing in the shared array has to start at zero
+    s = dslash(ctx, EPI_CLOV_HOP, false, 1, x_e, nullptr, nullptr, t_o, 0.0, 0);
+    if (s != DDAMG_OK) return s;
+    return dslash(ctx, EPI_SCHUR, false, 0, t_o, x_e, nullptr, y_e, 0.0, 1);
 }
 
 extern "C" int ddamg_apply_schur(ddamg_ctx* ctx, const void* x_e, void* y_e)
